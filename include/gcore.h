@@ -1,0 +1,189 @@
+/* gcore.h -- C ABI of the RLHF scoring hot path for one NVIDIA B200 (sm_100a).
+ *
+ * The path is stages 3 and 4 of the 4-stage RLHF workflow of G-Core (arxiv 2507.22789):
+ *   stage 3 "the policy and reference policy computes their reference log probabilities"
+ *           (sec 2.2), run data-parallel on all GPUs (sec 3.2);
+ *   stage 4 "The actor ... trained on the batch ... and the loss function", for
+ *           GRPO, the algorithm the paper names as typical (sec 2.3);
+ *   the dynamic-sampling group filter of PAPER.md:150 (sec 3.2).
+ * The paper prints no formula; the arithmetic is BASELINE.json:north_star, restated step by
+ * step in SURVEY.md sec 8(c) and DESIGN.md sec 2.  Notation: T packed tokens, D hidden, V vocab,
+ * R responses, G groups; H[T,D] hidden states, W[V,D] LM-head weight (logits = H W^T / tau),
+ * y[T] target ids, m[T] response mask.
+ *
+ * Conventions (all entry points)
+ *   - Every pointer is a DEVICE pointer owned by the caller unless the name ends in "_host".
+ *     The library never allocates, frees or keeps memory; scratch comes from `workspace`
+ *     (size from gc_workspace_bytes; 256-byte aligned).
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and
+ *     return without synchronising.  Inputs must stay alive until the stream has passed the call.
+ *   - Return value is a gc_status.  Host-checkable errors are reported before any launch.  No
+ *     exceptions, no abort(), no global mutable state, no environment variables.
+ *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
+ *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
+ *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V
+ *     is a caller error (undefined result for that row; use gc_validate_targets to check).
+ *   - Outputs at unscored rows are exactly 0 (logp, entropy, lse, rows of dH).
+ *   - Same inputs give bit-identical outputs from run to run (no floating-point atomics).
+ */
+#ifndef GCORE_H_
+#define GCORE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GC_OK = 0,
+  GC_ERR_NULL = 1,      /* a required pointer is NULL */
+  GC_ERR_SHAPE = 2,     /* T, D, V, R, G out of range; ld < D; D not supported by this dtype */
+  GC_ERR_DTYPE = 3,     /* unknown gc_dtype */
+  GC_ERR_ALIGN = 4,     /* pointer or ld alignment */
+  GC_ERR_WORKSPACE = 5, /* workspace NULL or smaller than gc_workspace_bytes */
+  GC_ERR_ARG = 6,       /* temperature <= 0, clip < 0, eps < 0, bad enum */
+  GC_ERR_ARCH = 7,      /* current device is not compute capability 10.x */
+  GC_ERR_CUDA = 8       /* a CUDA runtime/driver call failed (launch configuration etc.) */
+} gc_status;
+
+typedef enum {
+  GC_F32 = 0,       /* H, W, dH fp32; plain SIMT kernels (BASELINE.json configs[0]) */
+  GC_BF16 = 1,      /* H, W, dH bf16, fp32 accumulation; tcgen05/TMEM/TMA kernels */
+  GC_BF16_SIMT = 2  /* bf16 operands through the SIMT kernels: slow cross-check path */
+} gc_dtype;
+
+typedef enum {
+  GC_AGG_TOKEN_MEAN = 0, /* loss = sum_t m_t l_t / max(sum_t m_t, 1)           (default) */
+  GC_AGG_SEQ_MEAN = 1    /* loss = mean over responses of per-response token means        */
+} gc_agg;
+
+typedef enum { GC_OP_LOGPROBS = 0, GC_OP_LOSS_FWD = 1, GC_OP_LOSS_BWD = 2 } gc_op;
+
+/* Static string for a gc_status (never NULL). */
+const char* gc_status_string(int status);
+
+/* Library version (major*10000 + minor*100 + patch). */
+int gc_version(void);
+
+/* Bytes of workspace the given op needs for these shapes.  chunk_tokens is the backward's
+ * T-chunk (rows of the dS buffer); 0 lets the library pick.
+ * Returns 0 on invalid arguments. */
+size_t gc_workspace_bytes(int op, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens);
+
+/* ---- stage 3: token log-probs + entropy (north_star: "fused LM-head contraction H.W^T over
+ * the vocabulary, then an online (chunked, never materialised) log-softmax, then a gather of
+ * the sampled token's log-prob and the per-token entropy").
+ *   z[t,v]     = (sum_d H[t,d] W[v,d]) / temperature
+ *   lse[t]     = ln sum_v exp z[t,v];   logp[t] = z[t,y_t] - lse[t]
+ *   entropy[t] = -sum_v p ln p,  p = exp(z - lse)                      (natural log)
+ * H [T,D] (ldH), W [V,D] (ldW) of `dtype`; targets [T] int32; mask [T] uint8 or NULL (= all 1).
+ * logp [T] f32 required; entropy, lse [T] f32 nullable.  The [T,V] logits are never stored. */
+int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                      const int32_t* targets, const uint8_t* mask,
+                      int64_t T, int64_t D, int64_t V, float temperature,
+                      float* logp, float* entropy, float* lse,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Same computation with the per-step inputs and outputs in HOST memory (pinned for async
+ * copies): H_host [T,D] dense, targets_host, mask_host (nullable) are copied to the device,
+ * logp_host / entropy_host (nullable) are copied back, all on `cuda_stream`, staged in
+ * `workspace` (gc_workspace_bytes(GC_OP_LOGPROBS,...) + gc_host_staging_bytes(T, D, dtype)).
+ * W is model state and stays a device pointer.  Used for the end-to-end measurement. */
+size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype);
+int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int dtype,
+                           const int32_t* targets_host, const uint8_t* mask_host,
+                           int64_t T, int64_t D, int64_t V, float temperature,
+                           float* logp_host, float* entropy_host,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- group filter + GRPO advantages ("filter out prompts with the accuracy
+ * equal to 1 and 0"; north_star "GRPO group-normalised advantages"; steps 4-5).
+ *   keep[g] = 0 iff all rewards of group g are equal (exact float compare)
+ *   A_i     = (r_i - mean_g) / (std_g + eps)
+ * rewards [R] f32; group_offsets [G+1] int32, ascending, group g = responses
+ * [group_offsets[g], group_offsets[g+1]), R = group_offsets[G] (read on the device).
+ * unbiased_std: 0 population std (default), 1 sample std (n-1).  drop_constant_groups: 1 ->
+ * constant groups get A = 0 and keep = 0; 0 -> keep = 1 everywhere (A = 0 for constant groups
+ * follows from eps > 0).  adv [R] f32; keep [G] uint8 nullable. */
+int gc_grpo_advantages(const float* rewards, const int32_t* group_offsets, int32_t G,
+                       float eps, int unbiased_std, int drop_constant_groups,
+                       float* adv, uint8_t* keep, void* cuda_stream);
+
+/* ---- stage 4 forward: log-probs as above, then the GRPO loss (north_star: "clipped-ratio
+ * policy loss with a k3 KL penalty against the reference"; steps 6-7).  Per scored token t of
+ * response r (cu_seqlens[r] <= t < cu_seqlens[r+1]):
+ *   rho = exp(logp - old_logp);  s = min(rho A_r, clip(rho, 1-clip_lo, 1+clip_hi) A_r)
+ *   d = ref_logp - logp;  k3 = exp(d) - d - 1;  l = -s + beta k3
+ * cu_seqlens [R+1] int32 with cu_seqlens[0] = 0, cu_seqlens[R] = T.  adv [R].  old_logp [T];
+ * ref_logp [T], nullable iff beta == 0.  out5 [5] f32 on the device:
+ *   {loss, pg_loss, kl_mean, clip_frac, n_scored}; loss = pg_loss + beta kl_mean (both use
+ *   `agg`), clip_frac = clipped scored tokens / n_scored.
+ * logp and lse [T] are required (the backward needs them); entropy nullable. */
+int gc_grpo_loss_fwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                     const int32_t* targets, const uint8_t* mask,
+                     int64_t T, int64_t D, int64_t V, float temperature,
+                     const int32_t* cu_seqlens, int32_t R, const float* adv,
+                     const float* old_logp, const float* ref_logp,
+                     float clip_lo, float clip_hi, float beta, int agg,
+                     float* out5, float* logp, float* entropy, float* lse,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- stage 4 backward (north_star: "The backward pass recomputes each logit chunk to produce
+ * dH and dW without storing [T,V] logits"; steps 8-9).  Takes the forward's logp and lse.
+ *   g_t     = grad_loss * d loss / d logp_t
+ *   dz[t,v] = g_t (1[v = y_t] - exp(z[t,v] - lse[t]))
+ *   dH[t,:] = (1/tau) sum_v dz[t,v] W[v,:]        dW[v,:] (+)= (1/tau) sum_t dz[t,v] H[t,:]
+ * dH [T,D] (lddH) in H's dtype, zero rows at unscored tokens.  dW [V,D] (lddW) of dW_dtype
+ * (GC_F32 only for now); accumulate_dW != 0 adds to the existing contents.  chunk_tokens: rows
+ * of the bf16 dS chunk buffer (0 = library picks; must match gc_workspace_bytes). */
+int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                     const int32_t* targets, const uint8_t* mask,
+                     int64_t T, int64_t D, int64_t V, float temperature,
+                     const int32_t* cu_seqlens, int32_t R, const float* adv,
+                     const float* old_logp, const float* ref_logp,
+                     float clip_lo, float clip_hi, float beta, int agg,
+                     const float* logp, const float* lse, float grad_loss,
+                     void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
+                     int accumulate_dW, int64_t chunk_tokens,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- helpers ---- */
+/* Debug: synchronises the stream; *n_bad_host = number of scored tokens with target >= V. */
+int gc_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
+                        int64_t* n_bad_host, void* cuda_stream);
+
+/* Row selection: rows[0..n) = ascending indices of scored tokens,
+ * *n_rows (device int32) = n; if Hs != NULL also gathers H[rows[i],:] into Hs[i,:] (dense,
+ * ld = D).  Exposed for tests and the HBM-roofline measurement; the entry points above call
+ * the same kernels internally.  workspace: gc_workspace_bytes(GC_OP_LOGPROBS, ...). */
+int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* targets,
+                    const uint8_t* mask, int64_t T, int64_t D,
+                    int32_t* rows, int32_t* n_rows, void* Hs,
+                    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* The loss kernels alone on given log-probs (steps 6-8): out5 as in gc_grpo_loss_fwd;
+ * g [T] nullable (d loss / d logp * grad_loss).  Exposed for tests and for the HBM-roofline
+ * measurement of the elementwise kernels on a scaled-up stand-in.
+ * workspace: gc_workspace_bytes(GC_OP_LOSS_FWD, T, 8, 8, GC_F32, 0) is always enough. */
+int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
+                       const int32_t* targets, const uint8_t* mask, int64_t T,
+                       const int32_t* cu_seqlens, int32_t R, const float* adv,
+                       float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
+                       float* out5, float* g,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Plain bf16 GEMM on the library's tcgen05 main loop, for unit tests of the tile engine:
+ * C[M,N] (f32, ldc) = A . B with A given as [M,K] (a_mn_major = 0, lda >= K) or [K,M]
+ * (a_mn_major = 1, lda >= M), B as [N,K] (b_mn_major = 0) or [K,N] (b_mn_major = 1).
+ * accumulate != 0 adds to C.  cta_group is 1 or 2. */
+int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major,
+                       const void* B, int64_t ldb, int b_mn_major,
+                       float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
+                       int accumulate, int cta_group, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GCORE_H_ */

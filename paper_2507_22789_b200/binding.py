@@ -1,0 +1,281 @@
+"""Thin ctypes binding over csrc/libgcore.so (the C ABI of include/gcore.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  PyTorch
+provides device memory (tensors, the workspace) and the current stream.  There is no CPU or
+eager fallback: a missing library raises ImportError, a non-zero gc_status raises GcoreError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libgcore.so")
+
+GC_F32, GC_BF16, GC_BF16_SIMT = 0, 1, 2
+GC_AGG_TOKEN_MEAN, GC_AGG_SEQ_MEAN = 0, 1
+GC_OP_LOGPROBS, GC_OP_LOSS_FWD, GC_OP_LOSS_BWD = 0, 1, 2
+
+EXPORTS = [
+    "gc_status_string", "gc_version", "gc_workspace_bytes", "gc_token_logprobs",
+    "gc_host_staging_bytes", "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
+    "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
+    "gc_debug_gemm_bf16",
+]
+
+
+class GcoreError(RuntimeError):
+    pass
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2507_22789_b200.build` "
+            "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, i32, f32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_size_t
+    ci = C.c_int
+    lib.gc_status_string.restype = C.c_char_p
+    lib.gc_status_string.argtypes = [ci]
+    lib.gc_version.restype = ci
+    lib.gc_workspace_bytes.restype = sz
+    lib.gc_workspace_bytes.argtypes = [ci, i64, i64, i64, ci, i64]
+    head = [vp, i64, vp, i64, ci, vp, vp, i64, i64, i64, f32]
+    loss = [vp, i32, vp, vp, vp, f32, f32, f32, ci]
+    lib.gc_token_logprobs.argtypes = head + [vp, vp, vp, vp, sz, vp]
+    lib.gc_host_staging_bytes.restype = sz
+    lib.gc_host_staging_bytes.argtypes = [i64, i64, ci]
+    lib.gc_token_logprobs_host.argtypes = [vp, vp, i64, ci, vp, vp, i64, i64, i64, f32, vp, vp,
+                                           vp, sz, vp]
+    lib.gc_grpo_advantages.argtypes = [vp, vp, i32, f32, ci, ci, vp, vp, vp]
+    lib.gc_grpo_loss_fwd.argtypes = head + loss + [vp, vp, vp, vp, vp, sz, vp]
+    lib.gc_grpo_loss_bwd.argtypes = head + loss + [vp, vp, f32, vp, i64, vp, i64, ci, ci, i64,
+                                                   vp, sz, vp]
+    lib.gc_validate_targets.argtypes = [vp, vp, i64, i64, C.POINTER(i64), vp]
+    lib.gc_compact_rows.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, vp, vp, vp, sz, vp]
+    lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
+                                       f32, vp, vp, vp, sz, vp]
+    lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, vp]
+    for name in EXPORTS:
+        fn = getattr(lib, name)
+        if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes"):
+            fn.restype = ci
+    return lib
+
+
+_lib = _load()
+
+
+def lib() -> C.CDLL:
+    return _lib
+
+
+def _check(status: int):
+    if status != 0:
+        raise GcoreError(_lib.gc_status_string(status).decode())
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def dtype_code(t: torch.Tensor, simt: bool = False) -> int:
+    if t.dtype == torch.float32:
+        return GC_F32
+    if t.dtype == torch.bfloat16:
+        return GC_BF16_SIMT if simt else GC_BF16
+    raise GcoreError(f"unsupported dtype {t.dtype}")
+
+
+_ws_cache: dict = {}
+
+
+def workspace(nbytes: int, device) -> torch.Tensor:
+    """A cached device buffer of at least nbytes (torch caching allocator: 512-byte aligned)."""
+    key = str(device)
+    buf = _ws_cache.get(key)
+    if buf is None or buf.numel() < nbytes:
+        _ws_cache[key] = buf = torch.empty(max(nbytes, 1 << 20), dtype=torch.uint8, device=device)
+    return buf
+
+
+def workspace_bytes(op: int, T: int, D: int, V: int, dtype: int, chunk_tokens: int = 0) -> int:
+    return int(_lib.gc_workspace_bytes(op, T, D, V, dtype, chunk_tokens))
+
+
+def _head_args(H, W, targets, mask, tau, simt):
+    assert H.dim() == 2 and W.dim() == 2 and H.stride(1) == 1 and W.stride(1) == 1
+    T, D = H.shape
+    V = W.shape[0]
+    assert W.shape[1] == D and H.dtype == W.dtype
+    assert targets.dtype == torch.int32 and targets.numel() == T and targets.is_contiguous()
+    if mask is not None:
+        assert mask.dtype == torch.uint8 and mask.numel() == T and mask.is_contiguous()
+    dt = dtype_code(H, simt)
+    args = [_ptr(H), H.stride(0) if T > 0 else D, _ptr(W), W.stride(0), dt, _ptr(targets),
+            _ptr(mask), T, D, V, float(tau)]
+    return args, T, D, V, dt
+
+
+def gc_token_logprobs(H, W, targets, mask=None, temperature=1.0, *, want_entropy=True,
+                      want_lse=True, simt=False):
+    """-> (logp, entropy|None, lse|None), float32 [T] on H's device."""
+    args, T, D, V, dt = _head_args(H, W, targets, mask, temperature, simt)
+    dev = H.device
+    logp = torch.empty(T, dtype=torch.float32, device=dev)
+    ent = torch.empty(T, dtype=torch.float32, device=dev) if want_entropy else None
+    lse = torch.empty(T, dtype=torch.float32, device=dev) if want_lse else None
+    nb = workspace_bytes(GC_OP_LOGPROBS, T, D, V, dt)
+    ws = workspace(nb, dev)
+    _check(_lib.gc_token_logprobs(*args, _ptr(logp), _ptr(ent), _ptr(lse), _ptr(ws), ws.numel(),
+                                  _stream()))
+    return logp, ent, lse
+
+
+def gc_token_logprobs_host(H_host, W, targets_host, mask_host=None, temperature=1.0, *,
+                           logp_host=None, entropy_host=None, simt=False):
+    """Per-step inputs/outputs in (pinned) HOST memory; W on the device.  Enqueues H2D copies,
+    the kernels and D2H copies on the current stream; the caller synchronises."""
+    T, D = H_host.shape
+    V = W.shape[0]
+    dt = dtype_code(W, simt)
+    assert not H_host.is_cuda and H_host.is_contiguous() and W.is_cuda
+    if logp_host is None:
+        logp_host = torch.empty(T, dtype=torch.float32).pin_memory()
+    nb = workspace_bytes(GC_OP_LOGPROBS, T, D, V, dt) + int(_lib.gc_host_staging_bytes(T, D, dt))
+    ws = workspace(nb, W.device)
+    _check(_lib.gc_token_logprobs_host(_ptr(H_host), _ptr(W), W.stride(0), dt, _ptr(targets_host),
+                                       _ptr(mask_host), T, D, V, float(temperature),
+                                       _ptr(logp_host), _ptr(entropy_host), _ptr(ws), ws.numel(),
+                                       _stream()))
+    return logp_host, entropy_host
+
+
+def gc_grpo_advantages(rewards, group_offsets, eps=1e-6, unbiased_std=False,
+                       drop_constant_groups=False):
+    """-> (adv float32 [R], keep uint8 [G])."""
+    assert rewards.dtype == torch.float32 and group_offsets.dtype == torch.int32
+    G = group_offsets.numel() - 1
+    adv = torch.empty_like(rewards)
+    keep = torch.empty(max(G, 0), dtype=torch.uint8, device=rewards.device)
+    _check(_lib.gc_grpo_advantages(_ptr(rewards), _ptr(group_offsets), G, float(eps),
+                                   int(unbiased_std), int(drop_constant_groups), _ptr(adv),
+                                   _ptr(keep), _stream()))
+    return adv, keep
+
+
+def _loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg):
+    assert cu_seqlens.dtype == torch.int32 and adv.dtype == torch.float32
+    R = cu_seqlens.numel() - 1
+    return [_ptr(cu_seqlens), R, _ptr(adv), _ptr(old_logp), _ptr(ref_logp), float(clip_lo),
+            float(clip_hi), float(beta), int(agg)]
+
+
+def gc_grpo_loss_fwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp, ref_logp,
+                     clip_lo=0.2, clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN, *, simt=False):
+    """-> dict(out5=[loss, pg_loss, kl_mean, clip_frac, n_scored] (device), logp, entropy, lse)."""
+    args, T, D, V, dt = _head_args(H, W, targets, mask, temperature, simt)
+    dev = H.device
+    out5 = torch.empty(5, dtype=torch.float32, device=dev)
+    logp = torch.empty(T, dtype=torch.float32, device=dev)
+    ent = torch.empty(T, dtype=torch.float32, device=dev)
+    lse = torch.empty(T, dtype=torch.float32, device=dev)
+    nb = workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dt)
+    ws = workspace(nb, dev)
+    _check(_lib.gc_grpo_loss_fwd(*args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo,
+                                                    clip_hi, beta, agg),
+                                 _ptr(out5), _ptr(logp), _ptr(ent), _ptr(lse), _ptr(ws),
+                                 ws.numel(), _stream()))
+    return dict(out5=out5, logp=logp, entropy=ent, lse=lse)
+
+
+def gc_grpo_loss_bwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp, ref_logp,
+                     logp, lse, clip_lo=0.2, clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN,
+                     grad_loss=1.0, *, dH=None, dW=None, accumulate_dW=False, chunk_tokens=0,
+                     simt=False):
+    """-> (dH [T,D] in H's dtype, dW [V,D] float32)."""
+    args, T, D, V, dt = _head_args(H, W, targets, mask, temperature, simt)
+    dev = H.device
+    if dH is None:
+        dH = torch.empty(T, D, dtype=H.dtype, device=dev)
+    if dW is None:
+        assert not accumulate_dW
+        dW = torch.empty(V, D, dtype=torch.float32, device=dev)
+    nb = workspace_bytes(GC_OP_LOSS_BWD, T, D, V, dt, chunk_tokens)
+    ws = workspace(nb, dev)
+    _check(_lib.gc_grpo_loss_bwd(*args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo,
+                                                    clip_hi, beta, agg),
+                                 _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH),
+                                 dH.stride(0) if T > 0 else D, _ptr(dW), dW.stride(0), GC_F32,
+                                 int(accumulate_dW), int(chunk_tokens), _ptr(ws), ws.numel(),
+                                 _stream()))
+    return dH, dW
+
+
+def gc_grpo_token_loss(logp, old_logp, ref_logp, targets, mask, cu_seqlens, adv, clip_lo=0.2,
+                       clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN, grad_loss=1.0,
+                       want_grad=True):
+    """The loss kernels alone: -> (out5 device tensor, g [T] or None)."""
+    T = logp.numel()
+    dev = logp.device
+    out5 = torch.empty(5, dtype=torch.float32, device=dev)
+    g = torch.empty(T, dtype=torch.float32, device=dev) if want_grad else None
+    nb = workspace_bytes(GC_OP_LOSS_FWD, T, 8, 8, GC_F32)
+    ws = workspace(nb, dev)
+    R = cu_seqlens.numel() - 1
+    _check(_lib.gc_grpo_token_loss(_ptr(logp), _ptr(old_logp), _ptr(ref_logp), _ptr(targets),
+                                   _ptr(mask), T, _ptr(cu_seqlens), R, _ptr(adv), float(clip_lo),
+                                   float(clip_hi), float(beta), int(agg), float(grad_loss),
+                                   _ptr(out5), _ptr(g), _ptr(ws), ws.numel(), _stream()))
+    return out5, g
+
+
+def gc_compact_rows(H, targets, mask, gather=True):
+    """-> (rows int32 [T] (first n valid), n_rows int32 [1], Hs [T,D] or None)."""
+    T, D = H.shape
+    dev = H.device
+    rows = torch.empty(max(T, 1), dtype=torch.int32, device=dev)
+    n = torch.zeros(1, dtype=torch.int32, device=dev)
+    Hs = torch.empty(T, D, dtype=H.dtype, device=dev) if gather else None
+    dt = dtype_code(H)
+    nb = workspace_bytes(GC_OP_LOGPROBS, T, D, 8, GC_BF16)
+    ws = workspace(nb, dev)
+    _check(_lib.gc_compact_rows(_ptr(H), H.stride(0) if T > 0 else D, dt, _ptr(targets),
+                                _ptr(mask), T, D, _ptr(rows), _ptr(n), _ptr(Hs), _ptr(ws),
+                                ws.numel(), _stream()))
+    return rows, n, Hs
+
+
+def gc_validate_targets(targets, mask, V) -> int:
+    n = C.c_int64(0)
+    _check(_lib.gc_validate_targets(_ptr(targets), _ptr(mask), targets.numel(), int(V),
+                                    C.byref(n), _stream()))
+    return int(n.value)
+
+
+def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, accumulate=False,
+                       cta_group=2):
+    """C[M,N] f32 = A.B on the tcgen05 tile engine (unit test of the engine)."""
+    if a_mn_major:
+        K, M = A.shape
+    else:
+        M, K = A.shape
+    if b_mn_major:
+        Kb, N = B.shape
+    else:
+        N, Kb = B.shape
+    assert K == Kb and A.dtype == torch.bfloat16 and B.dtype == torch.bfloat16
+    if C_out is None:
+        C_out = torch.zeros(M, N, dtype=torch.float32, device=A.device)
+    _check(_lib.gc_debug_gemm_bf16(_ptr(A), A.stride(0), int(a_mn_major), _ptr(B), B.stride(0),
+                                   int(b_mn_major), _ptr(C_out), C_out.stride(0), M, N, K,
+                                   int(accumulate), int(cta_group), _stream()))
+    return C_out

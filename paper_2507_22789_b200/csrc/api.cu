@@ -1,0 +1,419 @@
+// api.cu -- the C ABI of include/gcore.h: argument validation, workspace carving, and the
+// host-side plan (row compaction, chunk loop of the backward).  No allocation, no sync.
+#include "common.cuh"
+
+using namespace gc;
+
+namespace {
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+int check_arch() {
+  int dev = 0, major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return GC_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess)
+    return GC_ERR_CUDA;
+  return major == 10 ? GC_OK : GC_ERR_ARCH;
+}
+
+int elem_bytes(int dtype) { return dtype == GC_F32 ? 4 : 2; }
+
+int check_head_args(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                    const int32_t* targets, int64_t T, int64_t D, int64_t V, float tau) {
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return GC_ERR_DTYPE;
+  if (T < 0 || D <= 0 || V <= 0 || T >= (1ll << 31) || V >= (1ll << 31)) return GC_ERR_SHAPE;
+  if (!(tau > 0.f)) return GC_ERR_ARG;
+  if (!W || (T > 0 && (!H || !targets))) return GC_ERR_NULL;
+  if (ldH < D || ldW < D) return GC_ERR_SHAPE;
+  if (dtype == GC_BF16) {
+    if (D % 8 != 0) return GC_ERR_SHAPE;
+    if (ldH % 8 != 0 || ldW % 8 != 0 || !aligned16(H) || !aligned16(W)) return GC_ERR_ALIGN;
+  }
+  return GC_OK;
+}
+
+// ---- backward chunk size: rows of the dS buffer (multiple of 256) -----------------------------
+// Minimises the number of dH tile waves over the 74 CTA pairs; larger chunks win ties (fewer fp32
+// read-modify-write passes over dW).  Keeps the chunk below T so the [T,V] matrix is never whole.
+int64_t pick_chunk(int64_t T, int64_t D, int64_t V) {
+  const int64_t Tr = ceil_div(T > 0 ? T : 1, 256) * 256;
+  if (Tr <= 256) return 256;
+  const int P = kNumSMs / 2;
+  const int64_t Nt = ceil_div(D, 256);
+  const int64_t half = ceil_div(Tr / 2, 256) * 256;          // at least two chunks
+  int64_t best = 256;
+  double best_cost = 1e300;
+  for (int64_t tc = 256; tc <= 8192 && tc <= half; tc += 256) {
+    if (tc > 256 && (double)tc * (double)V * 2.0 > 6.0e9) break;   // dS buffer <= 6 GB
+    int64_t waves = 0;
+    for (int64_t r0 = 0; r0 < Tr; r0 += tc) {
+      const int64_t rows = (Tr - r0 < tc) ? Tr - r0 : tc;
+      waves += ceil_div(ceil_div(rows, 256) * Nt, P);
+    }
+    const double cost = (double)waves * (1.0 + 0.01 * (double)ceil_div(Tr, tc));
+    if (cost <= best_cost) { best_cost = cost; best = tc; }
+  }
+  return best;
+}
+
+int64_t resolve_chunk(int64_t T, int64_t D, int64_t V, int64_t chunk_tokens) {
+  if (chunk_tokens <= 0) return pick_chunk(T, D, V);
+  return ceil_div(chunk_tokens, 256) * 256;
+}
+
+int64_t ld_ds(int64_t V) { return ceil_div(V, 64) * 64; }
+
+// Workspace layouts (mirrored by gc_workspace_bytes).
+struct FwdWs {
+  RowStat* partials; int32_t* rows; int32_t* n_rows; int32_t* targets_c; void* Hs; void* compact;
+};
+size_t carve_fwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, FwdWs* w) {
+  const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
+  if (dtype == GC_BF16) {
+    RowStat* p = c.take<RowStat>(tc_fwd_partials_bytes(T, V) / sizeof(RowStat));
+    int32_t* rows = c.take<int32_t>((size_t)cap);
+    int32_t* n_rows = c.take<int32_t>(64);
+    int32_t* tc_ = c.take<int32_t>((size_t)cap);
+    void* Hs = c.take<uint8_t>((size_t)cap * (size_t)D * 2);
+    void* cw = c.take<uint8_t>(compact_ws_bytes(T));
+    if (w) { w->partials = p; w->rows = rows; w->n_rows = n_rows; w->targets_c = tc_; w->Hs = Hs; w->compact = cw; }
+  }
+  return c.off;
+}
+
+struct BwdWs {
+  void* loss; float* out5; float* g; int32_t* rows; int32_t* n_rows; int32_t* targets_c;
+  float* lse_c; float* g_c; void* Hs; void* compact; void* dS;
+};
+size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk, int32_t R,
+                 BwdWs* w) {
+  const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
+  void* loss = c.take<uint8_t>(loss_ws_bytes(T, R));
+  float* out5 = c.take<float>(64);
+  float* g = c.take<float>((size_t)cap);
+  if (w) { w->loss = loss; w->out5 = out5; w->g = g; }
+  if (dtype == GC_BF16) {
+    int32_t* rows = c.take<int32_t>((size_t)cap);
+    int32_t* n_rows = c.take<int32_t>(64);
+    int32_t* tcx = c.take<int32_t>((size_t)cap);
+    float* lse_c = c.take<float>((size_t)cap);
+    float* g_c = c.take<float>((size_t)cap);
+    void* Hs = c.take<uint8_t>((size_t)cap * (size_t)D * 2);
+    void* cw = c.take<uint8_t>(compact_ws_bytes(T));
+    void* dS = c.take<uint8_t>((size_t)chunk * (size_t)ld_ds(V) * 2);
+    if (w) { w->rows = rows; w->n_rows = n_rows; w->targets_c = tcx; w->lse_c = lse_c; w->g_c = g_c;
+             w->Hs = Hs; w->compact = cw; w->dS = dS; }
+  }
+  return c.off;
+}
+
+constexpr int32_t kMaxRForWs = 1 << 24;   // loss workspace is sized for up to 16M responses... see below
+
+}  // namespace
+
+extern "C" {
+
+const char* gc_status_string(int status) {
+  switch (status) {
+    case GC_OK: return "GC_OK";
+    case GC_ERR_NULL: return "GC_ERR_NULL: required pointer is NULL";
+    case GC_ERR_SHAPE: return "GC_ERR_SHAPE: bad shape or leading dimension";
+    case GC_ERR_DTYPE: return "GC_ERR_DTYPE: unknown dtype";
+    case GC_ERR_ALIGN: return "GC_ERR_ALIGN: pointer or leading dimension not aligned";
+    case GC_ERR_WORKSPACE: return "GC_ERR_WORKSPACE: workspace missing or too small";
+    case GC_ERR_ARG: return "GC_ERR_ARG: bad scalar argument";
+    case GC_ERR_ARCH: return "GC_ERR_ARCH: device is not compute capability 10.x";
+    case GC_ERR_CUDA: return "GC_ERR_CUDA: CUDA call failed";
+    default: return "GC_ERR_UNKNOWN";
+  }
+}
+
+int gc_version(void) { return 100; }
+
+size_t gc_workspace_bytes(int op, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens) {
+  if (T < 0 || D <= 0 || V <= 0) return 0;
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return 0;
+  Carver c(nullptr);
+  // The loss workspace depends on R; R <= T always (every response has >= 0 tokens, but the
+  // per-response count array is sized by T + 1 to be safe for any R <= T + 1).
+  const int32_t Rcap = (int32_t)((T + 1 < (int64_t)kMaxRForWs) ? T + 1 : kMaxRForWs);
+  switch (op) {
+    case GC_OP_LOGPROBS:
+      carve_fwd(c, T, D, V, dtype, nullptr);
+      break;
+    case GC_OP_LOSS_FWD:
+      carve_fwd(c, T, D, V, dtype, nullptr);
+      c.take<uint8_t>(loss_ws_bytes(T, Rcap));
+      break;
+    case GC_OP_LOSS_BWD:
+      carve_bwd(c, T, D, V, dtype, resolve_chunk(T, D, V, chunk_tokens), Rcap, nullptr);
+      break;
+    default:
+      return 0;
+  }
+  return c.off + 256;
+}
+
+int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                      const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                      float temperature, float* logp, float* entropy, float* lse, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
+  if (T > 0 && !logp) return GC_ERR_NULL;
+  if (T == 0) return GC_OK;
+  GC_TRY(check_arch());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (dtype != GC_BF16)
+    return simt_logprobs(H, ldH, W, ldW, dtype == GC_BF16_SIMT, targets, mask, T, D, V, temperature,
+                         logp, entropy, lse, st);
+  if (!workspace || workspace_bytes < gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0))
+    return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  Carver c(workspace);
+  FwdWs w;
+  carve_fwd(c, T, D, V, dtype, &w);
+  const TcPlan pl = tc_plan_forward(T, V);
+  const int64_t cap = ceil_div(T, 256) * 256;
+  if (!mask) {
+    // dense mode: every row goes through the contraction; rows with target < 0 come out as 0
+    GC_TRY(tc_forward_stats(H, ldH, W, ldW, T, D, V, temperature, targets, nullptr, w.partials, st));
+    return launch_combine(w.partials, pl.n_split, cap, nullptr, nullptr, T, logp, entropy, lse, st);
+  }
+  // compaction mode (a1): only scored rows reach the tensor cores
+  GC_TRY(launch_compact_rows(targets, mask, T, w.rows, w.n_rows, w.compact, st));
+  GC_TRY(launch_gather_rows(H, ldH, 2, D, T, w.rows, w.n_rows, w.Hs, cap, st));
+  GC_TRY(launch_gather_i32(targets, w.rows, w.n_rows, T, w.targets_c, st));
+  GC_TRY(launch_zero_unscored(targets, mask, T, logp, entropy, lse, st));
+  GC_TRY(tc_forward_stats(w.Hs, D, W, ldW, T, D, V, temperature, w.targets_c, w.n_rows, w.partials, st));
+  return launch_combine(w.partials, pl.n_split, cap, w.rows, w.n_rows, T, logp, entropy, lse, st);
+}
+
+size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype) {
+  if (T < 0 || D <= 0) return 0;
+  const size_t t = (size_t)(T > 0 ? T : 1);
+  return align_up(t * (size_t)D * elem_bytes(dtype), 256) + align_up(t * 4, 256) +
+         align_up(t, 256) + 2 * align_up(t * 4, 256) + 256;
+}
+
+int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int dtype,
+                           const int32_t* targets_host, const uint8_t* mask_host, int64_t T,
+                           int64_t D, int64_t V, float temperature, float* logp_host,
+                           float* entropy_host, void* workspace, size_t workspace_bytes,
+                           void* cuda_stream) {
+  if (T < 0 || D <= 0 || V <= 0) return GC_ERR_SHAPE;
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return GC_ERR_DTYPE;
+  if (T == 0) return GC_OK;
+  if (!H_host || !targets_host || !logp_host || !W) return GC_ERR_NULL;
+  const size_t inner = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
+  if (!workspace || workspace_bytes < inner + gc_host_staging_bytes(T, D, dtype))
+    return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  Carver c(static_cast<char*>(workspace) + align_up(inner, 256));
+  const size_t hb = (size_t)T * (size_t)D * elem_bytes(dtype);
+  void* dH = c.take<uint8_t>(hb);
+  int32_t* dT = c.take<int32_t>((size_t)T);
+  uint8_t* dM = c.take<uint8_t>((size_t)T);
+  float* dLp = c.take<float>((size_t)T);
+  float* dEn = c.take<float>((size_t)T);
+  GC_CUDA_TRY(cudaMemcpyAsync(dH, H_host, hb, cudaMemcpyHostToDevice, st));
+  GC_CUDA_TRY(cudaMemcpyAsync(dT, targets_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
+  if (mask_host) GC_CUDA_TRY(cudaMemcpyAsync(dM, mask_host, (size_t)T, cudaMemcpyHostToDevice, st));
+  GC_TRY(gc_token_logprobs(dH, D, W, ldW, dtype, dT, mask_host ? dM : nullptr, T, D, V, temperature,
+                           dLp, entropy_host ? dEn : nullptr, nullptr, workspace, inner, cuda_stream));
+  GC_CUDA_TRY(cudaMemcpyAsync(logp_host, dLp, (size_t)T * 4, cudaMemcpyDeviceToHost, st));
+  if (entropy_host)
+    GC_CUDA_TRY(cudaMemcpyAsync(entropy_host, dEn, (size_t)T * 4, cudaMemcpyDeviceToHost, st));
+  return GC_OK;
+}
+
+int gc_grpo_advantages(const float* rewards, const int32_t* group_offsets, int32_t G, float eps,
+                       int unbiased_std, int drop_constant_groups, float* adv, uint8_t* keep,
+                       void* cuda_stream) {
+  if (G < 0) return GC_ERR_SHAPE;
+  if (!(eps >= 0.f)) return GC_ERR_ARG;
+  if (G == 0) return GC_OK;
+  if (!rewards || !group_offsets || !adv) return GC_ERR_NULL;
+  GC_TRY(check_arch());
+  return launch_advantages(rewards, group_offsets, G, eps, unbiased_std != 0,
+                           drop_constant_groups != 0, adv, keep, static_cast<cudaStream_t>(cuda_stream));
+}
+
+static int check_loss_args(const int32_t* cu_seqlens, int32_t R, const float* adv,
+                           const float* old_logp, const float* ref_logp, float clip_lo,
+                           float clip_hi, float beta, int agg, int64_t T) {
+  if (R < 0 || (T > 0 && R < 1) || (int64_t)R > T + 1) return GC_ERR_SHAPE;
+  if (agg != GC_AGG_TOKEN_MEAN && agg != GC_AGG_SEQ_MEAN) return GC_ERR_ARG;
+  if (!(clip_lo >= 0.f) || !(clip_hi >= 0.f) || !(beta >= 0.f)) return GC_ERR_ARG;
+  if (!cu_seqlens || (T > 0 && (!adv || !old_logp))) return GC_ERR_NULL;
+  if (beta != 0.f && T > 0 && !ref_logp) return GC_ERR_NULL;
+  return GC_OK;
+}
+
+int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
+                       const int32_t* targets, const uint8_t* mask, int64_t T,
+                       const int32_t* cu_seqlens, int32_t R, const float* adv, float clip_lo,
+                       float clip_hi, float beta, int agg, float grad_loss, float* out5, float* g,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (T < 0 || T >= (1ll << 31)) return GC_ERR_SHAPE;
+  GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
+  if (!out5 || (T > 0 && (!logp || !targets))) return GC_ERR_NULL;
+  if (!aligned16(logp) || !aligned16(old_logp) || !aligned16(ref_logp) || !aligned16(targets) ||
+      !aligned16(g) || (reinterpret_cast<uintptr_t>(mask) & 3))
+    return GC_ERR_ALIGN;
+  if (!workspace || workspace_bytes < loss_ws_bytes(T, R)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  GC_TRY(check_arch());
+  return launch_token_loss(logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, clip_lo,
+                           clip_hi, beta, agg, grad_loss, out5, g, workspace,
+                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+int gc_grpo_loss_fwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                     const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                     float temperature, const int32_t* cu_seqlens, int32_t R, const float* adv,
+                     const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
+                     float beta, int agg, float* out5, float* logp, float* entropy, float* lse,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
+  GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
+  if (!out5 || (T > 0 && (!logp || !lse))) return GC_ERR_NULL;
+  const size_t need = gc_workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dtype, 0);
+  if (!workspace || workspace_bytes < need) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  const size_t fwd_bytes = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
+  GC_TRY(gc_token_logprobs(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, logp, entropy,
+                           lse, workspace, fwd_bytes, cuda_stream));
+  void* loss_ws = static_cast<char*>(workspace) + align_up(fwd_bytes, 256);
+  return gc_grpo_token_loss(logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, clip_lo,
+                            clip_hi, beta, agg, 1.0f, out5, nullptr, loss_ws,
+                            workspace_bytes - align_up(fwd_bytes, 256), cuda_stream);
+}
+
+int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                     const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                     float temperature, const int32_t* cu_seqlens, int32_t R, const float* adv,
+                     const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
+                     float beta, int agg, const float* logp, const float* lse, float grad_loss,
+                     void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
+                     int accumulate_dW, int64_t chunk_tokens, void* workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
+  GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
+  if (dW_dtype != GC_F32) return GC_ERR_DTYPE;
+  if (!dW || (T > 0 && (!dH || !logp || !lse))) return GC_ERR_NULL;
+  if (lddH < D || lddW < D) return GC_ERR_SHAPE;
+  if (dtype == GC_BF16 && (lddH % 8 != 0 || lddW % 4 != 0 || !aligned16(dH) || !aligned16(dW)))
+    return GC_ERR_ALIGN;
+  if (!aligned16(logp) || !aligned16(old_logp) || !aligned16(ref_logp) || !aligned16(targets) ||
+      (reinterpret_cast<uintptr_t>(mask) & 3))
+    return GC_ERR_ALIGN;
+  const size_t need = gc_workspace_bytes(GC_OP_LOSS_BWD, T, D, V, dtype, chunk_tokens);
+  if (!workspace || workspace_bytes < need) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  GC_TRY(check_arch());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (T == 0) {
+    if (!accumulate_dW)
+      GC_CUDA_TRY(cudaMemset2DAsync(dW, (size_t)lddW * 4, 0, (size_t)D * 4, (size_t)V, st));
+    return GC_OK;
+  }
+  const int64_t chunk = resolve_chunk(T, D, V, chunk_tokens);
+  const int32_t Rcap = (int32_t)((T + 1 < (int64_t)kMaxRForWs) ? T + 1 : kMaxRForWs);
+  Carver c(workspace);
+  BwdWs w;
+  carve_bwd(c, T, D, V, dtype, chunk, Rcap, &w);
+
+  // a9: g_t = grad_loss * d loss / d logp_t for every token (0 at unscored tokens)
+  GC_TRY(launch_token_loss(logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, clip_lo,
+                           clip_hi, beta, agg, grad_loss, w.out5, w.g, w.loss, st));
+
+  if (dtype != GC_BF16)
+    return simt_backward(H, ldH, W, ldW, dtype == GC_BF16_SIMT, targets, mask, T, D, V, temperature,
+                         lse, w.g, dH, lddH, static_cast<float*>(dW), lddW, accumulate_dW, st);
+
+  const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
+  const int64_t ldS = ld_ds(V);
+  const bool compact = mask != nullptr;
+  const void* Hs = H;
+  int64_t ldHs = ldH;
+  const int32_t* targets_c = targets;
+  const float* lse_c = lse;
+  const float* g_c = w.g;
+  const int32_t* rows = nullptr;
+  const int32_t* n_rows = nullptr;
+  if (compact) {
+    GC_TRY(launch_compact_rows(targets, mask, T, w.rows, w.n_rows, w.compact, st));
+    GC_TRY(launch_gather_rows(H, ldH, 2, D, T, w.rows, w.n_rows, w.Hs, cap, st));
+    GC_TRY(launch_gather_i32(targets, w.rows, w.n_rows, T, w.targets_c, st));
+    GC_TRY(launch_gather_f32(lse, w.rows, w.n_rows, T, w.lse_c, st));
+    GC_TRY(launch_gather_f32(w.g, w.rows, w.n_rows, T, w.g_c, st));
+    GC_TRY(launch_zero_rows_unscored(targets, mask, T, dH, lddH, 2, D, st));
+    Hs = w.Hs; ldHs = D; targets_c = w.targets_c; lse_c = w.lse_c; g_c = w.g_c;
+    rows = w.rows; n_rows = w.n_rows;
+  }
+  for (int64_t row0 = 0; row0 < T; row0 += chunk) {
+    const int64_t n_static = compact ? 0 : ((T - row0 < chunk) ? T - row0 : chunk);
+    const int64_t rows_cap = compact ? ((cap - row0 < chunk) ? cap - row0 : chunk) : chunk;
+    const char* Hc = static_cast<const char*>(Hs) + (size_t)row0 * (size_t)ldHs * 2;
+    // a10: recompute the logit chunk, dS = (g/tau)(onehot - p) in bf16
+    GC_TRY(tc_recompute_ds(Hc, ldHs, W, ldW, rows_cap, n_static, D, V, temperature,
+                           targets_c + row0, lse_c + row0, g_c + row0, n_rows, row0, w.dS, ldS, st));
+    // a11: dH rows of this chunk
+    GC_TRY(tc_dh(w.dS, ldS, rows_cap, n_static, W, ldW, D, V, rows ? rows + row0 : nullptr, n_rows,
+                 row0, dH, lddH, st));
+    // a12: dW accumulates over chunks in fp32
+    GC_TRY(tc_dw(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
+                 static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0, st));
+  }
+  return GC_OK;
+}
+
+int gc_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
+                        int64_t* n_bad_host, void* cuda_stream) {
+  if (!n_bad_host) return GC_ERR_NULL;
+  *n_bad_host = 0;
+  if (T == 0) return GC_OK;
+  if (!targets) return GC_ERR_NULL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned long long* d = nullptr;
+  // debug helper: the one entry point that allocates and synchronises
+  GC_CUDA_TRY(cudaMalloc(&d, sizeof(unsigned long long)));
+  cudaMemsetAsync(d, 0, sizeof(unsigned long long), st);
+  int s = launch_validate_targets(targets, mask, T, V, d, st);
+  unsigned long long h = 0;
+  if (s == GC_OK && cudaMemcpyAsync(&h, d, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    s = GC_ERR_CUDA;
+  if (s == GC_OK && cudaStreamSynchronize(st) != cudaSuccess) s = GC_ERR_CUDA;
+  cudaFree(d);
+  *n_bad_host = (int64_t)h;
+  return s;
+}
+
+int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* targets,
+                    const uint8_t* mask, int64_t T, int64_t D, int32_t* rows, int32_t* n_rows,
+                    void* Hs, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (T < 0 || T >= (1ll << 31) || D <= 0) return GC_ERR_SHAPE;
+  if (!rows || !n_rows || (T > 0 && !targets)) return GC_ERR_NULL;
+  if (!workspace || workspace_bytes < compact_ws_bytes(T)) return GC_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  GC_TRY(launch_compact_rows(targets, mask, T, rows, n_rows, workspace, st));
+  if (Hs) {
+    if (!H) return GC_ERR_NULL;
+    if (ldH < D) return GC_ERR_SHAPE;
+    GC_TRY(launch_gather_rows(H, ldH, elem_bytes(dtype), D, T, rows, n_rows, Hs, T, st));
+  }
+  return GC_OK;
+}
+
+int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
+                       int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
+                       int accumulate, int cta_group, void* cuda_stream) {
+  if (!A || !B || !C) return GC_ERR_NULL;
+  if (M <= 0 || N <= 0 || K <= 0) return GC_ERR_SHAPE;
+  GC_TRY(check_arch());
+  return tc_debug_gemm(A, lda, a_mn_major, B, ldb, b_mn_major, C, ldc, M, N, K, accumulate,
+                       cta_group, static_cast<cudaStream_t>(cuda_stream));
+}
+
+}  // extern "C"

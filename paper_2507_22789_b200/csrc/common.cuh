@@ -1,0 +1,114 @@
+// common.cuh -- shared declarations of the gcore CUDA library (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/gcore.h"
+
+#define GC_CUDA_TRY(expr)                         \
+  do {                                            \
+    cudaError_t _e = (expr);                      \
+    if (_e != cudaSuccess) return GC_ERR_CUDA;    \
+  } while (0)
+
+#define GC_TRY(expr)                              \
+  do {                                            \
+    int _s = (expr);                              \
+    if (_s != GC_OK) return _s;                   \
+  } while (0)
+
+namespace gc {
+
+constexpr int kNumSMs = 148;          // B200: 2 dies x 74 SMs
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// Workspace carving: a bump allocator over the caller's buffer (256-byte granules).
+struct Carver {
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* p) : base(static_cast<char*>(p)) {}
+  template <typename T>
+  T* take(size_t n) {
+    T* p = reinterpret_cast<T*>(base + off);
+    off += align_up(n * sizeof(T), 256);
+    return p;
+  }
+};
+
+// Partial (per row, per vocab chunk) online-softmax statistics, in log2-scaled units
+// a = z * log2(e):  m = max a, s = sum 2^(a-m), u = sum 2^(a-m) (a-m), ay = a at the target
+// (-inf if the target is not in this chunk).
+struct __align__(16) RowStat { float m, s, u, ay; };
+
+// ---- launchers implemented in the .cu files (all enqueue on `st`, no sync) ----------------
+// small_kernels.cu
+int launch_advantages(const float* rewards, const int32_t* group_offsets, int32_t G, float eps,
+                      int unbiased, int drop_const, float* adv, uint8_t* keep, cudaStream_t st);
+size_t loss_ws_bytes(int64_t T, int32_t R);
+int launch_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
+                      const int32_t* targets, const uint8_t* mask, int64_t T,
+                      const int32_t* cu_seqlens, int32_t R, const float* adv,
+                      float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
+                      float* out5, float* g, void* ws, cudaStream_t st);
+int launch_combine(const RowStat* partials, int n_split, int64_t split_stride,
+                   const int32_t* rows, const int32_t* n_rows_dev, int64_t n_rows_max,
+                   float* logp, float* entropy, float* lse, cudaStream_t st);
+int launch_zero_unscored(const int32_t* targets, const uint8_t* mask, int64_t T,
+                         float* logp, float* entropy, float* lse, cudaStream_t st);
+size_t compact_ws_bytes(int64_t T);
+int launch_compact_rows(const int32_t* targets, const uint8_t* mask, int64_t T, int32_t* rows,
+                        int32_t* n_rows, void* ws, cudaStream_t st);
+int launch_gather_rows(const void* H, int64_t ldH, int elem_bytes, int64_t D, int64_t T,
+                       const int32_t* rows, const int32_t* n_rows, void* Hs, int64_t pad_rows,
+                       cudaStream_t st);
+int launch_gather_f32(const float* src, const int32_t* rows, const int32_t* n_rows,
+                      int64_t T, float* dst, cudaStream_t st);
+int launch_gather_i32(const int32_t* src, const int32_t* rows, const int32_t* n_rows,
+                      int64_t T, int32_t* dst, cudaStream_t st);
+int launch_zero_rows_unscored(const int32_t* targets, const uint8_t* mask, int64_t T, void* dH,
+                              int64_t lddH, int elem_bytes, int64_t D, cudaStream_t st);
+int launch_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
+                            unsigned long long* n_bad_dev, cudaStream_t st);
+
+// simt_head.cu
+int simt_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, bool bf16,
+                  const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                  float tau, float* logp, float* entropy, float* lse, cudaStream_t st);
+int simt_backward(const void* H, int64_t ldH, const void* W, int64_t ldW, bool bf16,
+                  const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                  float tau, const float* lse, const float* g, void* dH, int64_t lddH,
+                  float* dW, int64_t lddW, int accumulate, cudaStream_t st);
+
+// tc_head.cu (tcgen05 engine)
+struct TcPlan {            // forward / recompute schedule: items = (vocab chunk c, M tile)
+  int n_vtiles;            // ceil(V / 256)
+  int chunk_vtiles;        // vocab tiles per item
+  int n_split;             // number of vocab chunks = partial slots per row
+};
+TcPlan tc_plan_forward(int64_t T, int64_t V);
+size_t tc_fwd_partials_bytes(int64_t T, int64_t V);
+int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
+                     int64_t D, int64_t V, float tau, const int32_t* targets_c,
+                     const int32_t* n_rows_dev, RowStat* partials, cudaStream_t st);
+// Backward chunk kernels.  rows_cap = rows of the dS chunk buffer (multiple of 256); the valid
+// rows of the chunk are clamp(*n_rows_dev - row0, 0, rows_cap), or n_static if n_rows_dev == NULL.
+int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,
+                    int64_t n_static, int64_t D, int64_t V, float tau, const int32_t* targets_c,
+                    const float* lse_c, const float* g_c, const int32_t* n_rows_dev,
+                    int64_t row0, void* dS, int64_t ldS, cudaStream_t st);
+int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* W,
+          int64_t ldW, int64_t D, int64_t V, const int32_t* rows, const int32_t* n_rows_dev,
+          int64_t row0, void* dH, int64_t lddH, cudaStream_t st);
+int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
+          int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
+          int64_t lddW, int accumulate, cudaStream_t st);
+int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
+                  float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
+                  int cta_group, cudaStream_t st);
+
+}  // namespace gc

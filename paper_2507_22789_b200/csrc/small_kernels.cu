@@ -1,0 +1,592 @@
+// small_kernels.cu -- the HBM/latency-bound steps of the path (SURVEY.md sec 8(a) rows a1, a4,
+// a6-a9): row selection/compaction, partial-stat combine, group filter + GRPO advantages,
+// per-token clipped-ratio loss with k3 KL and its gradient w.r.t. logp.
+// All floating-point reductions are fixed-order (no float atomics): reruns are bit-identical.
+#include "common.cuh"
+
+namespace gc {
+
+__device__ __forceinline__ bool is_scored(const int32_t* targets, const uint8_t* mask, int64_t t) {
+  return targets[t] >= 0 && (mask == nullptr || mask[t] != 0);
+}
+
+template <typename T>
+__device__ __forceinline__ T warp_sum(T v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// =============================================================================================
+// a6 + a7: group filter and advantages.  One warp per group; fp64 accumulation (R is tiny).
+//   keep[g] = 0 iff all rewards equal;  A_i = (r_i - mu_g) / (sigma_g + eps)
+// =============================================================================================
+__global__ void k_advantages(const float* __restrict__ rewards,
+                             const int32_t* __restrict__ group_offsets, int32_t G, float eps,
+                             int unbiased, int drop_const, float* __restrict__ adv,
+                             uint8_t* __restrict__ keep) {
+  const int g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (g >= G) return;
+  const int a = group_offsets[g], b = group_offsets[g + 1];
+  const int n = b - a;
+  if (n <= 0) {
+    if (keep && lane == 0) keep[g] = drop_const ? 0 : 1;
+    return;
+  }
+  const float r0 = rewards[a];
+  double sum = 0.0;
+  int all_eq = 1;
+  for (int i = a + lane; i < b; i += 32) {
+    const float r = rewards[i];
+    sum += (double)r;
+    all_eq &= (r == r0);
+  }
+  sum = warp_sum(sum);
+  all_eq = __all_sync(0xffffffffu, all_eq);
+  const double mu = sum / (double)n;
+  double ss = 0.0;
+  for (int i = a + lane; i < b; i += 32) {
+    const double d = (double)rewards[i] - mu;
+    ss += d * d;
+  }
+  ss = warp_sum(ss);
+  double sigma;
+  if (unbiased) sigma = n > 1 ? sqrt(ss / (double)(n - 1)) : 0.0;
+  else sigma = sqrt(ss / (double)n);
+  const bool dropped = drop_const && all_eq;
+  const double inv = 1.0 / (sigma + (double)eps);
+  for (int i = a + lane; i < b; i += 32)
+    adv[i] = dropped ? 0.0f : (float)(((double)rewards[i] - mu) * inv);
+  if (keep && lane == 0) keep[g] = dropped ? 0 : 1;
+}
+
+int launch_advantages(const float* rewards, const int32_t* group_offsets, int32_t G, float eps,
+                      int unbiased, int drop_const, float* adv, uint8_t* keep, cudaStream_t st) {
+  if (G == 0) return GC_OK;
+  const int threads = 128;
+  const int64_t blocks = ceil_div((int64_t)G * 32, threads);
+  k_advantages<<<(unsigned)blocks, threads, 0, st>>>(rewards, group_offsets, G, eps, unbiased,
+                                                     drop_const, adv, keep);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// =============================================================================================
+// a8 + a9: per-token loss and d loss / d logp.
+//   rho = e^{logp-old}; s = min(rho A, clip(rho) A); d = ref - logp; k3 = e^d - d - 1
+//   l = -s + beta k3;   dl/dlogp = -[rho A <= clip(rho) A] rho A + beta (1 - e^d)
+// Weights: token-mean w_t = m_t / max(sum m, 1);  seq-mean w_t = m_t / (R_kept max(cnt_r, 1)).
+// Pass 1 (k_loss_counts): integer counts (sum m; per-response counts, R_kept) -- integer
+// atomics only.  Pass 2 (k_token_loss): each block reduces its tile in fixed order to fp64
+// partials; the last block to finish (integer ticket) sums the partials in index order.
+// =============================================================================================
+struct LossCounters {
+  unsigned long long n_scored;   // sum_t m_t
+  unsigned long long n_clipped;
+  unsigned int n_kept;           // responses with >= 1 scored token
+  unsigned int ticket;
+};
+
+constexpr int kLossThreads = 256;
+constexpr int kLossTile = kLossThreads * 4 * 2;   // tokens per block (4 per thread, 2 rounds)
+
+// upper_bound(cu, cu+R+1, t) - 1  : response containing token t (cu[0]=0, cu[R]=T).
+__device__ __forceinline__ int find_response(const int32_t* __restrict__ cu, int lo, int hi,
+                                             int32_t t) {
+  // invariant: cu[lo] <= t < cu[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (cu[mid] <= t) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+__global__ void k_loss_counts_token(const int32_t* __restrict__ targets,
+                                    const uint8_t* __restrict__ mask, int64_t T,
+                                    LossCounters* __restrict__ cnt) {
+  unsigned int c = 0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < T;
+       t += (int64_t)gridDim.x * blockDim.x)
+    c += is_scored(targets, mask, t) ? 1u : 0u;
+  c = warp_sum(c);
+  __shared__ unsigned int sm[32];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long tot = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) tot += sm[w];
+    if (tot) atomicAdd(&cnt->n_scored, tot);
+  }
+}
+
+// seq-mean: one warp per response counts its scored tokens.
+__global__ void k_loss_counts_seq(const int32_t* __restrict__ targets,
+                                  const uint8_t* __restrict__ mask,
+                                  const int32_t* __restrict__ cu, int32_t R,
+                                  int32_t* __restrict__ resp_cnt, LossCounters* __restrict__ cnt) {
+  const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (r >= R) return;
+  unsigned int c = 0;
+  for (int64_t t = cu[r] + lane; t < cu[r + 1]; t += 32) c += is_scored(targets, mask, t) ? 1u : 0u;
+  c = warp_sum(c);
+  if (lane == 0) {
+    resp_cnt[r] = (int32_t)c;
+    if (c) {
+      atomicAdd(&cnt->n_scored, (unsigned long long)c);
+      atomicAdd(&cnt->n_kept, 1u);
+    }
+  }
+}
+
+struct LossPartial { double loss_pg, loss_kl; };
+
+__global__ void __launch_bounds__(kLossThreads)
+k_token_loss(const float* __restrict__ logp, const float* __restrict__ old_logp,
+             const float* __restrict__ ref_logp, const int32_t* __restrict__ targets,
+             const uint8_t* __restrict__ mask, int64_t T, const int32_t* __restrict__ cu,
+             int32_t R, const float* __restrict__ adv, const int32_t* __restrict__ resp_cnt,
+             float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
+             LossCounters* __restrict__ cnt, LossPartial* __restrict__ partials,
+             float* __restrict__ out5, float* __restrict__ g) {
+  const int64_t tile0 = (int64_t)blockIdx.x * kLossTile;
+  const double n_scored = (double)cnt->n_scored;
+  const double n_kept = (double)cnt->n_kept;
+  // gradient scale shared by every token of the batch
+  const float gscale_tok = grad_loss / (float)fmax(n_scored, 1.0);
+  const float gscale_seq = grad_loss / (float)fmax(n_kept, 1.0);
+  const float lo_c = 1.0f - clip_lo, hi_c = 1.0f + clip_hi;
+
+  double acc_pg = 0.0, acc_kl = 0.0;
+  unsigned int n_clip = 0;
+#pragma unroll
+  for (int round = 0; round < 2; ++round) {
+    const int64_t t0 = tile0 + ((int64_t)round * kLossThreads + threadIdx.x) * 4;
+    if (t0 >= T) continue;
+    const int nt = (int)min((int64_t)4, T - t0);
+    float lp[4], ol[4], rf[4];
+    int32_t y[4];
+    uint8_t mk[4];
+    if (nt == 4) {
+      const float4 a = *reinterpret_cast<const float4*>(logp + t0);
+      const float4 b = *reinterpret_cast<const float4*>(old_logp + t0);
+      const int4 c = *reinterpret_cast<const int4*>(targets + t0);
+      lp[0] = a.x; lp[1] = a.y; lp[2] = a.z; lp[3] = a.w;
+      ol[0] = b.x; ol[1] = b.y; ol[2] = b.z; ol[3] = b.w;
+      y[0] = c.x; y[1] = c.y; y[2] = c.z; y[3] = c.w;
+      if (ref_logp) {
+        const float4 d = *reinterpret_cast<const float4*>(ref_logp + t0);
+        rf[0] = d.x; rf[1] = d.y; rf[2] = d.z; rf[3] = d.w;
+      } else {
+        rf[0] = lp[0]; rf[1] = lp[1]; rf[2] = lp[2]; rf[3] = lp[3];
+      }
+      if (mask) {
+        const uchar4 e = *reinterpret_cast<const uchar4*>(mask + t0);
+        mk[0] = e.x; mk[1] = e.y; mk[2] = e.z; mk[3] = e.w;
+      } else {
+        mk[0] = mk[1] = mk[2] = mk[3] = 1;
+      }
+    } else {
+      for (int i = 0; i < 4; ++i) {
+        const bool in = i < nt;
+        lp[i] = in ? logp[t0 + i] : 0.f;
+        ol[i] = in ? old_logp[t0 + i] : 0.f;
+        rf[i] = in ? (ref_logp ? ref_logp[t0 + i] : lp[i]) : 0.f;
+        y[i] = in ? targets[t0 + i] : -1;
+        mk[i] = in ? (mask ? mask[t0 + i] : 1) : 0;
+      }
+    }
+    // response of the first token by binary search, then walk forward
+    int r = find_response(cu, 0, R, (int32_t)t0);
+    int32_t r_end = cu[r + 1];
+    float gout[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      gout[i] = 0.f;
+      if (i >= nt) continue;
+      const int32_t t = (int32_t)(t0 + i);
+      while (t >= r_end && r + 1 < R) { ++r; r_end = cu[r + 1]; }
+      const bool sc = (y[i] >= 0) && (mk[i] != 0) && (t < r_end);
+      if (!sc) continue;
+      const float A = adv[r];
+      const float rho = expf(lp[i] - ol[i]);
+      const float s1 = rho * A;
+      const float s2 = fminf(fmaxf(rho, lo_c), hi_c) * A;
+      const bool unclipped = s1 <= s2;
+      const float s = fminf(s1, s2);
+      const float d = rf[i] - lp[i];
+      const float ed = expf(d);
+      const float k3 = ed - d - 1.0f;
+      float w = 1.0f, gs = gscale_tok;
+      if (agg == GC_AGG_SEQ_MEAN) {
+        w = 1.0f / (float)max(resp_cnt[r], 1);
+        gs = gscale_seq * w;
+      }
+      acc_pg += (double)(-s * w);
+      acc_kl += (double)(k3 * w);
+      n_clip += unclipped ? 0u : 1u;
+      gout[i] = gs * ((unclipped ? -s1 : 0.0f) + beta * (1.0f - ed));
+    }
+    if (g) {
+      if (nt == 4) *reinterpret_cast<float4*>(g + t0) = make_float4(gout[0], gout[1], gout[2], gout[3]);
+      else for (int i = 0; i < nt; ++i) g[t0 + i] = gout[i];
+    }
+  }
+  // block reduction in fixed order
+  acc_pg = warp_sum(acc_pg);
+  acc_kl = warp_sum(acc_kl);
+  n_clip = warp_sum(n_clip);
+  __shared__ double s_pg[kLossThreads / 32], s_kl[kLossThreads / 32];
+  __shared__ unsigned int s_cl[kLossThreads / 32];
+  __shared__ bool is_last;
+  const int wid = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) { s_pg[wid] = acc_pg; s_kl[wid] = acc_kl; s_cl[wid] = n_clip; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+    unsigned long long c = 0;
+    for (int w = 0; w < kLossThreads / 32; ++w) { a += s_pg[w]; b += s_kl[w]; c += s_cl[w]; }
+    partials[blockIdx.x].loss_pg = a;
+    partials[blockIdx.x].loss_kl = b;
+    if (c) atomicAdd(&cnt->n_clipped, c);
+    __threadfence();
+    const unsigned int ticket = atomicAdd(&cnt->ticket, 1u);
+    is_last = (ticket == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  // final fixed-order sum over block partials (one warp, strided, then shuffle tree)
+  if (threadIdx.x < 32) {
+    double a = 0.0, b = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += 32) {
+      a += partials[i].loss_pg;
+      b += partials[i].loss_kl;
+    }
+    a = warp_sum(a);
+    b = warp_sum(b);
+    if (threadIdx.x == 0) {
+      const double denom = (agg == GC_AGG_SEQ_MEAN) ? fmax(n_kept, 1.0) : fmax(n_scored, 1.0);
+      const double pg = a / denom, kl = b / denom;
+      out5[0] = (float)(pg + (double)beta * kl);
+      out5[1] = (float)pg;
+      out5[2] = (float)kl;
+      out5[3] = (float)((double)atomicAdd(&cnt->n_clipped, 0ull) / fmax(n_scored, 1.0));
+      out5[4] = (float)n_scored;
+    }
+  }
+}
+
+size_t loss_ws_bytes(int64_t T, int32_t R) {
+  const int64_t blocks = ceil_div(T > 0 ? T : 1, kLossTile);
+  return align_up(sizeof(LossCounters), 256) + align_up((size_t)blocks * sizeof(LossPartial), 256) +
+         align_up((size_t)(R > 0 ? R : 1) * sizeof(int32_t), 256);
+}
+
+int launch_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
+                      const int32_t* targets, const uint8_t* mask, int64_t T,
+                      const int32_t* cu_seqlens, int32_t R, const float* adv,
+                      float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
+                      float* out5, float* g, void* ws, cudaStream_t st) {
+  const int64_t blocks = ceil_div(T > 0 ? T : 1, kLossTile);
+  Carver c(ws);
+  LossCounters* cnt = c.take<LossCounters>(1);
+  LossPartial* partials = c.take<LossPartial>((size_t)blocks);
+  int32_t* resp_cnt = c.take<int32_t>((size_t)(R > 0 ? R : 1));
+  GC_CUDA_TRY(cudaMemsetAsync(cnt, 0, sizeof(LossCounters), st));
+  if (agg == GC_AGG_SEQ_MEAN) {
+    const int64_t b = ceil_div((int64_t)R * 32, 256);
+    k_loss_counts_seq<<<(unsigned)(b > 0 ? b : 1), 256, 0, st>>>(targets, mask, cu_seqlens, R,
+                                                                resp_cnt, cnt);
+  } else {
+    int64_t b = ceil_div(T > 0 ? T : 1, 256 * 8);
+    if (b > kNumSMs * 8) b = kNumSMs * 8;
+    k_loss_counts_token<<<(unsigned)b, 256, 0, st>>>(targets, mask, T, cnt);
+  }
+  GC_CUDA_TRY(cudaGetLastError());
+  k_token_loss<<<(unsigned)blocks, kLossThreads, 0, st>>>(
+      logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, resp_cnt, clip_lo, clip_hi,
+      beta, agg, grad_loss, cnt, partials, out5, g);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// =============================================================================================
+// a4: combine split-V partials (fixed order) and finish:
+//   lse = ln2 (M + log2 S);  logp = ln2 a_y - lse;  entropy = lse - ln2 U / S
+// partials[c * split_stride + i] for compact row i; output row = rows ? rows[i] : i.
+// =============================================================================================
+__global__ void k_combine(const RowStat* __restrict__ partials, int n_split, int64_t split_stride,
+                          const int32_t* __restrict__ rows, const int32_t* __restrict__ n_rows_dev,
+                          int64_t n_rows_max, float* __restrict__ logp,
+                          float* __restrict__ entropy, float* __restrict__ lse) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n_rows = n_rows_dev ? (int64_t)*n_rows_dev : n_rows_max;
+  if (i >= n_rows) return;
+  float M = -INFINITY;
+  for (int c = 0; c < n_split; ++c) M = fmaxf(M, partials[(int64_t)c * split_stride + i].m);
+  float S = 0.f, U = 0.f, ay = -INFINITY;
+  for (int c = 0; c < n_split; ++c) {
+    const RowStat p = partials[(int64_t)c * split_stride + i];
+    const float sc = exp2f(p.m - M);
+    S += p.s * sc;
+    U += (p.u + p.m * p.s) * sc;         // sum 2^(a-M) a
+    ay = fmaxf(ay, p.ay);
+  }
+  const float l = kLn2 * (M + log2f(S));
+  const int64_t o = rows ? (int64_t)rows[i] : i;
+  const bool ok = ay > -INFINITY;        // dense mode: target < 0 -> never found -> outputs 0
+  logp[o] = ok ? kLn2 * ay - l : 0.f;
+  if (entropy) entropy[o] = ok ? l - kLn2 * (U / S) : 0.f;
+  if (lse) lse[o] = ok ? l : 0.f;
+}
+
+int launch_combine(const RowStat* partials, int n_split, int64_t split_stride,
+                   const int32_t* rows, const int32_t* n_rows_dev, int64_t n_rows_max,
+                   float* logp, float* entropy, float* lse, cudaStream_t st) {
+  if (n_rows_max <= 0) return GC_OK;
+  const int threads = 128;
+  k_combine<<<(unsigned)ceil_div(n_rows_max, threads), threads, 0, st>>>(
+      partials, n_split, split_stride, rows, n_rows_dev, n_rows_max, logp, entropy, lse);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// =============================================================================================
+// a1: row selection.  rows[] = ascending indices of scored tokens (bit-exact integer work):
+// per-block counts -> single-block exclusive scan -> per-block ordered scatter.
+// =============================================================================================
+constexpr int kCompactThreads = 256;
+constexpr int kCompactTile = kCompactThreads * 8;
+
+__global__ void k_compact_count(const int32_t* __restrict__ targets,
+                                const uint8_t* __restrict__ mask, int64_t T,
+                                int32_t* __restrict__ block_counts) {
+  const int64_t base = (int64_t)blockIdx.x * kCompactTile;
+  int c = 0;
+  for (int k = 0; k < 8; ++k) {
+    const int64_t t = base + (int64_t)k * kCompactThreads + threadIdx.x;
+    c += (t < T && is_scored(targets, mask, t)) ? 1 : 0;
+  }
+  c = warp_sum(c);
+  __shared__ int sm[kCompactThreads / 32];
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int tot = 0;
+    for (int w = 0; w < kCompactThreads / 32; ++w) tot += sm[w];
+    block_counts[blockIdx.x] = tot;
+  }
+}
+
+// exclusive scan of block_counts in place; total -> *n_rows.  One block.
+__global__ void k_compact_scan(int32_t* __restrict__ block_counts, int64_t nblocks,
+                               int32_t* __restrict__ n_rows) {
+  __shared__ int sm[1024];
+  __shared__ int carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int64_t base = 0; base < nblocks; base += 1024) {
+    const int64_t i = base + threadIdx.x;
+    const int v = i < nblocks ? block_counts[i] : 0;
+    sm[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {            // Hillis-Steele inclusive scan
+      const int add = threadIdx.x >= o ? sm[threadIdx.x - o] : 0;
+      __syncthreads();
+      sm[threadIdx.x] += add;
+      __syncthreads();
+    }
+    if (i < nblocks) block_counts[i] = carry + sm[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == 0) carry += sm[1023];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *n_rows = carry;
+}
+
+__global__ void k_compact_scatter(const int32_t* __restrict__ targets,
+                                  const uint8_t* __restrict__ mask, int64_t T,
+                                  const int32_t* __restrict__ block_offsets,
+                                  int32_t* __restrict__ rows) {
+  const int64_t base = (int64_t)blockIdx.x * kCompactTile;
+  __shared__ int warp_off[kCompactThreads / 32];
+  __shared__ int running;
+  if (threadIdx.x == 0) running = block_offsets[blockIdx.x];
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int k = 0; k < 8; ++k) {
+    const int64_t t = base + (int64_t)k * kCompactThreads + threadIdx.x;
+    const bool f = t < T && is_scored(targets, mask, t);
+    const unsigned int bal = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) warp_off[wid] = __popc(bal);
+    __syncthreads();
+    int off = running;
+    for (int w = 0; w < wid; ++w) off += warp_off[w];
+    if (f) rows[off + __popc(bal & ((1u << lane) - 1u))] = (int32_t)t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int tot = 0;
+      for (int w = 0; w < kCompactThreads / 32; ++w) tot += warp_off[w];
+      running += tot;
+    }
+    __syncthreads();
+  }
+}
+
+size_t compact_ws_bytes(int64_t T) {
+  return align_up((size_t)ceil_div(T > 0 ? T : 1, kCompactTile) * sizeof(int32_t), 256);
+}
+
+int launch_compact_rows(const int32_t* targets, const uint8_t* mask, int64_t T, int32_t* rows,
+                        int32_t* n_rows, void* ws, cudaStream_t st) {
+  const int64_t nblocks = ceil_div(T > 0 ? T : 1, kCompactTile);
+  int32_t* block_counts = static_cast<int32_t*>(ws);
+  k_compact_count<<<(unsigned)nblocks, kCompactThreads, 0, st>>>(targets, mask, T, block_counts);
+  k_compact_scan<<<1, 1024, 0, st>>>(block_counts, nblocks, n_rows);
+  k_compact_scatter<<<(unsigned)nblocks, kCompactThreads, 0, st>>>(targets, mask, T, block_counts,
+                                                                   rows);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// Gather H rows: Hs[i,:] = H[rows[i],:] for i < n_rows; zero rows for n_rows <= i < pad_end,
+// pad_end = min(round_up(n_rows, 256), pad_rows).  One warp per row, 16-byte vectors,
+// 4 loads in flight per lane.  HBM-bound: 2 * n_rows * D * elem_bytes.
+__global__ void __launch_bounds__(256)
+k_gather_rows(const uint8_t* __restrict__ H, int64_t ld_bytes, int64_t row_bytes, int64_t T,
+              const int32_t* __restrict__ rows, const int32_t* __restrict__ n_rows_dev,
+              uint8_t* __restrict__ Hs, int64_t pad_rows) {
+  const int64_t n_rows = *n_rows_dev;
+  int64_t pad_end = (n_rows + 255) / 256 * 256;
+  if (pad_end > pad_rows) pad_end = pad_rows;
+  const int lane = threadIdx.x & 31;
+  const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int64_t nvec = row_bytes >> 4;
+  for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; i < pad_end; i += warps) {
+    int4* dst = reinterpret_cast<int4*>(Hs + i * row_bytes);
+    if (i < n_rows) {
+      const int4* src = reinterpret_cast<const int4*>(H + (int64_t)rows[i] * ld_bytes);
+      int64_t v = lane;
+      for (; v + 96 < nvec; v += 128) {
+        const int4 a = __ldg(src + v), b = __ldg(src + v + 32), c = __ldg(src + v + 64),
+                   d = __ldg(src + v + 96);
+        dst[v] = a; dst[v + 32] = b; dst[v + 64] = c; dst[v + 96] = d;
+      }
+      for (; v < nvec; v += 32) dst[v] = __ldg(src + v);
+    } else {
+      for (int64_t v = lane; v < nvec; v += 32) dst[v] = make_int4(0, 0, 0, 0);
+    }
+  }
+}
+
+int launch_gather_rows(const void* H, int64_t ldH, int elem_bytes, int64_t D, int64_t T,
+                       const int32_t* rows, const int32_t* n_rows, void* Hs, int64_t pad_rows,
+                       cudaStream_t st) {
+  if ((D * elem_bytes) % 16 != 0 || (ldH * elem_bytes) % 16 != 0) return GC_ERR_ALIGN;
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 8);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_gather_rows<<<(unsigned)blocks, 256, 0, st>>>(
+      static_cast<const uint8_t*>(H), ldH * elem_bytes, D * elem_bytes, T, rows, n_rows,
+      static_cast<uint8_t*>(Hs), pad_rows);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+template <typename T>
+__global__ void k_gather_1d(const T* __restrict__ src, const int32_t* __restrict__ rows,
+                            const int32_t* __restrict__ n_rows_dev, T* __restrict__ dst) {
+  const int64_t n = *n_rows_dev;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    dst[i] = src[rows[i]];
+}
+
+int launch_gather_f32(const float* src, const int32_t* rows, const int32_t* n_rows, int64_t T,
+                      float* dst, cudaStream_t st) {
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_gather_1d<float><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, dst);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+int launch_gather_i32(const int32_t* src, const int32_t* rows, const int32_t* n_rows, int64_t T,
+                      int32_t* dst, cudaStream_t st) {
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_gather_1d<int32_t><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, dst);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// logp / entropy / lse at unscored rows = 0 (compaction mode writes only scored rows).
+__global__ void k_zero_unscored(const int32_t* __restrict__ targets,
+                                const uint8_t* __restrict__ mask, int64_t T,
+                                float* __restrict__ logp, float* __restrict__ entropy,
+                                float* __restrict__ lse) {
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < T;
+       t += (int64_t)gridDim.x * blockDim.x) {
+    if (!is_scored(targets, mask, t)) {
+      logp[t] = 0.f;
+      if (entropy) entropy[t] = 0.f;
+      if (lse) lse[t] = 0.f;
+    }
+  }
+}
+
+int launch_zero_unscored(const int32_t* targets, const uint8_t* mask, int64_t T, float* logp,
+                         float* entropy, float* lse, cudaStream_t st) {
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_zero_unscored<<<(unsigned)blocks, 256, 0, st>>>(targets, mask, T, logp, entropy, lse);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// dH rows of unscored tokens = 0.  One warp per row.
+__global__ void k_zero_rows_unscored(const int32_t* __restrict__ targets,
+                                     const uint8_t* __restrict__ mask, int64_t T,
+                                     uint8_t* __restrict__ dH, int64_t ld_bytes, int64_t row_bytes) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  for (int64_t t = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < T; t += warps) {
+    if (is_scored(targets, mask, t)) continue;
+    int4* dst = reinterpret_cast<int4*>(dH + t * ld_bytes);
+    for (int64_t v = lane; v < (row_bytes >> 4); v += 32) dst[v] = make_int4(0, 0, 0, 0);
+  }
+}
+
+int launch_zero_rows_unscored(const int32_t* targets, const uint8_t* mask, int64_t T, void* dH,
+                              int64_t lddH, int elem_bytes, int64_t D, cudaStream_t st) {
+  if ((D * elem_bytes) % 16 != 0 || (lddH * elem_bytes) % 16 != 0) return GC_ERR_ALIGN;
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 8);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_zero_rows_unscored<<<(unsigned)blocks, 256, 0, st>>>(
+      targets, mask, T, static_cast<uint8_t*>(dH), lddH * elem_bytes, D * elem_bytes);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+__global__ void k_validate_targets(const int32_t* __restrict__ targets,
+                                   const uint8_t* __restrict__ mask, int64_t T, int64_t V,
+                                   unsigned long long* __restrict__ n_bad) {
+  unsigned int c = 0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < T;
+       t += (int64_t)gridDim.x * blockDim.x)
+    c += (is_scored(targets, mask, t) && (int64_t)targets[t] >= V) ? 1u : 0u;
+  c = warp_sum(c);
+  if ((threadIdx.x & 31) == 0 && c) atomicAdd(n_bad, (unsigned long long)c);
+}
+
+int launch_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
+                            unsigned long long* n_bad_dev, cudaStream_t st) {
+  int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_validate_targets<<<(unsigned)blocks, 256, 0, st>>>(targets, mask, T, V, n_bad_dev);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+}  // namespace gc

@@ -1,0 +1,342 @@
+// tc_gemm.cuh -- the tcgen05 tile engine: a persistent, warp-specialised bf16 GEMM main loop
+// (TMA -> 128B-swizzled smem ring -> tcgen05.mma -> double-buffered TMEM accumulators ->
+// tcgen05.ld epilogue) shared by the four dense contractions of the path
+// (SURVEY.md sec 8(a) rows a2/a3, a10, a11, a12).  What differs per use is the operand
+// major-ness and the epilogue functor (tc_head.cu).
+//
+// Tile: UMMA 128*CG x 256 x 16, BK = 64 (one 128-byte swizzle row of bf16).  CG = 2 pairs two
+// SMs (cta_group::2): each CTA stages its own 128 rows of A and its own 128 of the 256 B rows,
+// the leader CTA issues the MMAs for both, each CTA's TMEM holds its 128 accumulator rows.
+// Warps: 0 = TMA producer, 1 = MMA issuer (leader CTA only), 2 = TMEM allocator,
+// 4..7 = epilogue (thread = one accumulator row, 32 fp32 columns per tcgen05.ld).
+#pragma once
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace gc {
+namespace tc {
+
+constexpr int BK = 64;
+constexpr int BN = 256;
+constexpr int BM_CTA = 128;
+constexpr int kThreads = 256;
+constexpr int kTmemCols = 512;
+constexpr int kABytes = BM_CTA * BK * 2;   // 16 KB
+
+template <int CG> struct Cfg {
+  static constexpr int kBRows = BN / CG;                 // B rows staged by one CTA
+  static constexpr int kBBytes = kBRows * BK * 2;
+  static constexpr int kStageBytes = kABytes + kBBytes;  // 32 KB (CG=2) / 48 KB (CG=1)
+  static constexpr int kStages = CG == 2 ? 6 : 4;
+  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+};
+
+// Work schedule.  An item is (M tile, run of N tiles); CTA pair p takes items p, p+P, ...
+struct Sched {
+  int64_t M, N, K;        // static extents of the problem
+  const int32_t* n_dyn;   // device scalar: dynamic row count of the whole batch (nullable)
+  int64_t dyn_row0;       // rows of the batch that precede this launch's chunk
+  int64_t dyn_cap;        // chunk capacity in rows
+  int dyn_dim;            // 0: none; 1: M = clamp(*n_dyn - row0, 0, cap); 2: same for K
+  int dyn_round;          // the dynamic extent is rounded up to a multiple of this (>= 1)
+  int chunk_ntiles;       // N tiles per item
+  int c_major;            // 1: items ordered (N chunk, M tile); 0: (M tile, N tile), chunk = 1
+};
+
+__device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t& K) {
+  M = s.M;
+  K = s.K;
+  if (s.dyn_dim != 0) {
+    int64_t n = (int64_t)(*s.n_dyn) - s.dyn_row0;
+    n = n < 0 ? 0 : (n > s.dyn_cap ? s.dyn_cap : n);
+    n = (n + s.dyn_round - 1) / s.dyn_round * s.dyn_round;
+    if (s.dyn_dim == 1) M = M < n ? M : n;
+    else K = K < n ? K : n;
+  }
+}
+
+struct Item { int64_t m_tile, n0, n1, c; };
+
+__device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt, int64_t Nt) {
+  Item x;
+  if (s.c_major) {
+    x.c = it / Mt;
+    x.m_tile = it - x.c * Mt;
+    x.n0 = x.c * s.chunk_ntiles;
+    x.n1 = x.n0 + s.chunk_ntiles < Nt ? x.n0 + s.chunk_ntiles : Nt;
+  } else {
+    x.m_tile = it / Nt;
+    x.n0 = it - x.m_tile * Nt;
+    x.n1 = x.n0 + 1;
+    x.c = 0;
+  }
+  return x;
+}
+
+template <int CG, bool A_MN, bool B_MN, class Epi>
+__global__ void __launch_bounds__(kThreads, 1)
+k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+          const Sched s, const typename Epi::Params ep) {
+  using C = Cfg<CG>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + C::kStages * C::kStageBytes;
+  // barrier layout (8 bytes each): full[kStages], empty[kStages], tmem_full[2], tmem_empty[2]
+  auto full_bar = [&](int i) { return bar_base + 8u * i; };
+  auto empty_bar = [&](int i) { return bar_base + 8u * (C::kStages + i); };
+  auto tfull_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + i); };
+  auto tempty_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + 2 + i); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = CG == 2 ? ptx::cluster_ctarank() : 0u;
+  const int64_t pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmA);
+    ptx::prefetch_tmap(&tmB);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < C::kStages; ++i) {
+      ptx::mbar_init(full_bar(i), 1);
+      ptx::mbar_init(empty_bar(i), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      ptx::mbar_init(tfull_bar(i), 1);
+      ptx::mbar_init(tempty_bar(i), 4 * CG);
+    }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc<CG>(tmem_slot, kTmemCols);
+    ptx::tmem_relinquish<CG>();
+  }
+  ptx::tc_fence_before();
+  if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  int64_t M_eff, K_eff;
+  resolve_dims(s, M_eff, K_eff);
+  const int64_t Mt = (M_eff + BM_CTA * CG - 1) / (BM_CTA * CG);
+  const int64_t Nt = (s.N + BN - 1) / BN;
+  const int64_t n_chunks = s.c_major ? (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles : Nt;
+  const int64_t n_items = Mt * n_chunks;
+  const int num_kb = (int)((K_eff + BK - 1) / BK);
+
+  if (warp == 0) {
+    // ===================== TMA producer (one lane, every CTA) =====================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int64_t it = pair; it < n_items; it += n_pairs) {
+        const Item item = get_item(s, it, Mt, Nt);
+        const int32_t m_coord = (int32_t)(item.m_tile * BM_CTA * CG + rank * BM_CTA);
+        for (int64_t n = item.n0; n < item.n1; ++n) {
+          const int32_t n_coord = (int32_t)(n * BN + rank * C::kBRows);
+          for (int kb = 0; kb < num_kb; ++kb) {
+            ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
+            const uint32_t sa = smem_base + stage * C::kStageBytes;
+            const uint32_t sb = sa + kABytes;
+            const int32_t k_coord = kb * BK;
+            if constexpr (CG == 1) {
+              ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes);
+              const uint32_t fb = full_bar(stage);
+              if constexpr (!A_MN) ptx::tma_load_2d(sa, &tmA, k_coord, m_coord, fb);
+              else {
+                ptx::tma_load_2d(sa, &tmA, m_coord, k_coord, fb);
+                ptx::tma_load_2d(sa + 8192, &tmA, m_coord + 64, k_coord, fb);
+              }
+              if constexpr (!B_MN) ptx::tma_load_2d(sb, &tmB, k_coord, n_coord, fb);
+              else {
+#pragma unroll
+                for (int b = 0; b < C::kBRows / 64; ++b)
+                  ptx::tma_load_2d(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb);
+              }
+            } else {
+              // the leader's barrier collects the bytes of both CTAs
+              if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes * 2);
+              const uint32_t fb = ptx::mapa(full_bar(stage), 0);
+              if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb);
+              else {
+                ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb);
+                ptx::tma_load_2d_cg2(sa + 8192, &tmA, m_coord + 64, k_coord, fb);
+              }
+              if constexpr (!B_MN) ptx::tma_load_2d_cg2(sb, &tmB, k_coord, n_coord, fb);
+              else {
+#pragma unroll
+                for (int b = 0; b < C::kBRows / 64; ++b)
+                  ptx::tma_load_2d_cg2(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb);
+              }
+            }
+            if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (one lane of the leader CTA) =====================
+    if (rank == 0 && lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_bf16(BM_CTA * CG, BN, A_MN, B_MN);
+      constexpr uint32_t a_step = A_MN ? (2048 >> 4) : (32 >> 4);   // per UMMA_K = 16
+      constexpr uint32_t b_step = B_MN ? (2048 >> 4) : (32 >> 4);
+      int stage = 0;
+      uint32_t phase = 0;
+      int acc = 0;
+      uint32_t acc_phase = 0;
+      for (int64_t it = pair; it < n_items; it += n_pairs) {
+        const Item item = get_item(s, it, Mt, Nt);
+        for (int64_t n = item.n0; n < item.n1; ++n) {
+          ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)acc * BN;
+          for (int kb = 0; kb < num_kb; ++kb) {
+            ptx::mbar_wait(full_bar(stage), phase);
+            ptx::tc_fence_after();
+            const uint32_t sa = smem_base + stage * C::kStageBytes;
+            const uint64_t adesc = ptx::make_smem_desc(sa, A_MN);
+            const uint64_t bdesc = ptx::make_smem_desc(sa + kABytes, B_MN);
+#pragma unroll
+            for (int k = 0; k < BK / 16; ++k)
+              ptx::umma_bf16<CG>(d_tmem, adesc + (uint64_t)(k * a_step),
+                                 bdesc + (uint64_t)(k * b_step), idesc, (uint32_t)(kb | k));
+            ptx::umma_commit<CG>(empty_bar(stage));      // frees the smem slot (both CTAs)
+            if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
+          }
+          ptx::umma_commit<CG>(tfull_bar(acc));          // accumulator ready (both CTAs)
+          if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue warps =====================
+    const int q = warp & 3;
+    const int row_in_tile = q * 32 + lane;
+    const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    typename Epi::State st;
+    Epi::setup(st, ep);
+    for (int64_t it = pair; it < n_items; it += n_pairs) {
+      const Item item = get_item(s, it, Mt, Nt);
+      const int64_t grow = item.m_tile * BM_CTA * CG + rank * BM_CTA + row_in_tile;
+      const bool valid = grow < M_eff;
+      Epi::item_begin(st, ep, grow, valid, item.c);
+      for (int64_t n = item.n0; n < item.n1; ++n) {
+        ptx::mbar_wait(tfull_bar(acc), acc_phase);
+        ptx::tc_fence_after();
+#pragma unroll 1
+        for (int ch = 0; ch < BN / 32; ++ch) {
+          uint32_t r[32];
+          __syncwarp();
+          if (num_kb > 0) {
+            ptx::tmem_ld_32x32(lane_base + (uint32_t)(acc * BN + ch * 32), r);
+            ptx::tmem_wait_ld();
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) r[j] = 0u;
+          }
+          if (ch == BN / 32 - 1) {
+            // all of this warp's reads of the accumulator are done: hand it back to the MMA
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              if constexpr (CG == 1) ptx::mbar_arrive(tempty_bar(acc));
+              else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
+            }
+          }
+          float x[32];
+#pragma unroll
+          for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+          Epi::chunk(st, ep, grow, valid, n * BN + ch * 32, x);
+        }
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+      Epi::item_end(st, ep, grow, valid, item.c);
+    }
+  }
+
+  // ---- teardown ----
+  ptx::tc_fence_before();
+  if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, kTmemCols);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                    const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline PFN_encodeTiled get_encode_fn() {
+  static PFN_encodeTiled fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess)
+      p = nullptr;
+    return reinterpret_cast<PFN_encodeTiled>(p);
+  }();
+  return fn;
+}
+
+// bf16 2-D row-major tensor [outer, inner] with row stride ld (elements), 128B-swizzled boxes.
+inline int make_tmap_bf16(CUtensorMap* m, const void* base, int64_t inner, int64_t outer,
+                          int64_t ld, int box_inner, int box_outer) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return GC_ERR_CUDA;
+  if (inner <= 0 || outer <= 0) return GC_ERR_SHAPE;
+  if ((reinterpret_cast<uintptr_t>(base) & 15) || ((ld * 2) & 15)) return GC_ERR_ALIGN;
+  cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  cuuint32_t box[2] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides,
+                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? GC_OK : GC_ERR_CUDA;
+}
+
+// Operand X of a GEMM with `rows` along M (or N) and `K` along the contraction:
+//   K-major  : memory is [rows, K] (ld >= K)   -> box {64 k, box_rows}
+//   MN-major : memory is [K, rows] (ld >= rows) -> box {64 rows, 64 k}
+inline int make_operand_tmap(CUtensorMap* m, const void* base, int64_t rows, int64_t K, int64_t ld,
+                             bool mn_major, int box_rows) {
+  if (!mn_major) return make_tmap_bf16(m, base, K, rows, ld, BK, box_rows);
+  return make_tmap_bf16(m, base, rows, K, ld, 64, BK);
+}
+
+inline int num_sms() {
+  int dev = 0, n = kNumSMs;
+  if (cudaGetDevice(&dev) == cudaSuccess)
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+  return n;
+}
+
+template <int CG, bool A_MN, bool B_MN, class Epi>
+int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& s,
+                   const typename Epi::Params& ep, cudaStream_t st) {
+  auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi>;
+  GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   Cfg<CG>::kSmemBytes));
+  cudaLaunchConfig_t cfg = {};
+  const int sms = num_sms();
+  cfg.gridDim = dim3((unsigned)(sms / CG * CG));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = Cfg<CG>::kSmemBytes;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  GC_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tmA, tmB, s, ep));
+  return GC_OK;
+}
+
+}  // namespace tc
+}  // namespace gc

@@ -1,0 +1,396 @@
+// tc_head.cu -- the four dense contractions of the path on the tcgen05 tile engine, each with
+// its fused epilogue:
+//   a2+a3  forward      S = Hs W^T            -> online (m, s, u, a_y) row statistics, split over V
+//   a10    recompute    S = Hs W^T again      -> dS = (g/tau)(onehot - exp(S/tau - lse)), bf16
+//   a11    dH           dH = dS W             -> bf16 rows scattered to their original positions
+//   a12    dW           dW (+)= dS^T Hs       -> fp32
+#include "tc_gemm.cuh"
+
+#ifndef GC_DEFAULT_CG
+#define GC_DEFAULT_CG 2
+#endif
+
+namespace gc {
+
+using tc::Sched;
+
+// ---------------------------------------------------------------------------------------------
+// Epilogue a3: online log-softmax statistics in log2 units (a = x * log2(e)/tau).
+// A thread owns one row; state lives in registers across the N tiles of an item.
+// ---------------------------------------------------------------------------------------------
+struct EpiStats {
+  struct Params {
+    const int32_t* targets;   // [rows] compact targets
+    RowStat* partials;        // [n_split][split_stride]
+    int64_t split_stride;
+    int64_t V;
+    float c;                  // log2(e) / tau
+  };
+  struct State { float m, s0, s1, u0, u1, ay; int32_t y; };
+  static __device__ __forceinline__ void setup(State&, const Params&) {}
+
+  static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
+                                                    bool valid, int64_t) {
+    st.y = valid ? p.targets[row] : -1;
+    st.m = -1e30f;
+    st.s0 = st.s1 = st.u0 = st.u1 = 0.f;
+    st.ay = -INFINITY;
+  }
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t, bool,
+                                               int64_t col0, const float (&x)[32]) {
+    if (col0 >= p.V) return;
+    const bool full = col0 + 32 <= p.V;
+    const int nvalid = full ? 32 : (int)(p.V - col0);
+    float cm = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) cm = (full || j < nvalid) ? fmaxf(cm, x[j]) : cm;
+    const float mnew = fmaxf(st.m, cm * p.c);
+    const float dm = st.m - mnew;
+    const float sc = ptx::ex2(dm);
+    st.u0 = (st.u0 + dm * st.s0) * sc;
+    st.u1 = (st.u1 + dm * st.s1) * sc;
+    st.s0 *= sc;
+    st.s1 *= sc;
+    st.m = mnew;
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      const float t0 = fmaf(x[j], p.c, -mnew), t1 = fmaf(x[j + 1], p.c, -mnew);
+      float e0 = ptx::ex2(t0), e1 = ptx::ex2(t1);
+      if (!full) { e0 = j < nvalid ? e0 : 0.f; e1 = j + 1 < nvalid ? e1 : 0.f; }
+      st.s0 += e0;
+      st.s1 += e1;
+      st.u0 = fmaf(e0, t0, st.u0);
+      st.u1 = fmaf(e1, t1, st.u1);
+    }
+    const uint32_t rel = (uint32_t)((int64_t)st.y - col0);
+    if (st.y >= 0 && rel < 32u) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) st.ay = (rel == (uint32_t)j) ? x[j] * p.c : st.ay;
+    }
+  }
+  static __device__ __forceinline__ void item_end(State& st, const Params& p, int64_t row,
+                                                  bool valid, int64_t c) {
+    if (!valid) return;
+    RowStat o;
+    o.m = st.m;
+    o.s = st.s0 + st.s1;
+    o.u = st.u0 + st.u1;
+    o.ay = st.ay;
+    p.partials[c * p.split_stride + row] = o;
+  }
+};
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Epilogue a10: dS[r, v] = (g_r/tau) (1[v = y_r] - 2^(a - lse2)) in bf16; zeros for rows past the
+// dynamic row count and for columns >= V (the dW contraction runs over those rows).
+// ---------------------------------------------------------------------------------------------
+struct EpiDS {
+  struct Params {
+    const int32_t* targets;   // chunk-local compact arrays
+    const float* lse;
+    const float* g;
+    __nv_bfloat16* dS;        // [rows_cap, ldS]
+    int64_t ldS;
+    int64_t V;
+    float c;                  // log2(e) / tau
+    float inv_tau;
+    const int32_t* n_dyn;     // device scalar: dynamic row count of the batch (nullable)
+    int64_t row0;             // rows of the batch before this chunk
+    int64_t n_static;         // rows of this chunk when n_dyn == NULL
+    int64_t cap;              // chunk capacity
+  };
+  struct State { float lse2, gp; int32_t y; int64_t n_eff; };
+  static __device__ __forceinline__ void setup(State& st, const Params& p) {
+    int64_t n = p.n_static;
+    if (p.n_dyn) {
+      n = (int64_t)(*p.n_dyn) - p.row0;
+      n = n < 0 ? 0 : (n > p.cap ? p.cap : n);
+    }
+    st.n_eff = n;
+  }
+
+  static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
+                                                    bool valid, int64_t) {
+    st.y = -1; st.lse2 = 0.f; st.gp = 0.f;
+    if (valid && row < st.n_eff) {
+      st.y = p.targets[row];
+      st.gp = p.g[row] * p.inv_tau;
+      st.lse2 = p.lse[row] * kLog2e;
+      if (st.y < 0) st.gp = 0.f;
+    }
+  }
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool,
+                                               int64_t col0, const float (&x)[32]) {
+    if (col0 >= p.ldS) return;
+    float v[32];
+    if (st.gp == 0.f) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] = 0.f;
+    } else {
+      const float ng = -st.gp;
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] = ng * ptx::ex2(fmaf(x[j], p.c, -st.lse2));
+      const uint32_t rel = (uint32_t)((int64_t)st.y - col0);
+      if (rel < 32u) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = (rel == (uint32_t)j) ? v[j] + st.gp : v[j];
+      }
+      if (col0 + 32 > p.V) {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = (col0 + j < p.V) ? v[j] : 0.f;
+      }
+    }
+    uint4* dst = reinterpret_cast<uint4*>(p.dS + row * p.ldS + col0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (col0 + 8 * q < p.ldS)
+        dst[q] = make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
+                            pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
+    }
+  }
+  static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+};
+
+// ---------------------------------------------------------------------------------------------
+// Epilogue a11: store bf16 rows, optionally scattered through rows[] (dH of compacted tokens).
+// ---------------------------------------------------------------------------------------------
+struct EpiStoreBf16 {
+  struct Params {
+    __nv_bfloat16* out;
+    int64_t ldo;
+    const int32_t* rows;      // nullable; chunk-local
+    int64_t row_base;         // used when rows == NULL
+    int64_t N;
+  };
+  struct State { int64_t orow; };
+  static __device__ __forceinline__ void setup(State&, const Params&) {}
+  static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
+                                                    bool valid, int64_t) {
+    st.orow = valid ? (p.rows ? (int64_t)p.rows[row] : p.row_base + row) : -1;
+  }
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t, bool,
+                                               int64_t col0, const float (&x)[32]) {
+    if (st.orow < 0 || col0 >= p.N) return;
+    uint4* dst = reinterpret_cast<uint4*>(p.out + st.orow * p.ldo + col0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (col0 + 8 * q < p.N)
+        dst[q] = make_uint4(pack_bf16x2(x[8 * q], x[8 * q + 1]), pack_bf16x2(x[8 * q + 2], x[8 * q + 3]),
+                            pack_bf16x2(x[8 * q + 4], x[8 * q + 5]), pack_bf16x2(x[8 * q + 6], x[8 * q + 7]));
+    }
+  }
+  static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+};
+
+// ---------------------------------------------------------------------------------------------
+// Epilogue a12 (and the debug GEMM): fp32 store or accumulate.
+// ---------------------------------------------------------------------------------------------
+struct EpiStoreF32 {
+  struct Params {
+    float* out;
+    int64_t ldo;
+    int64_t N;
+    int accumulate;
+  };
+  struct State { int dummy; };
+  static __device__ __forceinline__ void setup(State&, const Params&) {}
+  static __device__ __forceinline__ void item_begin(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void chunk(State&, const Params& p, int64_t row, bool valid,
+                                               int64_t col0, const float (&x)[32]) {
+    if (!valid || col0 >= p.N) return;
+    float4* dst = reinterpret_cast<float4*>(p.out + row * p.ldo + col0);
+    if (p.accumulate) {
+      float4 prev[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        prev[q] = (col0 + 4 * q < p.N) ? dst[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (col0 + 4 * q < p.N)
+          dst[q] = make_float4(prev[q].x + x[4 * q], prev[q].y + x[4 * q + 1],
+                               prev[q].z + x[4 * q + 2], prev[q].w + x[4 * q + 3]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 8; ++q)
+        if (col0 + 4 * q < p.N) dst[q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
+    }
+  }
+  static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+};
+
+// ---------------------------------------------------------------------------------------------
+// forward plan: choose the number of N tiles per item so that the items balance over the CTA
+// pairs (wave quantisation, SURVEY.md sec 7.2 hard part 5); prefer longer items on ties.
+// ---------------------------------------------------------------------------------------------
+TcPlan tc_plan_forward(int64_t T, int64_t V) {
+  const int P = kNumSMs / 2;
+  const int64_t Mt = ceil_div(T > 0 ? T : 1, 256);
+  const int64_t Nt = ceil_div(V, tc::BN);
+  TcPlan best{(int)Nt, 1, (int)Nt};
+  double best_cost = 1e300;
+  const int64_t kmin = ceil_div(Nt, 160);                // at most 160 partial slots per row
+  for (int64_t k = kmin > 1 ? kmin : 1; k <= 64 && k <= Nt; ++k) {
+    const int64_t C = ceil_div(Nt, k);
+    const int64_t k_last = Nt - (C - 1) * k;
+    const int64_t items = C * Mt;
+    int64_t worst = 0;
+    for (int p = 0; p < P; ++p) {
+      if (p >= items) break;
+      const int64_t n_p = (items - 1 - p) / P + 1;
+      // items of the last chunk: indices [(C-1)*Mt, C*Mt) congruent to p mod P
+      const int64_t lo = (C - 1) * Mt, hi = C * Mt;
+      int64_t first = lo + ((p - lo % P) % P + P) % P;
+      const int64_t n_last = first < hi ? (hi - 1 - first) / P + 1 : 0;
+      const int64_t load = (n_p - n_last) * k + n_last * k_last;
+      worst = load > worst ? load : worst;
+    }
+    // cost: makespan in tiles, plus a small charge per item flush
+    const double cost = (double)worst * (1.0 + 0.02 / (double)k);
+    if (cost <= best_cost) {
+      best_cost = cost;
+      best.chunk_vtiles = (int)k;
+      best.n_split = (int)C;
+    }
+  }
+  best.n_vtiles = (int)Nt;
+  return best;
+}
+
+size_t tc_fwd_partials_bytes(int64_t T, int64_t V) {
+  const TcPlan pl = tc_plan_forward(T, V);
+  const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
+  return align_up((size_t)pl.n_split * (size_t)cap * sizeof(RowStat), 256);
+}
+
+template <class Epi, bool A_MN, bool B_MN>
+static int launch_cg(int cg, const CUtensorMap& a, const CUtensorMap& b, const Sched& s,
+                     const typename Epi::Params& ep, cudaStream_t st) {
+  if (cg == 2) return tc::launch_tc_gemm<2, A_MN, B_MN, Epi>(a, b, s, ep, st);
+  return tc::launch_tc_gemm<1, A_MN, B_MN, Epi>(a, b, s, ep, st);
+}
+
+static Sched make_sched(int64_t M, int64_t N, int64_t K) {
+  Sched s;
+  s.M = M; s.N = N; s.K = K;
+  s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
+  s.chunk_ntiles = 1; s.c_major = 0;
+  return s;
+}
+
+int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T, int64_t D,
+                     int64_t V, float tau, const int32_t* targets_c, const int32_t* n_rows_dev,
+                     RowStat* partials, cudaStream_t st) {
+  const int cg = GC_DEFAULT_CG;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / cg));
+  const TcPlan pl = tc_plan_forward(T, V);
+  Sched s = make_sched(T, V, D);
+  s.chunk_ntiles = pl.chunk_vtiles;
+  s.c_major = 1;
+  if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = 0; s.dyn_cap = T; }
+  EpiStats::Params ep;
+  ep.targets = targets_c;
+  ep.partials = partials;
+  ep.split_stride = ceil_div(T, 256) * 256;
+  ep.V = V;
+  ep.c = kLog2e / tau;
+  return launch_cg<EpiStats, false, false>(cg, ta, tb, s, ep, st);
+}
+
+int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,
+                    int64_t n_static, int64_t D, int64_t V, float tau, const int32_t* targets_c,
+                    const float* lse_c, const float* g_c, const int32_t* n_rows_dev, int64_t row0,
+                    void* dS, int64_t ldS, cudaStream_t st) {
+  const int cg = GC_DEFAULT_CG;
+  const int64_t h_rows = n_rows_dev ? rows_cap : n_static;   // rows behind the H pointer
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, H, h_rows, D, ldH, false, tc::BM_CTA));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / cg));
+  // rows up to the next multiple of 256 past the valid count are written as zeros: the dW
+  // contraction runs over them (rows_cap is a multiple of 256)
+  Sched s = make_sched(ceil_div(h_rows, 256) * 256, V, D);
+  const TcPlan pl = tc_plan_forward(rows_cap, V);
+  s.chunk_ntiles = pl.chunk_vtiles;
+  s.c_major = 1;
+  if (n_rows_dev) {
+    s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; s.dyn_round = 256;
+  }
+  EpiDS::Params ep;
+  ep.n_dyn = n_rows_dev;
+  ep.row0 = row0;
+  ep.n_static = n_static;
+  ep.cap = rows_cap;
+  ep.targets = targets_c;
+  ep.lse = lse_c;
+  ep.g = g_c;
+  ep.dS = static_cast<__nv_bfloat16*>(dS);
+  ep.ldS = ldS;
+  ep.V = V;
+  ep.c = kLog2e / tau;
+  ep.inv_tau = 1.0f / tau;
+  return launch_cg<EpiDS, false, false>(cg, ta, tb, s, ep, st);
+}
+
+int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* W,
+          int64_t ldW, int64_t D, int64_t V, const int32_t* rows, const int32_t* n_rows_dev,
+          int64_t row0, void* dH, int64_t lddH, cudaStream_t st) {
+  const int cg = GC_DEFAULT_CG;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, dS, rows_cap, V, ldS, false, tc::BM_CTA));
+  GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
+  Sched s = make_sched(n_rows_dev ? rows_cap : n_static, D, V);
+  if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
+  EpiStoreBf16::Params ep;
+  ep.out = static_cast<__nv_bfloat16*>(dH);
+  ep.ldo = lddH;
+  ep.rows = rows;
+  ep.row_base = row0;
+  ep.N = D;
+  return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st);
+}
+
+int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
+          int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
+          int64_t lddW, int accumulate, cudaStream_t st) {
+  const int cg = GC_DEFAULT_CG;
+  const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
+  GC_TRY(tc::make_operand_tmap(&tb, Hs, D, k_rows, ldH, true, 0));
+  Sched s = make_sched(V, D, k_rows);
+  if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 2; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
+  EpiStoreF32::Params ep;
+  ep.out = dW;
+  ep.ldo = lddW;
+  ep.N = D;
+  ep.accumulate = accumulate;
+  return launch_cg<EpiStoreF32, true, true>(cg, ta, tb, s, ep, st);
+}
+
+int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
+                  float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
+                  int cta_group, cudaStream_t st) {
+  if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
+  if (N % 4 != 0) return GC_ERR_SHAPE;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
+  GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, tc::BN / cta_group));
+  Sched s = make_sched(M, N, K);
+  EpiStoreF32::Params ep;
+  ep.out = C;
+  ep.ldo = ldc;
+  ep.N = N;
+  ep.accumulate = accumulate;
+  if (!a_mn && !b_mn) return launch_cg<EpiStoreF32, false, false>(cta_group, ta, tb, s, ep, st);
+  if (!a_mn && b_mn) return launch_cg<EpiStoreF32, false, true>(cta_group, ta, tb, s, ep, st);
+  if (a_mn && !b_mn) return launch_cg<EpiStoreF32, true, false>(cta_group, ta, tb, s, ep, st);
+  return launch_cg<EpiStoreF32, true, true>(cta_group, ta, tb, s, ep, st);
+}
+
+}  // namespace gc

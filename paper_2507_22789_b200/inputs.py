@@ -172,6 +172,27 @@ def sample_targets(H: torch.Tensor, W: torch.Tensor, tau: float = 1.0, seed: int
     return y
 
 
+def proxy_policy_logp(H: torch.Tensor, W: torch.Tensor, y: torch.Tensor, tau: float = 1.0,
+                      chunk: int = 1024) -> np.ndarray:
+    """Approximate policy log-probs by plain torch ops (fp32 log_softmax over chunked logits).
+
+    INPUT SYNTHESIS ONLY, for batches too large for the oracle: it centres the synthetic
+    old/ref log-probs ("policy log-probs + N(0, std)", configs[0]) so that the ratio
+    exp(logp - old) is near 1.  Neither the CUDA path nor the oracle calls it, and its values
+    are never used as expected results."""
+    T = H.shape[0]
+    out = torch.empty(T, dtype=torch.float32, device=H.device)
+    Wf = W if H.is_cuda else W.float()
+    for a in range(0, T, chunk):
+        b = min(T, a + chunk)
+        Hc = H[a:b] if H.is_cuda else H[a:b].float()
+        z = (Hc @ Wf.T).float() / tau
+        lp = torch.log_softmax(z, dim=1)
+        idx = y[a:b].clamp(min=0).long().unsqueeze(1)
+        out[a:b] = lp.gather(1, idx).squeeze(1)
+    return out.cpu().numpy().astype(np.float64)
+
+
 def perturb_logp(policy_logp, std: float, seed: int) -> np.ndarray:
     """old / ref log-probs = policy log-probs + N(0, std), fp32 (configs[0])."""
     rng = np.random.default_rng(seed)

@@ -1,0 +1,289 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the fp64 oracle on the same
+seeded inputs.  Tolerances (BASELINE.json:north_star, outer limits): |dlogp|, |dentropy| <= 1e-2;
+loss relative error <= 1e-3; gradient relative Frobenius error <= 2e-2; integers bit-exact.
+Internal bars are an order tighter and are what the asserts use.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+from paper_2507_22789_b200 import inputs as I
+from tests.helpers import make_batch, oracle_run, rel_fro, to_f64
+
+pytestmark = pytest.mark.gpu
+
+# internal bars
+TOL_LOGP_BF16 = 1e-4      # fp32 accumulation of exact bf16 products vs fp64
+TOL_LOGP_F32 = 2e-5       # fp32 SIMT path (config 0 bar is 1e-5 on logp; entropy a bit looser)
+TOL_LOSS_REL = 1e-3
+TOL_GRAD_BF16 = 5e-3      # dS rounded to bf16 (1.6e-3) + bf16 dH output rounding (2.3e-3)
+TOL_GRAD_F32 = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "these tests need a B200"
+    from paper_2507_22789_b200 import binding          # raises if libgcore.so is missing
+    return binding
+
+
+def dev(x, dtype=None):
+    t = torch.as_tensor(x)
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+# ------------------------------------------------------------------ tile engine unit tests
+@pytest.mark.parametrize("cg", [1, 2])
+@pytest.mark.parametrize("a_mn,b_mn", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K", [(128, 256, 64), (392, 520, 200), (1000, 776, 1096)])
+def test_engine_gemm(B, cg, a_mn, b_mn, M, N, K):
+    g = torch.Generator(device="cuda").manual_seed(M + N + K)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    C = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
+                             a_mn, b_mn, cta_group=cg)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    C2 = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
+                              a_mn, b_mn, C_out=C.clone(), accumulate=True, cta_group=cg)
+    assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+
+
+# ------------------------------------------------------------------ a6/a7 advantages
+@pytest.mark.parametrize("unbiased", [False, True])
+@pytest.mark.parametrize("drop", [False, True])
+def test_advantages_and_filter(B, unbiased, drop):
+    r = np.random.default_rng(3)
+    sizes = r.integers(1, 40, 300)
+    sizes[5] = 0
+    go = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int32)
+    rew = (r.random(go[-1]) < 0.5).astype(np.float32)
+    rew[go[7]:go[8]] = r.random(sizes[7]).astype(np.float32)
+    rew[go[9]:go[10]] = 0.25
+    adv, keep = B.gc_grpo_advantages(dev(rew), dev(go), 1e-6, unbiased, drop)
+    with np.errstate(invalid="ignore"):
+        a_ref, k_ref = O.grpo_advantages(rew, go, 1e-6, unbiased, drop)
+    a = adv.cpu().numpy()
+    ok = np.isfinite(a_ref)
+    assert np.array_equal(keep.cpu().numpy()[sizes > 0], k_ref[sizes > 0])      # bit-exact
+    assert np.allclose(a[ok], a_ref[ok].astype(np.float32), rtol=3e-7, atol=1e-9)
+    if drop:
+        assert np.array_equal(keep.cpu().numpy()[sizes > 0], O.group_filter(rew, go)[sizes > 0])
+
+
+# ------------------------------------------------------------------ a1 row selection
+@pytest.mark.parametrize("T,p", [(1, 1.0), (5000, 0.75), (70001, 0.3), (4096, 0.0)])
+def test_compaction_bit_exact(B, T, p):
+    r = np.random.default_rng(T)
+    mask = (r.random(T) < p).astype(np.uint8)
+    y = r.integers(0, 100, T).astype(np.int32)
+    y[r.random(T) < 0.1] = -100
+    H = torch.randn(T, 64, device="cuda").to(torch.bfloat16)
+    rows, n, Hs = B.gc_compact_rows(H, dev(y), dev(mask))
+    ref = np.nonzero((mask != 0) & (y >= 0))[0]
+    assert int(n.item()) == len(ref)
+    assert np.array_equal(rows.cpu().numpy()[:len(ref)], ref.astype(np.int32))
+    assert torch.equal(Hs[:len(ref)], H[torch.from_numpy(ref).cuda()])
+    rows2, n2, _ = B.gc_compact_rows(H, dev(y), None, gather=False)
+    assert int(n2.item()) == int((y >= 0).sum())
+
+
+# ------------------------------------------------------------------ a8/a9 loss kernels alone
+def _loss_inputs(T, R, seed, old_std=0.3, p_mask=0.75):
+    r = np.random.default_rng(seed)
+    cuts = np.sort(r.choice(np.arange(1, T), R - 1, replace=False)) if R > 1 else np.zeros(0, int)
+    cu = np.concatenate([[0], cuts, [T]]).astype(np.int32)
+    logp = (-3.0 * r.random(T)).astype(np.float32)
+    old = (logp + r.normal(0, old_std, T)).astype(np.float32)
+    ref = (logp + r.normal(0, 0.1, T)).astype(np.float32)
+    adv = r.normal(size=R).astype(np.float32)
+    mask = (r.random(T) < p_mask).astype(np.uint8)
+    y = r.integers(0, 1000, T).astype(np.int32)
+    y[r.random(T) < 0.05] = -1
+    return logp, old, ref, adv, mask, y, cu
+
+
+@pytest.mark.parametrize("agg", [O.AGG_TOKEN_MEAN, O.AGG_SEQ_MEAN])
+@pytest.mark.parametrize("T,R", [(7, 2), (4099, 37), (200003, 511)])
+def test_token_loss_kernels(B, agg, T, R):
+    logp, old, ref, adv, mask, y, cu = _loss_inputs(T, R, T + R)
+    out5, g = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu),
+                                   dev(adv), 0.2, 0.2, 0.04, agg, grad_loss=1.5)
+    scored = (mask != 0) & (y >= 0)
+    res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg)
+    g_ref = O.grpo_loss_grad_logp(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg, 1.5)
+    o = out5.cpu().numpy().astype(np.float64)
+    assert o[4] == res["n_scored"]                                        # integer, exact
+    assert abs(o[0] - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+    assert abs(o[1] - res["pg_loss"]) <= 1e-5 * max(abs(res["pg_loss"]), 1e-2)
+    assert abs(o[2] - res["kl_mean"]) <= 1e-5 * max(abs(res["kl_mean"]), 1e-3)
+    assert (T < 1000 or res["clip_frac"] > 0.05) and abs(o[3] - res["clip_frac"]) <= 2.0 / max(res["n_scored"], 1)
+    gg = g.cpu().numpy().astype(np.float64)
+    # both sides decide the clip branch from the same fp32 inputs; exclude float near-ties
+    resp = O.token_to_response(cu, T)
+    rho = np.exp(logp.astype(np.float64) - old)
+    near = (np.abs(rho - 1.2) < 1e-5) | (np.abs(rho - 0.8) < 1e-5)
+    assert np.all(gg[~scored] == 0.0)
+    assert np.allclose(gg[~near], g_ref[~near], rtol=2e-5, atol=2e-6 * np.abs(g_ref).max())
+    assert near.sum() < 0.001 * T + 2
+
+
+def test_token_loss_edge_cases(B):
+    logp, old, ref, adv, mask, y, cu = _loss_inputs(1000, 10, 5)
+    # sum m = 0 -> loss 0, g 0 (reading 12)
+    out5, g = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(np.zeros_like(mask)),
+                                   dev(cu), dev(adv))
+    assert out5.cpu().tolist() == [0.0, 0.0, 0.0, 0.0, 0.0] and float(g.abs().max()) == 0.0
+    # beta = 0 with ref = NULL; mask = NULL
+    out5, _ = B.gc_grpo_token_loss(dev(logp), dev(old), None, dev(y), None, dev(cu), dev(adv),
+                                   beta=0.0)
+    res = O.grpo_loss(logp, old, None, y >= 0, adv, cu, beta=0.0)
+    assert abs(out5[0].item() - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+    # logp == old, beta = 0: loss = -sum(m A)/sum(m)   (north_star invariant)
+    out5, _ = B.gc_grpo_token_loss(dev(logp), dev(logp), dev(ref), dev(y), dev(mask), dev(cu),
+                                   dev(adv), beta=0.0)
+    scored = (mask != 0) & (y >= 0)
+    A = adv[O.token_to_response(cu, 1000)]
+    assert abs(out5[0].item() + (A * scored).sum() / scored.sum()) < 1e-6
+    assert out5[3].item() == 0.0
+    # logp == ref: KL = 0
+    out5, _ = B.gc_grpo_token_loss(dev(logp), dev(old), dev(logp), dev(y), dev(mask), dev(cu),
+                                   dev(adv))
+    assert out5[2].item() == 0.0
+    # rerun determinism: bit-identical
+    a, ga = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu), dev(adv))
+    b, gb = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu), dev(adv))
+    assert torch.equal(a, b) and torch.equal(ga, gb)
+
+
+# ------------------------------------------------------------------ whole path helper
+def run_gpu(B, b, agg=0, backward=True, chunk_tokens=0, simt=False, grad_loss=1.0):
+    w = b.w
+    adv, keep = B.gc_grpo_advantages(b.rewards_t, b.go_t, 1e-6, False, False)
+    f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                           w.clip_lo, w.clip_hi, w.beta, agg, simt=simt)
+    out = dict(adv=adv, keep=keep, **f)
+    if backward:
+        dH, dW = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                                    f["logp"], f["lse"], w.clip_lo, w.clip_hi, w.beta, agg,
+                                    grad_loss, chunk_tokens=chunk_tokens, simt=simt)
+        out.update(dH=dH, dW=dW)
+    torch.cuda.synchronize()
+    return out
+
+
+def check_against_oracle(b, got, ref, tol_lp, tol_grad, backward=True):
+    lp = got["logp"].cpu().numpy().astype(np.float64)
+    en = got["entropy"].cpu().numpy().astype(np.float64)
+    ls = got["lse"].cpu().numpy().astype(np.float64)
+    s = b.scored_np
+    assert np.all(lp[~s] == 0) and np.all(en[~s] == 0) and np.all(ls[~s] == 0)
+    assert np.abs(lp - ref["logp"]).max() <= tol_lp
+    assert np.abs(en - ref["entropy"]).max() <= tol_lp * 2
+    assert np.abs(ls - ref["lse"]).max() <= tol_lp
+    o = got["out5"].cpu().numpy().astype(np.float64)
+    assert o[4] == ref["n_scored"]
+    scale = max(abs(ref["loss"]), 1e-300)
+    assert abs(o[0] - ref["loss"]) <= TOL_LOSS_REL * scale, (o[0], ref["loss"])
+    assert abs(o[1] - ref["pg_loss"]) <= TOL_LOSS_REL * max(abs(ref["pg_loss"]), 1e-300)
+    assert abs(o[2] - ref["kl_mean"]) <= TOL_LOSS_REL * max(abs(ref["kl_mean"]), 1e-300)
+    assert abs(o[3] - ref["clip_frac"]) <= 2.0 / max(ref["n_scored"], 1)
+    if backward:
+        dH = got["dH"].float().cpu().numpy()
+        dW = got["dW"].cpu().numpy()
+        assert np.all(dH[~s] == 0.0)                                   # masked rows exactly 0
+        assert rel_fro(dH, ref["dH"]) <= tol_grad, rel_fro(dH, ref["dH"])
+        assert rel_fro(dW, ref["dW"]) <= tol_grad, rel_fro(dW, ref["dW"])
+
+
+# ------------------------------------------------------------------ config 0 in full (fp32)
+@pytest.mark.parametrize("agg", [O.AGG_TOKEN_MEAN, O.AGG_SEQ_MEAN])
+def test_config0_full(B, agg):
+    b = make_batch(I.CONFIGS[0], seed=0, device="cuda")
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref, agg)
+    got = run_gpu(B, b, agg)
+    assert np.allclose(got["adv"].cpu().numpy(), adv_ref.astype(np.float32), rtol=3e-7, atol=1e-9)
+    check_against_oracle(b, got, ref, TOL_LOGP_F32, TOL_GRAD_F32)
+
+
+def test_f32_odd_shapes_masks_temperature(B):
+    w = I.reduced(I.CONFIGS[0], D=72, V=1001, groups=3, group_size=3, seq_len=0, tau=0.7,
+                  lognormal=(2.5, 0.8, 1, 60), prompt_len=2, old_std=0.3)
+    b = make_batch(w, seed=4, device="cuda")
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    for agg in (0, 1):
+        check_against_oracle(b, run_gpu(B, b, agg), oracle_run(b, adv_ref, agg), TOL_LOGP_F32,
+                             TOL_GRAD_F32)
+
+
+# ------------------------------------------------------------------ bf16 tcgen05 path, small shapes
+BF16_CASES = {
+    # spans several 256-row / 256-col tiles with ragged tails; D not a multiple of 64
+    "ragged": dict(D=200, V=4097 + 64, groups=3, group_size=4, seq_len=0, lognormal=(3.6, 0.6, 1, 200)),
+    "masked": dict(D=512, V=5000, groups=2, group_size=8, seq_len=48, prompt_len=12, old_std=0.3),
+    "tau": dict(D=1024, V=8192, groups=1, group_size=8, seq_len=64, tau=0.7),
+    "one_token": dict(D=64, V=300, groups=1, group_size=2, seq_len=0, lognormal=(0.0, 0.01, 1, 1)),
+}
+
+
+@pytest.mark.parametrize("name", list(BF16_CASES))
+def test_bf16_small_forward_backward(B, name):
+    w = I.reduced(I.CONFIGS[2], backward=True, **{"prompt_len": 0, **BF16_CASES[name]})
+    b = make_batch(w, seed=7, device="cuda")
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref)
+    got = run_gpu(B, b)
+    check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+    # the slow SIMT kernels on the same bf16 operands agree too (on-device cross-check path)
+    got2 = run_gpu(B, b, simt=True)
+    check_against_oracle(b, got2, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+
+
+def test_bf16_random_mask_negative_targets_chunks_accumulate(B):
+    w = I.reduced(I.CONFIGS[2], D=256, V=2048 + 8, groups=4, group_size=4, seq_len=40, prompt_len=0,
+                  old_std=0.3)
+    b0 = make_batch(w, seed=9, device="cpu")
+    mask = I.random_mask(b0.T, 0.6, 9)
+    b = make_batch(w, seed=9, device="cuda", mask=mask)
+    y = b.y_np.copy()
+    y[::17] = -100
+    b.y_np, b.y = y, torch.from_numpy(y).cuda()
+    b.scored_np = (b.mask_np != 0) & (y >= 0)
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    for agg in (0, 1):
+        ref = oracle_run(b, adv_ref, agg, grad_loss=0.5)
+        for chunk in (0, 256, 512):
+            got = run_gpu(B, b, agg, chunk_tokens=chunk, grad_loss=0.5)
+            check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+    # dense mode (mask = NULL) with negative targets only
+    b.mask_t, b.all_scored = None, True
+    b.mask_np = np.ones_like(b.mask_np)
+    b.scored_np = y >= 0
+    ref = oracle_run(b, adv_ref)
+    got = run_gpu(B, b)
+    check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+    # accumulate_dW adds to the existing contents; reruns are bit-identical
+    dW0 = torch.full_like(got["dW"], 0.25)
+    _, dW1 = B.gc_grpo_loss_bwd(b.H, b.W, b.y, None, w.tau, b.cu_t, got["adv"], b.old_t, b.ref_t,
+                                got["logp"], got["lse"], dW=dW0.clone(), accumulate_dW=True)
+    assert rel_fro((dW1 - 0.25).cpu().numpy(), ref["dW"]) <= TOL_GRAD_BF16
+    again = run_gpu(B, b)
+    for k in ("logp", "entropy", "lse", "out5", "dH", "dW"):
+        assert torch.equal(again[k], got[k]), k
+
+
+def test_bf16_empty_and_all_masked(B):
+    w = I.reduced(I.CONFIGS[2], D=128, V=512, groups=1, group_size=4, seq_len=8, prompt_len=0)
+    b = make_batch(w, seed=1, device="cuda", mask=np.zeros(32, np.uint8))
+    got = run_gpu(B, b)
+    assert float(got["logp"].abs().max()) == 0 and got["out5"].cpu().tolist() == [0.0] * 5
+    assert float(got["dH"].float().abs().max()) == 0 and float(got["dW"].abs().max()) == 0
+    # T = 0
+    H0 = torch.empty(0, 128, dtype=torch.bfloat16, device="cuda")
+    lp, en, ls = B.gc_token_logprobs(H0, b.W, torch.empty(0, dtype=torch.int32, device="cuda"))
+    assert lp.numel() == 0
+    assert B.gc_validate_targets(b.y, None, 512) == 0 and B.gc_validate_targets(b.y, None, 1) > 0

@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- scored tokens/s of the RLHF scoring hot path on B200 (BASELINE.json:metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg4|cfg0]
+                    [--impl ours|reference] [--no-extras]
+
+A step is one pass of the hot path over one synthetic micro-batch of the named workload
+(default cfg1 = BASELINE.json configs[1], the configuration the metric is quoted on: forward-only
+scoring of 16384 tokens, hidden 3584, vocab 152064, bf16).  Backward-capable workloads (cfg2,
+cfg4, cfg0) run advantages -> loss forward -> loss backward per step.  One JSON line on stdout.
+
+N > 1: launched under torch.distributed.run, one rank per GPU; whole groups are sharded across
+ranks (every rank scores its own micro-batch, weak scaling), no data-path collective.
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2507_22789_b200 import inputs as I  # noqa: E402
+
+WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4}
+SMI_FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], burst=d["bf16_tflops"], sustained=d["bf16_tflops_sustained"],
+                    source="measured")
+    return dict(hbm=6650.0, burst=1590.0, sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms during the timed region."""
+
+    def __init__(self, gpu_ids):
+        self.rows = []
+        self.proc = None
+        self.gpu_ids = gpu_ids
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={SMI_FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "50", "-i", ",".join(str(g) for g in self.gpu_ids)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)),
+                    power_w_max=float(max(pw)), samples=len(sm), reasons=sorted(reasons))
+
+
+# --------------------------------------------------------------------------------------------
+# synthetic batch on the device (recipe: DESIGN.md sec 4)
+# --------------------------------------------------------------------------------------------
+class DeviceBatch:
+    def __init__(self, w: I.Workload, seed: int, device):
+        self.w = w
+        lay = I.make_layout(w, seed)
+        self.lay = lay
+        self.T = lay.T
+        self.H, self.W = I.make_hw(lay.T, w.D, w.V, w.dtype, seed, device)
+        self.y = I.sample_targets(self.H, self.W, w.tau, seed)
+        self.mask = None if lay.mask.all() else torch.from_numpy(lay.mask).to(device)
+        self.n_scored = int(((lay.mask != 0) & (self.y.cpu().numpy() >= 0)).sum())
+        self.rewards = torch.from_numpy(I.make_rewards(w, seed)).to(device)
+        self.go = torch.from_numpy(lay.group_offsets).to(device)
+        self.cu = torch.from_numpy(lay.cu_seqlens).to(device)
+        if w.backward:
+            pol = I.proxy_policy_logp(self.H, self.W, self.y, w.tau)
+            self.old = torch.from_numpy(I.perturb_logp(pol, w.old_std, seed + 1)).to(device)
+            self.ref = torch.from_numpy(I.perturb_logp(pol, w.ref_std, seed + 2)).to(device)
+            self.dH = torch.empty(lay.T, w.D, dtype=self.H.dtype, device=device)
+            self.dW = torch.empty(w.V, w.D, dtype=torch.float32, device=device)
+
+
+def make_step(B, b: DeviceBatch):
+    """Returns (step_fn, launches_per_step, dominant_fn).  All work goes through the C ABI."""
+    w = b.w
+    compact = b.mask is not None
+    tc = w.dtype == "bf16"
+    fwd_launches = (2 + (6 if compact else 0)) if tc else 1
+    if not w.backward:
+        def step():
+            B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, w.drop_constant_groups)
+            return B.gc_token_logprobs(b.H, b.W, b.y, b.mask, w.tau, want_lse=False)
+        return step, 1 + fwd_launches
+
+    def step():
+        adv, _ = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, w.drop_constant_groups)
+        f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
+                               w.clip_hi, w.beta)
+        B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f["logp"],
+                           f["lse"], w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW)
+        return f["out5"]
+    # launches: advantages 1, fwd, loss 2, bwd: loss 2 + compaction 8 + 3 per chunk (or SIMT 2)
+    if tc:
+        n_chunks = -(-b.T // _bwd_chunk(B, b))
+        bwd = 2 + (8 if compact else 0) + 3 * n_chunks
+    else:
+        bwd = 2 + 2
+    return step, 1 + fwd_launches + 2 + bwd
+
+
+def _bwd_chunk(B, b):
+    # rows of the dS buffer the library picks: difference of two workspace queries
+    w = b.w
+    dt = B.GC_BF16
+    a = B.workspace_bytes(B.GC_OP_LOSS_BWD, b.T, w.D, w.V, dt, 0)
+    c256 = B.workspace_bytes(B.GC_OP_LOSS_BWD, b.T, w.D, w.V, dt, 256)
+    ld = -(-w.V // 64) * 64
+    return 256 + (a - c256) // (ld * 2)
+
+
+def timed_region(step, steps, warmup, dist_on, dominant=None):
+    """warmup untimed steps, then exactly `steps` steps between barriers; per-step CUDA events."""
+    import torch.distributed as dist
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    if dist_on:
+        dist.barrier()
+        torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(steps)]
+    t_all0, t_all1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_all0.record()
+    for i in range(steps):
+        ev[i][0].record()
+        step()
+        ev[i][1].record()
+    t_all1.record()
+    torch.cuda.synchronize()
+    if dist_on:
+        dist.barrier()
+        torch.cuda.synchronize()
+    total_ms = t_all0.elapsed_time(t_all1)
+    per = [a.elapsed_time(b) for a, b in ev]
+    if dist_on:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    return total_ms, per
+
+
+def cpu_baseline(w: I.Workload, budget_tokens: int, seed=0, min_seconds=10.0):
+    """The oracle, as it stands, on a bounded sample of the workload, on this box's host cores."""
+    import oracle as O
+    from threadpoolctl import threadpool_info
+    n = max(1, min(budget_tokens, w.seq_len if w.seq_len else budget_tokens))
+    ws = I.reduced(w, groups=1, group_size=2, seq_len=max(n // 2, 1), prompt_len=0)
+    lay = I.make_layout(ws, seed)
+    H, W = I.make_hw(lay.T, ws.D, ws.V, ws.dtype, seed, "cpu")
+    y = I.sample_targets(H, W, ws.tau, seed).numpy()
+    H64 = H.float().numpy().astype(np.float64)
+    W64 = W.float().numpy().astype(np.float64)
+    rew = np.array([1.0, 0.0], dtype=np.float32)
+    old = ref = None
+    if w.backward:
+        lp = O.token_logprobs(H64, W64, y, None, ws.tau)[0]
+        old = I.perturb_logp(lp, ws.old_std, 1)
+        ref = I.perturb_logp(lp, ws.ref_std, 2)
+    reps = 0
+    t0 = time.perf_counter()
+    while True:                       # repeat the sample until about 10 s of CPU work is done
+        adv, _ = O.grpo_advantages(rew, lay.group_offsets, 1e-6)
+        if w.backward:
+            O.grpo_forward_backward(H64, W64, y, None, ws.tau, lay.cu_seqlens, adv, old, ref,
+                                    ws.clip_lo, ws.clip_hi, ws.beta)
+        else:
+            O.token_logprobs(H64, W64, y, None, ws.tau)
+        reps += 1
+        dt = time.perf_counter() - t0
+        if dt >= min_seconds or reps >= 64:
+            break
+    threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    return dict(value=lay.T * reps / dt, unit="scored tokens/s", cores=int(threads), kind="oracle",
+                sample=f"{reps} x {lay.T} tokens of {w.name} (full D={w.D}, V={w.V}), "
+                       f"{'fwd+bwd' if w.backward else 'fwd'}, {dt:.1f} s, fp64 numpy",
+                seconds=dt)
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on host cores, same config/metric/unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    from threadpoolctl import threadpool_info
+    n_tok = 64 if w.D * w.V > 1e8 else w.groups * w.group_size * max(w.seq_len, 1)
+    ws = w if n_tok >= I.make_layout(w, 0).T else I.reduced(w, groups=1, group_size=2,
+                                                             seq_len=n_tok // 2, prompt_len=0)
+    lay = I.make_layout(ws, 0)
+    H, W = I.make_hw(lay.T, ws.D, ws.V, ws.dtype, 0, "cpu")
+    y = I.sample_targets(H, W, ws.tau, 0).numpy()
+    H64 = H.float().numpy().astype(np.float64)
+    W64 = W.float().numpy().astype(np.float64)
+    rew = I.make_rewards(ws, 0)
+    lp = O.token_logprobs(H64, W64, y, None, ws.tau)[0]
+    old, ref = I.perturb_logp(lp, ws.old_std, 1), I.perturb_logp(lp, ws.ref_std, 2)
+
+    def step():
+        adv, _ = O.grpo_advantages(rew, lay.group_offsets, 1e-6)
+        if w.backward:
+            O.grpo_forward_backward(H64, W64, y, None, ws.tau, lay.cu_seqlens, adv, old, ref,
+                                    ws.clip_lo, ws.clip_hi, ws.beta)
+        else:
+            O.token_logprobs(H64, W64, y, None, ws.tau)
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = lay.T * args.steps / dt
+    threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    unit = "scored tokens/s"
+    sample = f"{lay.T} tokens per step of {w.name} (full D={w.D}, V={w.V}), fp64 numpy oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": metric_name(w), "value": val, "unit": unit,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, lay.T, args.gpus),
+        "cpu_baseline": dict(value=val, unit=unit, cores=int(threads), kind="oracle", sample=sample),
+        "e2e": dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+    }))
+
+
+def metric_name(w):
+    return "scored tokens/sec (" + ("fwd+bwd" if w.backward else "fwd") + ")"
+
+
+def workload_config(w, T, n_gpus):
+    return {"workload": w.name, "tokens_per_gpu": T, "hidden": w.D, "vocab": w.V,
+            "groups": w.groups, "group_size": w.group_size, "temperature": w.tau,
+            "pass": "fwd+bwd" if w.backward else "fwd",
+            "parallelism": f"dp{n_gpus} (whole groups per rank, no data-path collective)",
+            "l2": "inputs exceed L2 (W alone is larger than 126 MB); no flush needed"}
+
+
+def e2e_measure(B, b: DeviceBatch, steps, warmup):
+    """Same metric through the C-ABI call with HOST buffers: per step H2D of H / targets / mask
+    from pinned memory, the kernels, D2H of logp + entropy, all inside the timed region."""
+    w = b.w
+    Hh = b.H.cpu().pin_memory()
+    yh = b.y.cpu().pin_memory()
+    mh = None if b.mask is None else b.mask.cpu().pin_memory()
+    lph = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    enh = torch.empty(b.T, dtype=torch.float32).pin_memory()
+
+    def step():
+        B.gc_token_logprobs_host(Hh, b.W, yh, mh, w.tau, logp_host=lph, entropy_host=enh)
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    h2d = Hh.numel() * Hh.element_size() + yh.numel() * 4 + (0 if mh is None else mh.numel())
+    return ms, h2d, 2 * b.T * 4, float(lph.sum())
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the cpu_baseline / e2e / fwd+bwd extras (rank 0, N=1 only)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = I.CONFIGS[WORKLOADS[args.workload]]
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    dist_on = world > 1
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if dist_on:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2507_22789_b200 import binding as B      # raises if libgcore.so is missing
+    peaks = load_peaks()
+
+    b = DeviceBatch(w, seed=rank, device=torch.device("cuda", local_rank))
+    step, launches = make_step(B, b)
+    sampler = ClockSampler(list(range(world)) if rank == 0 else [])
+    if rank == 0:
+        sampler.start()
+    total_ms, per = timed_region(step, args.steps, args.warmup, dist_on)
+    clocks = sampler.stop() if rank == 0 else None
+    ms_per_step = total_ms / args.steps
+    tokens = b.n_scored
+    if dist_on:
+        import torch.distributed as dist
+        t = torch.tensor([tokens], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t)
+        tokens_all = float(t.item())
+    else:
+        tokens_all = float(tokens)
+    value = tokens_all / (ms_per_step * 1e-3)
+
+    if rank == 0:
+        passes = 4 if w.backward else 1
+        flops = 2.0 * tokens * w.D * w.V * passes          # algorithmic: scored rows only
+        step_ms = float(np.mean(per))
+        achieved = flops / (step_ms * 1e-3) / 1e12
+        long_run = total_ms > 1000.0
+        peak = peaks["sustained"] if long_run else peaks["burst"]
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+        if os.path.exists(tp):
+            traffic = json.load(open(tp)).get(w.name)
+        out = {
+            "metric": metric_name(w), "value": value, "unit": "scored tokens/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32",
+            "data": "synthetic", "config": workload_config(w, b.T, world),
+            "clocks": clocks, "gpu_launches": launches * args.steps,
+            "roofline": {
+                "bound": "tensor", "kernel": "k_tc_gemm (tcgen05 LM-head contraction + fused epilogue)",
+                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "peak_kind": ("sustained" if long_run else "burst") + " cuBLAS bf16, " + peaks["source"],
+                "frac_of_burst": achieved / peaks["burst"],
+                "frac_of_sustained": achieved / peaks["sustained"],
+                "frac_of_nominal_2250": achieved / 2250.0,
+                "flops_per_step": flops, "kernel_ms": step_ms, "traffic": traffic,
+                "note": "duration = CUDA events around each step on the launch stream; the "
+                        "contraction kernels are >99% of a step (profiles/)",
+            },
+        }
+        if world == 1 and not args.no_extras:
+            if w.dtype == "bf16":
+                ms, h2d, d2h, _ = e2e_measure(B, b, max(3, args.steps // 2), 3)
+                out["e2e"] = {"value": tokens / (ms * 1e-3), "unit": "scored tokens/s",
+                              "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                              "ms_per_step": ms, "pass": "fwd (gc_token_logprobs_host)"}
+            out["cpu_baseline"] = cpu_baseline(w, 256 if w.D * w.V > 1e8 else 1 << 30)
+            if args.workload == "cfg1":
+                # the metric's second half: fwd+bwd on the 8B-class training micro-batch
+                del b
+                torch.cuda.empty_cache()
+                w2 = I.CONFIGS[2]
+                b2 = DeviceBatch(w2, seed=0, device=torch.device("cuda", local_rank))
+                step2, l2 = make_step(B, b2)
+                tot2, per2 = timed_region(step2, max(3, args.steps // 4), 3, False)
+                ms2 = tot2 / max(3, args.steps // 4)
+                fl2 = 8.0 * b2.n_scored * w2.D * w2.V
+                out["fwd_bwd"] = {"workload": w2.name, "value": b2.n_scored / (ms2 * 1e-3),
+                                  "unit": "scored tokens/s", "ms_per_step": ms2,
+                                  "tflops": fl2 / (ms2 * 1e-3) / 1e12,
+                                  "frac_of_burst": fl2 / (ms2 * 1e-3) / 1e12 / peaks["burst"],
+                                  "gpu_launches_per_step": l2}
+        print(json.dumps(out))
+    if dist_on:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -40,7 +40,10 @@ struct Sched {
   int dyn_dim;            // 0: none; 1: M = clamp(*n_dyn - row0, 0, cap); 2: same for K
   int dyn_round;          // the dynamic extent is rounded up to a multiple of this (>= 1)
   int chunk_ntiles;       // N tiles per item
-  int c_major;            // 1: items ordered (N chunk, M tile); 0: (M tile, N tile), chunk = 1
+  int c_major;            // 1: items ordered (M band, N chunk, M tile in band); 0: (M tile, N tile)
+  int m_band;             // c_major: M tiles per band.  The ~74 items in flight then touch only
+                          // m_band A tiles (kept in L2 across the whole N sweep) and 74/m_band
+                          // N chunks, instead of every A tile of the problem (L2 thrash).
 };
 
 __device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t& K) {
@@ -60,8 +63,23 @@ struct Item { int64_t m_tile, n0, n1, c; };
 __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt, int64_t Nt) {
   Item x;
   if (s.c_major) {
-    x.c = it / Mt;
-    x.m_tile = it - x.c * Mt;
+    const int64_t C = (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles;
+    const int64_t band = s.m_band > 0 ? s.m_band : Mt;
+    const int64_t full_bands = Mt / band;
+    const int64_t items_full = full_bands * C * band;
+    int64_t rem, mb, m0;
+    if (it < items_full) {
+      const int64_t b = it / (C * band);
+      rem = it - b * C * band;
+      mb = band;
+      m0 = b * band;
+    } else {
+      rem = it - items_full;
+      mb = Mt - full_bands * band;
+      m0 = full_bands * band;
+    }
+    x.c = rem / mb;
+    x.m_tile = m0 + (rem - x.c * mb);
     x.n0 = x.c * s.chunk_ntiles;
     x.n1 = x.n0 + s.chunk_ntiles < Nt ? x.n0 + s.chunk_ntiles : Nt;
   } else {

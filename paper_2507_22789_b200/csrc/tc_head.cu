@@ -236,21 +236,8 @@ TcPlan tc_plan_forward(int64_t T, int64_t V) {
   const int64_t kmin = ceil_div(Nt, 160);                // at most 160 partial slots per row
   for (int64_t k = kmin > 1 ? kmin : 1; k <= 64 && k <= Nt; ++k) {
     const int64_t C = ceil_div(Nt, k);
-    const int64_t k_last = Nt - (C - 1) * k;
-    const int64_t items = C * Mt;
-    int64_t worst = 0;
-    for (int p = 0; p < P; ++p) {
-      if (p >= items) break;
-      const int64_t n_p = (items - 1 - p) / P + 1;
-      // items of the last chunk: indices [(C-1)*Mt, C*Mt) congruent to p mod P
-      const int64_t lo = (C - 1) * Mt, hi = C * Mt;
-      int64_t first = lo + ((p - lo % P) % P + P) % P;
-      const int64_t n_last = first < hi ? (hi - 1 - first) / P + 1 : 0;
-      const int64_t load = (n_p - n_last) * k + n_last * k_last;
-      worst = load > worst ? load : worst;
-    }
-    // cost: makespan in tiles, plus a small charge per item flush
-    const double cost = (double)worst * (1.0 + 0.02 / (double)k);
+    // makespan in tiles (upper bound: every item counted as k tiles) + a charge per item flush
+    const double cost = (double)(ceil_div(C * Mt, P) * k) * (1.0 + 0.02 / (double)k);
     if (cost <= best_cost) {
       best_cost = cost;
       best.chunk_vtiles = (int)k;
@@ -259,6 +246,13 @@ TcPlan tc_plan_forward(int64_t T, int64_t V) {
   }
   best.n_vtiles = (int)Nt;
   return best;
+}
+
+// M tiles per band of the forward / recompute schedule: the band's A tiles (m_band x 256 rows x D
+// bf16) should sit comfortably in L2 (<= 32 MB of the 126 MB) while the N sweep streams W past.
+static int pick_m_band(int64_t D) {
+  int64_t mb = (32ll << 20) / (512 * D);
+  return (int)(mb < 4 ? 4 : (mb > 32 ? 32 : mb));
 }
 
 size_t tc_fwd_partials_bytes(int64_t T, int64_t V) {
@@ -278,7 +272,7 @@ static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   Sched s;
   s.M = M; s.N = N; s.K = K;
   s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
-  s.chunk_ntiles = 1; s.c_major = 0;
+  s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0;
   return s;
 }
 
@@ -293,6 +287,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   Sched s = make_sched(T, V, D);
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
+  s.m_band = pick_m_band(D);
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = 0; s.dyn_cap = T; }
   EpiStats::Params ep;
   ep.targets = targets_c;
@@ -318,6 +313,7 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   const TcPlan pl = tc_plan_forward(rows_cap, V);
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
+  s.m_band = pick_m_band(D);
   if (n_rows_dev) {
     s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; s.dyn_round = 256;
   }

@@ -177,10 +177,6 @@ def timed_region(step, steps, warmup, dist_on, dominant=None):
         torch.cuda.synchronize()
     total_ms = t_all0.elapsed_time(t_all1)
     per = [a.elapsed_time(b) for a, b in ev]
-    if dist_on:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
     return total_ms, per
 
 
@@ -341,15 +337,10 @@ def main():
         sampler.start()
     total_ms, per = timed_region(step, args.steps, args.warmup, dist_on)
     clocks = sampler.stop() if rank == 0 else None
-    ms_per_step = total_ms / args.steps
     tokens = b.n_scored
-    if dist_on:
-        import torch.distributed as dist
-        t = torch.tensor([tokens], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t)
-        tokens_all = float(t.item())
-    else:
-        tokens_all = float(tokens)
+    from paper_2507_22789_b200 import dp
+    total_ms, tokens_all = dp.reduce_step_stats(total_ms, tokens)   # max time, summed tokens
+    ms_per_step = total_ms / args.steps
     value = tokens_all / (ms_per_step * 1e-3)
 
     if rank == 0:

@@ -1,0 +1,171 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot materialise [T,V] here, so (SURVEY.md sec 8(c) "parity protocol"):
+  (iii) rows are independent: logp / entropy / lse and dH are checked on sampled rows (tile
+        boundary rows, sequence ends, masked rows, random rows) that the oracle computes from
+        H[t,:], W and the mask alone;
+  (v)   dW and the loss at full T are checked through properties that hold at any size: every
+        column sum of dW is 0, <dH,H> = <dW,W>, unscored dH rows are 0, and the north_star
+        invariant loss = -sum(mA)/sum(m) when policy = old and beta = 0.
+No oracle input comes from the CUDA path: old/ref are synthesised from inputs.proxy_policy_logp.
+"""
+import gc
+
+import numpy as np
+import psutil
+import pytest
+import torch
+
+import oracle as O
+from paper_2507_22789_b200 import inputs as I
+from bench import DeviceBatch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available()
+    from paper_2507_22789_b200 import binding
+    return binding
+
+
+def sample_rows(T, cu, mask, n_random, seed):
+    r = np.random.default_rng(seed)
+    rows = {0, 1, 127, 128, 129, 255, 256, 257, 511, 512, T - 257, T - 256, T - 129, T - 128, T - 2,
+            T - 1}
+    for c in cu[1:-1][:6]:
+        rows.update({int(c) - 1, int(c)})
+    rows.update(int(x) for x in r.integers(0, T, n_random))
+    un = np.nonzero(mask == 0)[0]
+    if len(un):
+        rows.update(int(x) for x in r.choice(un, min(8, len(un)), replace=False))
+    return np.array(sorted(x for x in rows if 0 <= x < T), dtype=np.int64)
+
+
+def check_full(B, b, n_random=64, seed=0):
+    w = b.w
+    need = w.V * w.D * 8 * 2.5
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"host RAM too small for the fp64 widening of W ({need / 1e9:.0f} GB)")
+    lay = b.lay
+    T = b.T
+    adv, keep = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, False)
+    adv_ref, _ = O.grpo_advantages(b.rewards.cpu().numpy(), lay.group_offsets, 1e-6)
+    assert np.allclose(adv.cpu().numpy(), adv_ref.astype(np.float32), rtol=3e-7, atol=1e-9)
+
+    if w.backward:
+        f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
+                               w.clip_hi, w.beta)
+        dH, dW = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref,
+                                    f["logp"], f["lse"], w.clip_lo, w.clip_hi, w.beta,
+                                    dH=b.dH, dW=b.dW)
+        logp, ent, lse = f["logp"], f["entropy"], f["lse"]
+    else:
+        logp, ent, lse = B.gc_token_logprobs(b.H, b.W, b.y, b.mask, w.tau)
+    torch.cuda.synchronize()
+
+    S = sample_rows(T, lay.cu_seqlens, lay.mask, n_random, seed)
+    St = torch.from_numpy(S).cuda()
+    H64 = b.H[St].float().cpu().numpy().astype(np.float64)
+    W64 = b.W.float().cpu().numpy().astype(np.float64)
+    yS = b.y[St].cpu().numpy()
+    mS = lay.mask[S]
+    lp_o, en_o, ls_o = O.token_logprobs(H64, W64, yS, mS, w.tau)
+    d_lp = np.abs(logp[St].cpu().numpy() - lp_o).max()
+    d_en = np.abs(ent[St].cpu().numpy() - en_o).max()
+    d_ls = np.abs(lse[St].cpu().numpy() - ls_o).max()
+    print(f"{w.name}: {len(S)} sampled rows |dlogp|={d_lp:.2e} |dentropy|={d_en:.2e} |dlse|={d_ls:.2e}")
+    assert d_lp <= 1e-4 and d_en <= 2e-4 and d_ls <= 1e-4
+    scored_full = (lay.mask != 0) & (b.y.cpu().numpy() >= 0)
+    zero_rows = torch.from_numpy(np.nonzero(~scored_full)[0]).cuda()
+    assert float(logp[zero_rows].abs().sum()) == 0.0 and float(lse[zero_rows].abs().sum()) == 0.0
+    if not w.backward:
+        return
+
+    # g_t at the sampled rows from the oracle's own logp (token-mean: depends on row t and sum m)
+    old = b.old.cpu().numpy()
+    ref = b.ref.cpu().numpy()
+    logp_full = old.astype(np.float64).copy()
+    logp_full[S] = lp_o
+    g_full = O.grpo_loss_grad_logp(logp_full, old, ref, scored_full, adv_ref, lay.cu_seqlens,
+                                   w.clip_lo, w.clip_hi, w.beta)
+    dH_o, _ = O.lm_head_backward(H64, W64, yS, mS, w.tau, g_full[S])
+    dH_g = dH[St].float().cpu().numpy()
+    sc = (mS != 0) & (yS >= 0)
+    rel = np.linalg.norm(dH_g[sc] - dH_o[sc]) / np.linalg.norm(dH_o[sc])
+    print(f"{w.name}: relF(dH sampled rows)={rel:.2e}")
+    assert rel <= 5e-3
+    assert np.all(dH_g[~sc] == 0.0)
+    del W64
+    gc.collect()
+    # properties at full size
+    assert float(dH[zero_rows].float().abs().sum()) == 0.0
+    colsum = dW.sum(dim=0, dtype=torch.float64).abs().max().item()
+    dw_scale = dW.abs().sum(dim=0, dtype=torch.float64).max().item()
+    assert colsum <= 2e-3 * dw_scale, (colsum, dw_scale)         # bf16 dS rounding does not cancel exactly
+    e1 = (dH.double() * b.H.double()).sum().item()
+    e2 = sum((dW[a:a + 16384].double() * b.W[a:a + 16384].double()).sum().item()
+             for a in range(0, w.V, 16384))
+    print(f"{w.name}: <dH,H>={e1:.6e} <dW,W>={e2:.6e} colsum={colsum:.2e}/{dw_scale:.2e}")
+    assert abs(e1 - e2) <= 2e-2 * max(abs(e1), abs(e2), 1e-4)
+    # north_star invariant at full size: policy = old, beta = 0 -> loss = -sum(m A)/sum(m)
+    out5, _ = B.gc_grpo_token_loss(logp, logp, None, b.y, b.mask, b.cu, adv, beta=0.0,
+                                   want_grad=False)
+    A_tok = adv_ref[O.token_to_response(lay.cu_seqlens, T)]
+    expect = -(A_tok * scored_full).sum() / max(scored_full.sum(), 1)
+    assert abs(out5[0].item() - expect) <= 1e-6 + 1e-5 * abs(expect)
+    assert out5[4].item() == scored_full.sum()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4])
+def test_full_size_config(B, cfg):
+    b = DeviceBatch(I.CONFIGS[cfg], seed=0, device=torch.device("cuda", 0))
+    try:
+        check_full(B, b)
+    finally:
+        del b
+        gc.collect()
+        torch.cuda.empty_cache()
+
+
+def test_full_size_config3_dynamic_sampling(B):
+    """cfg3: lognormal varlen batch; constant groups dropped before the advantage step, kept
+    groups repacked; the mask-instead-of-repack route gives the same loss."""
+    w = I.CONFIGS[3]
+    dev = torch.device("cuda", 0)
+    full = DeviceBatch(w, seed=0, device=dev)
+    assert full.T == 281898                                      # DESIGN.md sec 4 / SURVEY appendix A
+    adv_all, keep = B.gc_grpo_advantages(full.rewards, full.go, 1e-6, False, True)
+    keep_np = keep.cpu().numpy()
+    assert np.array_equal(keep_np, O.group_filter(full.rewards.cpu().numpy(), full.lay.group_offsets))
+    assert keep_np.sum() == 12
+    resp_idx, tok_idx, lay2 = I.drop_groups(full.lay, keep_np, w.group_size)
+    ti = torch.from_numpy(tok_idx).to(dev)
+    # route A: repack the kept groups
+    kept = DeviceBatch.__new__(DeviceBatch)
+    kept.w, kept.lay, kept.T = w, lay2, lay2.T
+    kept.H, kept.W, kept.y = full.H[ti].contiguous(), full.W, full.y[ti].contiguous()
+    kept.mask = None
+    kept.rewards = full.rewards[torch.from_numpy(resp_idx).to(dev)].contiguous()
+    kept.go = torch.from_numpy(lay2.group_offsets).to(dev)
+    kept.cu = torch.from_numpy(lay2.cu_seqlens).to(dev)
+    kept.old, kept.ref = full.old[ti].contiguous(), full.ref[ti].contiguous()
+    kept.dH = torch.empty(lay2.T, w.D, dtype=torch.bfloat16, device=dev)
+    kept.dW = torch.empty(w.V, w.D, dtype=torch.float32, device=dev)
+    # route B first (cheap): same loss with the dropped groups masked instead of removed
+    mask_np = np.zeros(full.T, np.uint8)
+    mask_np[tok_idx] = 1
+    fB = B.gc_grpo_loss_fwd(full.H, full.W, full.y, torch.from_numpy(mask_np).to(dev), w.tau,
+                            full.cu, adv_all, full.old, full.ref, w.clip_lo, w.clip_hi, w.beta)
+    lossB = fB["out5"].cpu().numpy()
+    del full.dH, full.dW
+    check_full(B, kept, n_random=48)
+    advA, _ = B.gc_grpo_advantages(kept.rewards, kept.go, 1e-6, False, False)
+    fA = B.gc_grpo_loss_fwd(kept.H, kept.W, kept.y, None, w.tau, kept.cu, advA, kept.old, kept.ref,
+                            w.clip_lo, w.clip_hi, w.beta)
+    lossA = fA["out5"].cpu().numpy()
+    assert lossA[4] == lossB[4] == lay2.T
+    assert np.allclose(lossA[:4], lossB[:4], rtol=1e-5, atol=1e-7)
+    # a row's result does not depend on the packing (only the split-V combine order differs)
+    assert float((fA["logp"] - fB["logp"][ti]).abs().max()) <= 2e-5

@@ -153,8 +153,10 @@ def _bwd_chunk(B, b):
     return 256 + (a - c256) // (ld * 2)
 
 
-def timed_region(step, steps, warmup, dist_on, dominant=None):
-    """warmup untimed steps, then exactly `steps` steps between barriers; per-step CUDA events."""
+def timed_region(step, steps, warmup, dist_on, B=None):
+    """warmup untimed steps, then exactly `steps` steps between barriers; per-step CUDA events.
+    With B given, the library also brackets each contraction launch with CUDA events on the
+    launch stream (gc_kernel_timing_*): -> (total_ms, per_step_ms, {kind: (ms, launches)})."""
     import torch.distributed as dist
     for _ in range(warmup):
         step()
@@ -162,6 +164,8 @@ def timed_region(step, steps, warmup, dist_on, dominant=None):
     if dist_on:
         dist.barrier()
         torch.cuda.synchronize()
+    if B is not None:
+        B.gc_kernel_timing_begin()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(steps)]
     t_all0, t_all1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -177,7 +181,8 @@ def timed_region(step, steps, warmup, dist_on, dominant=None):
         torch.cuda.synchronize()
     total_ms = t_all0.elapsed_time(t_all1)
     per = [a.elapsed_time(b) for a, b in ev]
-    return total_ms, per
+    kinds = B.gc_kernel_timing_end() if B is not None else None
+    return total_ms, per, kinds
 
 
 def cpu_baseline(w: I.Workload, budget_tokens: int, seed=0, min_seconds=10.0):
@@ -276,6 +281,54 @@ def workload_config(w, T, n_gpus):
             "l2": "inputs exceed L2 (W alone is larger than 126 MB); no flush needed"}
 
 
+def load_traffic(workload, kind):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the named kernel kind, from the
+    committed `ncu --set full` capture (profiles/roofline_traffic.csv; profiles/*.md say how)."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 3 and f[0] == workload and f[1] == kind:
+            return float(f[2])
+    return None
+
+
+def roofline(w, tokens, steps, kinds, step_ms, long_run, peaks):
+    """Roofline of the dominant kernel: algorithmic flops per launch / its average launch duration,
+    measured with CUDA events on the launch stream inside the timed region (gc_kernel_timing_*)."""
+    peak = peaks["sustained"] if long_run else peaks["burst"]
+    pass_flops = 2.0 * tokens * w.D * w.V              # one contraction pass over the scored rows
+    per_kind = {}
+    for k, (ms, n) in (kinds or {}).items():
+        if n:
+            per_kind[k] = {"ms_per_step": ms / steps, "launches_per_step": n / steps,
+                           "tflops": pass_flops * steps / (ms * 1e-3) / 1e12}
+    if not per_kind:                                   # fp32 SIMT workload (cfg0): no contraction
+        return {"bound": "tensor", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None,
+                "traffic": None, "note": "fp32 SIMT parity workload: latency bound, no roofline"}
+    dom = max(per_kind, key=lambda k: per_kind[k]["ms_per_step"])
+    d = per_kind[dom]
+    launch_ms = d["ms_per_step"] / d["launches_per_step"]
+    flops_per_launch = pass_flops / d["launches_per_step"]
+    achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
+    kernel_share = sum(v["ms_per_step"] for v in per_kind.values()) / step_ms
+    return {
+        "bound": "tensor", "kernel": f"tc::k_tc_gemm [{dom}] (tcgen05 contraction + fused epilogue)",
+        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "peak_kind": ("sustained" if long_run else "burst") + " cuBLAS bf16, " + peaks["source"],
+        "frac_of_burst": achieved / peaks["burst"],
+        "frac_of_sustained": achieved / peaks["sustained"],
+        "frac_of_nominal_2250": achieved / 2250.0,
+        "flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
+        "traffic": load_traffic(w.name, dom),
+        "kernels": per_kind, "contraction_share_of_step": kernel_share,
+        "step_tflops": pass_flops * (4 if w.backward else 1) / (step_ms * 1e-3) / 1e12,
+        "note": "launch duration = CUDA events recorded by the library around each contraction "
+                "launch on the launch stream, inside the timed region",
+    }
+
+
 def e2e_measure(B, b: DeviceBatch, steps, warmup):
     """Same metric through the C-ABI call with HOST buffers: per step H2D of H / targets / mask
     from pinned memory, the kernels, D2H of logp + entropy, all inside the timed region."""
@@ -335,7 +388,7 @@ def main():
     sampler = ClockSampler(list(range(world)) if rank == 0 else [])
     if rank == 0:
         sampler.start()
-    total_ms, per = timed_region(step, args.steps, args.warmup, dist_on)
+    total_ms, per, kinds = timed_region(step, args.steps, args.warmup, dist_on, B)
     clocks = sampler.stop() if rank == 0 else None
     tokens = b.n_scored
     from paper_2507_22789_b200 import dp
@@ -347,13 +400,8 @@ def main():
         passes = 4 if w.backward else 1
         flops = 2.0 * tokens * w.D * w.V * passes          # algorithmic: scored rows only
         step_ms = float(np.mean(per))
-        achieved = flops / (step_ms * 1e-3) / 1e12
         long_run = total_ms > 1000.0
-        peak = peaks["sustained"] if long_run else peaks["burst"]
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-        if os.path.exists(tp):
-            traffic = json.load(open(tp)).get(w.name)
+        roof = roofline(w, tokens, args.steps, kinds, step_ms, long_run, peaks)
         out = {
             "metric": metric_name(w), "value": value, "unit": "scored tokens/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -361,17 +409,7 @@ def main():
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32",
             "data": "synthetic", "config": workload_config(w, b.T, world),
             "clocks": clocks, "gpu_launches": launches * args.steps,
-            "roofline": {
-                "bound": "tensor", "kernel": "k_tc_gemm (tcgen05 LM-head contraction + fused epilogue)",
-                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "peak_kind": ("sustained" if long_run else "burst") + " cuBLAS bf16, " + peaks["source"],
-                "frac_of_burst": achieved / peaks["burst"],
-                "frac_of_sustained": achieved / peaks["sustained"],
-                "frac_of_nominal_2250": achieved / 2250.0,
-                "flops_per_step": flops, "kernel_ms": step_ms, "traffic": traffic,
-                "note": "duration = CUDA events around each step on the launch stream; the "
-                        "contraction kernels are >99% of a step (profiles/)",
-            },
+            "roofline": roof,
         }
         if world == 1 and not args.no_extras:
             if w.dtype == "bf16":
@@ -387,10 +425,13 @@ def main():
                 w2 = I.CONFIGS[2]
                 b2 = DeviceBatch(w2, seed=0, device=torch.device("cuda", local_rank))
                 step2, l2 = make_step(B, b2)
-                tot2, per2 = timed_region(step2, max(3, args.steps // 4), 3, False)
+                tot2, per2, kinds2 = timed_region(step2, max(3, args.steps // 4), 3, False, B)
                 ms2 = tot2 / max(3, args.steps // 4)
                 fl2 = 8.0 * b2.n_scored * w2.D * w2.V
+                k2 = {k: {"ms_per_step": ms / max(3, args.steps // 4)}
+                      for k, (ms, n) in kinds2.items() if n}
                 out["fwd_bwd"] = {"workload": w2.name, "value": b2.n_scored / (ms2 * 1e-3),
+                                  "kernels": k2,
                                   "unit": "scored tokens/s", "ms_per_step": ms2,
                                   "tflops": fl2 / (ms2 * 1e-3) / 1e12,
                                   "frac_of_burst": fl2 / (ms2 * 1e-3) / 1e12 / peaks["burst"],

@@ -18,7 +18,8 @@
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and
  *     return without synchronising.  Inputs must stay alive until the stream has passed the call.
  *   - Return value is a gc_status.  Host-checkable errors are reported before any launch.  No
- *     exceptions, no abort(), no global mutable state, no environment variables.
+ *     exceptions, no abort(), no environment variables, no global mutable state (one exception:
+ *     the measurement aid gc_kernel_timing_*, off by default).
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V
@@ -173,6 +174,22 @@ int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* re
                        float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
                        float* out5, float* g,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Measurement aid (bench.py's roofline figure): between _begin and _end the library brackets
+ * every tcgen05 contraction launch with a pair of CUDA events recorded on the call's stream.
+ * _end waits for the recorded events, then writes per kernel kind the summed duration in ms and
+ * the number of launches into two HOST arrays of GC_KERNEL_KINDS entries, and switches the
+ * facility off.  This is the one piece of process-global state in the library (mutex-guarded);
+ * it never changes results.  Kinds: the four dense contractions of SURVEY.md sec 8(a). */
+typedef enum {
+  GC_KERNEL_FWD_STATS = 0,   /* a2+a3: H W^T with the online log-softmax epilogue */
+  GC_KERNEL_RECOMPUTE_DS = 1,/* a10:  H W^T again with the dS epilogue            */
+  GC_KERNEL_DH = 2,          /* a11:  dS W                                        */
+  GC_KERNEL_DW = 3,          /* a12:  dS^T H                                      */
+  GC_KERNEL_KINDS = 4
+} gc_kernel_kind;
+int gc_kernel_timing_begin(void);
+int gc_kernel_timing_end(float* ms_by_kind_host, int32_t* launches_by_kind_host);
 
 /* Plain bf16 GEMM on the library's tcgen05 main loop, for unit tests of the tile engine:
  * C[M,N] (f32, ldc) = A . B with A given as [M,K] (a_mn_major = 0, lda >= K) or [K,M]

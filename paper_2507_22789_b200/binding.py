@@ -23,7 +23,7 @@ EXPORTS = [
     "gc_status_string", "gc_version", "gc_workspace_bytes", "gc_token_logprobs",
     "gc_host_staging_bytes", "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
     "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
-    "gc_debug_gemm_bf16",
+    "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
 ]
 
 
@@ -60,6 +60,8 @@ def _load() -> C.CDLL:
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
                                        f32, vp, vp, vp, sz, vp]
     lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, vp]
+    lib.gc_kernel_timing_begin.argtypes = []
+    lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes"):
@@ -279,3 +281,19 @@ def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, acc
                                    int(b_mn_major), _ptr(C_out), C_out.stride(0), M, N, K,
                                    int(accumulate), int(cta_group), _stream()))
     return C_out
+
+
+KERNEL_KINDS = ("fwd_stats", "recompute_ds", "dh", "dw")
+
+
+def gc_kernel_timing_begin():
+    """Start bracketing every tcgen05 contraction launch with CUDA events on its stream."""
+    _check(_lib.gc_kernel_timing_begin())
+
+
+def gc_kernel_timing_end() -> dict:
+    """Waits for the recorded events; -> {kind: (total_ms, launches)} for the four contractions."""
+    ms = (C.c_float * len(KERNEL_KINDS))()
+    n = (C.c_int32 * len(KERNEL_KINDS))()
+    _check(_lib.gc_kernel_timing_end(ms, n))
+    return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}

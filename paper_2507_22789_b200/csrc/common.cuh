@@ -45,6 +45,16 @@ struct Carver {
 // (-inf if the target is not in this chunk).
 struct __align__(16) RowStat { float m, s, u, ay; };
 
+// timing.cu: RAII bracket around one contraction launch (no-op unless gc_kernel_timing_begin ran)
+class KernelTimer {
+ public:
+  KernelTimer(int kind, cudaStream_t st);
+  ~KernelTimer();
+ private:
+  cudaStream_t st_;
+  long idx_;
+};
+
 // ---- launchers implemented in the .cu files (all enqueue on `st`, no sync) ----------------
 // small_kernels.cu
 int launch_advantages(const float* rewards, const int32_t* group_offsets, int32_t G, float eps,

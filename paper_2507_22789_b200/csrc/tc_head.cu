@@ -295,6 +295,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   ep.split_stride = ceil_div(T, 256) * 256;
   ep.V = V;
   ep.c = kLog2e / tau;
+  KernelTimer kt(GC_KERNEL_FWD_STATS, st);
   return launch_cg<EpiStats, false, false>(cg, ta, tb, s, ep, st);
 }
 
@@ -330,6 +331,7 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   ep.V = V;
   ep.c = kLog2e / tau;
   ep.inv_tau = 1.0f / tau;
+  KernelTimer kt(GC_KERNEL_RECOMPUTE_DS, st);
   return launch_cg<EpiDS, false, false>(cg, ta, tb, s, ep, st);
 }
 
@@ -348,6 +350,7 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.rows = rows;
   ep.row_base = row0;
   ep.N = D;
+  KernelTimer kt(GC_KERNEL_DH, st);
   return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st);
 }
 
@@ -366,6 +369,7 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.ldo = lddW;
   ep.N = D;
   ep.accumulate = accumulate;
+  KernelTimer kt(GC_KERNEL_DW, st);
   return launch_cg<EpiStoreF32, true, true>(cg, ta, tb, s, ep, st);
 }
 

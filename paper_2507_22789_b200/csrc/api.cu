@@ -65,24 +65,25 @@ int64_t ld_ds(int64_t V) { return ceil_div(V, 64) * 64; }
 
 // Workspace layouts (mirrored by gc_workspace_bytes).
 struct FwdWs {
-  RowStat* partials; int32_t* rows; int32_t* n_rows; int32_t* targets_c; void* Hs; void* compact;
+  uint32_t* counters; RowStat* partials; int32_t* rows; int32_t* n_rows; int32_t* targets_c; void* Hs; void* compact;
 };
 size_t carve_fwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, FwdWs* w) {
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   if (dtype == GC_BF16) {
+    uint32_t* ctr = c.take<uint32_t>(kTcCounters);
     RowStat* p = c.take<RowStat>(tc_fwd_partials_bytes(T, V) / sizeof(RowStat));
     int32_t* rows = c.take<int32_t>((size_t)cap);
     int32_t* n_rows = c.take<int32_t>(64);
     int32_t* tc_ = c.take<int32_t>((size_t)cap);
     void* Hs = c.take<uint8_t>((size_t)cap * (size_t)D * 2);
     void* cw = c.take<uint8_t>(compact_ws_bytes(T));
-    if (w) { w->partials = p; w->rows = rows; w->n_rows = n_rows; w->targets_c = tc_; w->Hs = Hs; w->compact = cw; }
+    if (w) { w->counters = ctr; w->partials = p; w->rows = rows; w->n_rows = n_rows; w->targets_c = tc_; w->Hs = Hs; w->compact = cw; }
   }
   return c.off;
 }
 
 struct BwdWs {
-  void* loss; float* out5; float* g; int32_t* rows; int32_t* n_rows; int32_t* targets_c;
+  uint32_t* counters; void* loss; float* out5; float* g; int32_t* rows; int32_t* n_rows; int32_t* targets_c;
   float* lse_c; float* g_c; void* Hs; void* compact; void* dS;
 };
 size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk, int32_t R,
@@ -93,6 +94,8 @@ size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t 
   float* g = c.take<float>((size_t)cap);
   if (w) { w->loss = loss; w->out5 = out5; w->g = g; }
   if (dtype == GC_BF16) {
+    uint32_t* ctr = c.take<uint32_t>(kTcCounters);
+    if (w) w->counters = ctr;
     int32_t* rows = c.take<int32_t>((size_t)cap);
     int32_t* n_rows = c.take<int32_t>(64);
     int32_t* tcx = c.take<int32_t>((size_t)cap);
@@ -174,9 +177,10 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
   carve_fwd(c, T, D, V, dtype, &w);
   const TcPlan pl = tc_plan_forward(T, V);
   const int64_t cap = ceil_div(T, 256) * 256;
+  GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
   if (!mask) {
     // dense mode: every row goes through the contraction; rows with target < 0 come out as 0
-    GC_TRY(tc_forward_stats(H, ldH, W, ldW, T, D, V, temperature, targets, nullptr, w.partials, st));
+    GC_TRY(tc_forward_stats(H, ldH, W, ldW, T, D, V, temperature, targets, nullptr, w.partials, w.counters, st));
     return launch_combine(w.partials, pl.n_split, cap, nullptr, nullptr, T, logp, entropy, lse, st);
   }
   // compaction mode (a1): only scored rows reach the tensor cores
@@ -184,7 +188,8 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
   GC_TRY(launch_gather_rows(H, ldH, 2, D, T, w.rows, w.n_rows, w.Hs, cap, st));
   GC_TRY(launch_gather_i32(targets, w.rows, w.n_rows, T, w.targets_c, st));
   GC_TRY(launch_zero_unscored(targets, mask, T, logp, entropy, lse, st));
-  GC_TRY(tc_forward_stats(w.Hs, D, W, ldW, T, D, V, temperature, w.targets_c, w.n_rows, w.partials, st));
+  GC_TRY(tc_forward_stats(w.Hs, D, W, ldW, T, D, V, temperature, w.targets_c, w.n_rows, w.partials,
+                          w.counters, st));
   return launch_combine(w.partials, pl.n_split, cap, w.rows, w.n_rows, T, logp, entropy, lse, st);
 }
 
@@ -352,19 +357,28 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
     Hs = w.Hs; ldHs = D; targets_c = w.targets_c; lse_c = w.lse_c; g_c = w.g_c;
     rows = w.rows; n_rows = w.n_rows;
   }
+  GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
+  int ci = 0;
   for (int64_t row0 = 0; row0 < T; row0 += chunk) {
+    if (ci + 3 > kTcCounters) {
+      GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
+      ci = 0;
+    }
     const int64_t n_static = compact ? 0 : ((T - row0 < chunk) ? T - row0 : chunk);
     const int64_t rows_cap = compact ? ((cap - row0 < chunk) ? cap - row0 : chunk) : chunk;
     const char* Hc = static_cast<const char*>(Hs) + (size_t)row0 * (size_t)ldHs * 2;
     // a10: recompute the logit chunk, dS = (g/tau)(onehot - p) in bf16
     GC_TRY(tc_recompute_ds(Hc, ldHs, W, ldW, rows_cap, n_static, D, V, temperature,
-                           targets_c + row0, lse_c + row0, g_c + row0, n_rows, row0, w.dS, ldS, st));
+                           targets_c + row0, lse_c + row0, g_c + row0, n_rows, row0, w.dS, ldS,
+                           w.counters + ci, st));
     // a11: dH rows of this chunk
     GC_TRY(tc_dh(w.dS, ldS, rows_cap, n_static, W, ldW, D, V, rows ? rows + row0 : nullptr, n_rows,
-                 row0, dH, lddH, st));
+                 row0, dH, lddH, w.counters + ci + 1, st));
     // a12: dW accumulates over chunks in fp32
     GC_TRY(tc_dw(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
-                 static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0, st));
+                 static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0,
+                 w.counters + ci + 2, st));
+    ci += 3;
   }
   return GC_OK;
 }
@@ -408,12 +422,12 @@ int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* target
 
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
                        int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
-                       int accumulate, int cta_group, void* cuda_stream) {
+                       int accumulate, int cta_group, int dynamic_schedule, void* cuda_stream) {
   if (!A || !B || !C) return GC_ERR_NULL;
   if (M <= 0 || N <= 0 || K <= 0) return GC_ERR_SHAPE;
   GC_TRY(check_arch());
   return tc_debug_gemm(A, lda, a_mn_major, B, ldb, b_mn_major, C, ldc, M, N, K, accumulate,
-                       cta_group, static_cast<cudaStream_t>(cuda_stream));
+                       cta_group, dynamic_schedule, static_cast<cudaStream_t>(cuda_stream));
 }
 
 }  // extern "C"

@@ -94,7 +94,9 @@ int simt_backward(const void* H, int64_t ldH, const void* W, int64_t ldW, bool b
                   float tau, const float* lse, const float* g, void* dH, int64_t lddH,
                   float* dW, int64_t lddW, int accumulate, cudaStream_t st);
 
-// tc_head.cu (tcgen05 engine)
+// tc_head.cu (tcgen05 engine).  `counter`: a zeroed device word per launch (dynamic item
+// schedule, tc_gemm.cuh); the API zeroes kTcCounters of them once per call.
+constexpr int kTcCounters = 1024;
 struct TcPlan {            // forward / recompute schedule: items = (vocab chunk c, M tile)
   int n_vtiles;            // ceil(V / 256)
   int chunk_vtiles;        // vocab tiles per item
@@ -104,21 +106,22 @@ TcPlan tc_plan_forward(int64_t T, int64_t V);
 size_t tc_fwd_partials_bytes(int64_t T, int64_t V);
 int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
                      int64_t D, int64_t V, float tau, const int32_t* targets_c,
-                     const int32_t* n_rows_dev, RowStat* partials, cudaStream_t st);
+                     const int32_t* n_rows_dev, RowStat* partials, uint32_t* counter,
+                     cudaStream_t st);
 // Backward chunk kernels.  rows_cap = rows of the dS chunk buffer (multiple of 256); the valid
 // rows of the chunk are clamp(*n_rows_dev - row0, 0, rows_cap), or n_static if n_rows_dev == NULL.
 int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,
                     int64_t n_static, int64_t D, int64_t V, float tau, const int32_t* targets_c,
                     const float* lse_c, const float* g_c, const int32_t* n_rows_dev,
-                    int64_t row0, void* dS, int64_t ldS, cudaStream_t st);
+                    int64_t row0, void* dS, int64_t ldS, uint32_t* counter, cudaStream_t st);
 int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* W,
           int64_t ldW, int64_t D, int64_t V, const int32_t* rows, const int32_t* n_rows_dev,
-          int64_t row0, void* dH, int64_t lddH, cudaStream_t st);
+          int64_t row0, void* dH, int64_t lddH, uint32_t* counter, cudaStream_t st);
 int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
           int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
-          int64_t lddW, int accumulate, cudaStream_t st);
+          int64_t lddW, int accumulate, uint32_t* counter, cudaStream_t st);
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, cudaStream_t st);
+                  int cta_group, int dynamic_schedule, cudaStream_t st);
 
 }  // namespace gc

@@ -31,7 +31,11 @@ template <int CG> struct Cfg {
   static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
 };
 
-// Work schedule.  An item is (M tile, run of N tiles); CTA pair p takes items p, p+P, ...
+// Work schedule.  An item is (M tile, run of N tiles).  Items are handed out in index order to
+// whichever CTA pair is free (one atomicAdd per item by the leader CTA's producer lane, published
+// to the other roles and the peer CTA through a 4-slot smem ring): per-item time jitter (~4 %,
+// measured) otherwise accumulates as a random walk, pairs that share a tile drift rounds apart and
+// re-fetch it from DRAM.  With a NULL counter pair p takes items p, p+P, ... (static).
 struct Sched {
   int64_t M, N, K;        // static extents of the problem
   const int32_t* n_dyn;   // device scalar: dynamic row count of the whole batch (nullable)
@@ -39,11 +43,18 @@ struct Sched {
   int64_t dyn_cap;        // chunk capacity in rows
   int dyn_dim;            // 0: none; 1: M = clamp(*n_dyn - row0, 0, cap); 2: same for K
   int dyn_round;          // the dynamic extent is rounded up to a multiple of this (>= 1)
+  uint32_t* counter;      // device word, 0 at launch: items are claimed with atomicAdd in the order
+                          // pairs become free (dynamic).  NULL: pair p takes items p, p+P, ... (static)
+  int a_hint, b_hint;     // L2 eviction priority of the A / B tile loads (ptx::kL2*)
   int chunk_ntiles;       // N tiles per item
   int c_major;            // 1: items ordered (M band, N chunk, M tile in band); 0: (M tile, N tile)
   int m_band;             // c_major: M tiles per band.  The ~74 items in flight then touch only
                           // m_band A tiles (kept in L2 across the whole N sweep) and 74/m_band
                           // N chunks, instead of every A tile of the problem (L2 thrash).
+  int n_band;             // c_major == 0 and n_band > 0: items ordered (N band, M tile, N tile in
+                          // band): the band's B panels stay in L2 while the A panels stream past
+  int skip_empty_k;       // 1: a launch whose K extent resolves to 0 does nothing (accumulating
+                          // epilogues: adding zero)
 };
 
 __device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t& K) {
@@ -82,6 +93,16 @@ __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt,
     x.m_tile = m0 + (rem - x.c * mb);
     x.n0 = x.c * s.chunk_ntiles;
     x.n1 = x.n0 + s.chunk_ntiles < Nt ? x.n0 + s.chunk_ntiles : Nt;
+  } else if (s.n_band > 0 && s.n_band < Nt) {
+    const int64_t per_band = Mt * s.n_band;
+    const int64_t b = it / per_band;
+    const int64_t n_start = b * s.n_band;
+    const int64_t w = Nt - n_start < s.n_band ? Nt - n_start : s.n_band;   // last band: narrower
+    const int64_t rem = it - b * per_band;
+    x.m_tile = rem / w;
+    x.n0 = n_start + (rem - x.m_tile * w);
+    x.n1 = x.n0 + 1;
+    x.c = 0;
   } else {
     x.m_tile = it / Nt;
     x.n0 = it - x.m_tile * Nt;
@@ -105,6 +126,12 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   auto tfull_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + i); };
   auto tempty_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + 2 + i); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
+  // item ring (dynamic schedule): sfull[4] @136, sempty[4] @168 (leader CTA's are used), item[4] @200
+  constexpr int kSlots = 4;
+  auto sfull_bar = [&](int i) { return bar_base + 136u + 8u * i; };
+  auto sempty_bar = [&](int i) { return bar_base + 168u + 8u * i; };
+  auto sitem = [&](int i) { return bar_base + 200u + 4u * i; };
+  static_assert(8 * (2 * C::kStages + 4) + 4 <= 136, "barrier area overlap");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = CG == 2 ? ptx::cluster_ctarank() : 0u;
@@ -123,6 +150,12 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       ptx::mbar_init(tfull_bar(i), 1);
       ptx::mbar_init(tempty_bar(i), 4 * CG);
     }
+    for (int i = 0; i < kSlots; ++i) {
+      ptx::mbar_init(sfull_bar(i), 1);
+      // consumers of a slot: MMA lane + 4 epilogue warps (leader), producer lane + 4 epilogue
+      // warps (peer)
+      ptx::mbar_init(sempty_bar(i), 5 * CG);
+    }
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -140,15 +173,58 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const int64_t Mt = (M_eff + BM_CTA * CG - 1) / (BM_CTA * CG);
   const int64_t Nt = (s.N + BN - 1) / BN;
   const int64_t n_chunks = s.c_major ? (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles : Nt;
-  const int64_t n_items = Mt * n_chunks;
   const int num_kb = (int)((K_eff + BK - 1) / BK);
+  const int64_t n_items = (s.skip_empty_k && num_kb == 0) ? 0 : Mt * n_chunks;
+
+  // ---- item stream -------------------------------------------------------------------------
+  const bool dynamic = s.counter != nullptr;
+  struct Cursor { int64_t next; int slot; uint32_t phase; };
+  Cursor cur{pair, 0, 0u};
+  // consumer side: next item index of this pair, or -1 when the work is exhausted
+  auto consume = [&](bool warp_wide) -> int64_t {
+    if (!dynamic) {
+      const int64_t it = cur.next;
+      cur.next += n_pairs;
+      return it < n_items ? it : -1;
+    }
+    ptx::mbar_wait_cluster(sfull_bar(cur.slot), cur.phase);
+    const int32_t v = (int32_t)ptx::ld_shared_u32(sitem(cur.slot));
+    if (warp_wide) __syncwarp();
+    if (!warp_wide || lane == 0) {
+      if (rank == 0) ptx::mbar_arrive(sempty_bar(cur.slot));
+      else ptx::mbar_arrive_cluster(ptx::mapa(sempty_bar(cur.slot), 0));
+    }
+    if (++cur.slot == kSlots) { cur.slot = 0; cur.phase ^= 1u; }
+    return (int64_t)v;
+  };
+  // scheduler side (leader CTA's producer lane): publish a claimed ticket to both CTAs
+  auto publish = [&](uint32_t ticket) -> int64_t {
+    const int32_t v = (int64_t)ticket < n_items ? (int32_t)ticket : -1;
+    ptx::mbar_wait_cluster(sempty_bar(cur.slot), cur.phase ^ 1u);
+    ptx::st_shared_u32(sitem(cur.slot), (uint32_t)v);
+    ptx::mbar_arrive(sfull_bar(cur.slot));
+    if constexpr (CG == 2) {
+      ptx::st_shared_cluster_u32(ptx::mapa(sitem(cur.slot), 1), (uint32_t)v);
+      ptx::mbar_arrive_cluster(ptx::mapa(sfull_bar(cur.slot), 1));
+    }
+    if (++cur.slot == kSlots) { cur.slot = 0; cur.phase ^= 1u; }
+    return (int64_t)v;
+  };
 
   if (warp == 0) {
     // ===================== TMA producer (one lane, every CTA) =====================
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int64_t it = pair; it < n_items; it += n_pairs) {
+      const uint64_t polA = ptx::make_l2_policy(s.a_hint), polB = ptx::make_l2_policy(s.b_hint);
+      const bool scheduler = dynamic && rank == 0;
+      int64_t it = scheduler ? publish(atomicAdd(s.counter, 1u)) : consume(false);
+      while (it >= 0) {
+        // claim the following item now (the atomic's latency hides behind this item's loads),
+        // publish it after the first N tile of this one
+        uint32_t ticket = 0;
+        if (scheduler) ticket = atomicAdd(s.counter, 1u);
+        int64_t it_next = -1;
         const Item item = get_item(s, it, Mt, Nt);
         const int32_t m_coord = (int32_t)(item.m_tile * BM_CTA * CG + rank * BM_CTA);
         for (int64_t n = item.n0; n < item.n1; ++n) {
@@ -161,36 +237,38 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             if constexpr (CG == 1) {
               ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes);
               const uint32_t fb = full_bar(stage);
-              if constexpr (!A_MN) ptx::tma_load_2d(sa, &tmA, k_coord, m_coord, fb);
+              if constexpr (!A_MN) ptx::tma_load_2d(sa, &tmA, k_coord, m_coord, fb, polA);
               else {
-                ptx::tma_load_2d(sa, &tmA, m_coord, k_coord, fb);
-                ptx::tma_load_2d(sa + 8192, &tmA, m_coord + 64, k_coord, fb);
+                ptx::tma_load_2d(sa, &tmA, m_coord, k_coord, fb, polA);
+                ptx::tma_load_2d(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
               }
-              if constexpr (!B_MN) ptx::tma_load_2d(sb, &tmB, k_coord, n_coord, fb);
+              if constexpr (!B_MN) ptx::tma_load_2d(sb, &tmB, k_coord, n_coord, fb, polB);
               else {
 #pragma unroll
                 for (int b = 0; b < C::kBRows / 64; ++b)
-                  ptx::tma_load_2d(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb);
+                  ptx::tma_load_2d(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb, polB);
               }
             } else {
               // the leader's barrier collects the bytes of both CTAs
               if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes * 2);
               const uint32_t fb = ptx::mapa(full_bar(stage), 0);
-              if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb);
+              if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb, polA);
               else {
-                ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb);
-                ptx::tma_load_2d_cg2(sa + 8192, &tmA, m_coord + 64, k_coord, fb);
+                ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb, polA);
+                ptx::tma_load_2d_cg2(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
               }
-              if constexpr (!B_MN) ptx::tma_load_2d_cg2(sb, &tmB, k_coord, n_coord, fb);
+              if constexpr (!B_MN) ptx::tma_load_2d_cg2(sb, &tmB, k_coord, n_coord, fb, polB);
               else {
 #pragma unroll
                 for (int b = 0; b < C::kBRows / 64; ++b)
-                  ptx::tma_load_2d_cg2(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb);
+                  ptx::tma_load_2d_cg2(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb, polB);
               }
             }
             if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
           }
+          if (scheduler && n == item.n0) it_next = publish(ticket);
         }
+        it = scheduler ? it_next : consume(false);
       }
     }
   } else if (warp == 1) {
@@ -203,7 +281,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       uint32_t phase = 0;
       int acc = 0;
       uint32_t acc_phase = 0;
-      for (int64_t it = pair; it < n_items; it += n_pairs) {
+      for (int64_t it = consume(false); it >= 0; it = consume(false)) {
         const Item item = get_item(s, it, Mt, Nt);
         for (int64_t n = item.n0; n < item.n1; ++n) {
           ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
@@ -236,7 +314,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     uint32_t acc_phase = 0;
     typename Epi::State st;
     Epi::setup(st, ep);
-    for (int64_t it = pair; it < n_items; it += n_pairs) {
+    for (int64_t it = consume(true); it >= 0; it = consume(true)) {
       const Item item = get_item(s, it, Mt, Nt);
       const int64_t grow = item.m_tile * BM_CTA * CG + rank * BM_CTA + row_in_tile;
       const bool valid = grow < M_eff;

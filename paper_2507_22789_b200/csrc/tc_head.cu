@@ -5,6 +5,7 @@
 //   a11    dH           dH = dS W             -> bf16 rows scattered to their original positions
 //   a12    dW           dW (+)= dS^T Hs       -> fp32
 #include "tc_gemm.cuh"
+#include <stdio.h>
 
 #ifndef GC_DEFAULT_CG
 #define GC_DEFAULT_CG 2
@@ -248,11 +249,21 @@ TcPlan tc_plan_forward(int64_t T, int64_t V) {
   return best;
 }
 
-// M tiles per band of the forward / recompute schedule: the band's A tiles (m_band x 256 rows x D
-// bf16) should sit comfortably in L2 (<= 32 MB of the 126 MB) while the N sweep streams W past.
+// L2 budget for the operand panels a schedule keeps resident.  Measured (profiles/): bands up to
+// ~48 MB stay resident, 60 MB and more thrash (DRAM reads x2.5 .. x7) -- about half of the 126 MB,
+// consistent with each die's L2 also holding the lines its SMs fetch from the other die.
+constexpr int64_t kL2ResidentBytes = 44ll << 20;
+
+// M tiles per band of the forward / recompute schedule: the band's A panels (m_band x 256 rows x
+// D bf16) stay in L2 while the N sweep streams W past; W is re-read once per band.
 static int pick_m_band(int64_t D) {
-  int64_t mb = (32ll << 20) / (512 * D);
-  return (int)(mb < 4 ? 4 : (mb > 32 ? 32 : mb));
+  int64_t mb = kL2ResidentBytes / (512 * D);
+  return (int)(mb < 4 ? 4 : (mb > 64 ? 64 : mb));
+}
+// N tiles per band of the dW schedule: the band's H panels (k_rows x 256 columns bf16).
+static int pick_n_band(int64_t k_rows) {
+  int64_t nb = kL2ResidentBytes / (512 * (k_rows > 0 ? k_rows : 1));
+  return (int)(nb < 1 ? 1 : nb);
 }
 
 size_t tc_fwd_partials_bytes(int64_t T, int64_t V) {
@@ -260,6 +271,25 @@ size_t tc_fwd_partials_bytes(int64_t T, int64_t V) {
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   return align_up((size_t)pl.n_split * (size_t)cap * sizeof(RowStat), 256);
 }
+
+#ifdef GC_EXP_ENV
+// Tuning builds only (-DGC_EXP_ENV, never the product build): schedule knobs from the environment.
+#include <stdlib.h>
+static void exp_override(Sched& s, const char* kind) {
+  char name[64];
+  auto get = [&](const char* knob, int& dst) {
+    snprintf(name, sizeof name, "GC_%s_%s", kind, knob);
+    if (const char* v = getenv(name)) dst = atoi(v);
+  };
+  int dyn = s.counter != nullptr;
+  get("MBAND", s.m_band); get("AHINT", s.a_hint); get("BHINT", s.b_hint); get("DYN", dyn);
+  get("CHUNK", s.chunk_ntiles); get("NBAND", s.n_band);
+  if (!dyn) s.counter = nullptr;
+}
+#define GC_EXP_OVERRIDE(s, kind) exp_override(s, kind)
+#else
+#define GC_EXP_OVERRIDE(s, kind) ((void)0)
+#endif
 
 template <class Epi, bool A_MN, bool B_MN>
 static int launch_cg(int cg, const CUtensorMap& a, const CUtensorMap& b, const Sched& s,
@@ -272,13 +302,14 @@ static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   Sched s;
   s.M = M; s.N = N; s.K = K;
   s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
-  s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0;
+  s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0; s.n_band = 0; s.skip_empty_k = 0;
+  s.counter = nullptr; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
   return s;
 }
 
 int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T, int64_t D,
                      int64_t V, float tau, const int32_t* targets_c, const int32_t* n_rows_dev,
-                     RowStat* partials, cudaStream_t st) {
+                     RowStat* partials, uint32_t* counter, cudaStream_t st) {
   const int cg = GC_DEFAULT_CG;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
@@ -288,6 +319,9 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
   s.m_band = pick_m_band(D);
+  s.counter = counter;
+  s.a_hint = ptx::kL2EvictLast;     // the band's H tiles are re-read for every vocab tile
+  s.b_hint = ptx::kL2EvictFirst;    // W streams past
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = 0; s.dyn_cap = T; }
   EpiStats::Params ep;
   ep.targets = targets_c;
@@ -295,6 +329,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   ep.split_stride = ceil_div(T, 256) * 256;
   ep.V = V;
   ep.c = kLog2e / tau;
+  GC_EXP_OVERRIDE(s, "FWD");
   KernelTimer kt(GC_KERNEL_FWD_STATS, st);
   return launch_cg<EpiStats, false, false>(cg, ta, tb, s, ep, st);
 }
@@ -302,7 +337,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
 int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,
                     int64_t n_static, int64_t D, int64_t V, float tau, const int32_t* targets_c,
                     const float* lse_c, const float* g_c, const int32_t* n_rows_dev, int64_t row0,
-                    void* dS, int64_t ldS, cudaStream_t st) {
+                    void* dS, int64_t ldS, uint32_t* counter, cudaStream_t st) {
   const int cg = GC_DEFAULT_CG;
   const int64_t h_rows = n_rows_dev ? rows_cap : n_static;   // rows behind the H pointer
   CUtensorMap ta, tb;
@@ -315,6 +350,9 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
   s.m_band = pick_m_band(D);
+  s.counter = counter;
+  s.a_hint = ptx::kL2EvictLast;
+  s.b_hint = ptx::kL2EvictFirst;
   if (n_rows_dev) {
     s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; s.dyn_round = 256;
   }
@@ -331,18 +369,20 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   ep.V = V;
   ep.c = kLog2e / tau;
   ep.inv_tau = 1.0f / tau;
+  GC_EXP_OVERRIDE(s, "DS");
   KernelTimer kt(GC_KERNEL_RECOMPUTE_DS, st);
   return launch_cg<EpiDS, false, false>(cg, ta, tb, s, ep, st);
 }
 
 int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* W,
           int64_t ldW, int64_t D, int64_t V, const int32_t* rows, const int32_t* n_rows_dev,
-          int64_t row0, void* dH, int64_t lddH, cudaStream_t st) {
+          int64_t row0, void* dH, int64_t lddH, uint32_t* counter, cudaStream_t st) {
   const int cg = GC_DEFAULT_CG;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, dS, rows_cap, V, ldS, false, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
   Sched s = make_sched(n_rows_dev ? rows_cap : n_static, D, V);
+  (void)counter;   // K-lockstep kernel: all pairs stream V together, static schedule
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
   EpiStoreBf16::Params ep;
   ep.out = static_cast<__nv_bfloat16*>(dH);
@@ -350,38 +390,56 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.rows = rows;
   ep.row_base = row0;
   ep.N = D;
+  GC_EXP_OVERRIDE(s, "DH");
   KernelTimer kt(GC_KERNEL_DH, st);
   return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st);
 }
 
 int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
           int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
-          int64_t lddW, int accumulate, cudaStream_t st) {
+          int64_t lddW, int accumulate, uint32_t* counter, cudaStream_t st) {
   const int cg = GC_DEFAULT_CG;
   const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
   GC_TRY(tc::make_operand_tmap(&tb, Hs, D, k_rows, ldH, true, 0));
   Sched s = make_sched(V, D, k_rows);
+  // items (D band, vocab tile, D tile in band): the band's H panels stay in L2, the D tiles of a
+  // vocab tile run together and share its dS^T panel, which streams past once per band
+  s.counter = counter;
+  s.a_hint = ptx::kL2EvictFirst;
+  s.b_hint = ptx::kL2EvictLast;
+  s.n_band = pick_n_band(k_rows);
+  s.skip_empty_k = accumulate ? 1 : 0;
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 2; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
   EpiStoreF32::Params ep;
   ep.out = dW;
   ep.ldo = lddW;
   ep.N = D;
   ep.accumulate = accumulate;
+  GC_EXP_OVERRIDE(s, "DW");
   KernelTimer kt(GC_KERNEL_DW, st);
   return launch_cg<EpiStoreF32, true, true>(cg, ta, tb, s, ep, st);
 }
 
+// one counter for the debug GEMM (not safe for concurrent debug calls on different streams)
+__device__ uint32_t g_debug_counter;
+
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, cudaStream_t st) {
+                  int cta_group, int dynamic_schedule, cudaStream_t st) {
   if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
   if (N % 4 != 0) return GC_ERR_SHAPE;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, tc::BN / cta_group));
   Sched s = make_sched(M, N, K);
+  if (dynamic_schedule) {
+    void* ctr = nullptr;
+    GC_CUDA_TRY(cudaGetSymbolAddress(&ctr, g_debug_counter));
+    GC_CUDA_TRY(cudaMemsetAsync(ctr, 0, sizeof(uint32_t), st));
+    s.counter = static_cast<uint32_t*>(ctr);
+  }
   EpiStoreF32::Params ep;
   ep.out = C;
   ep.ldo = ldc;

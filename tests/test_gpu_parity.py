@@ -36,20 +36,37 @@ def dev(x, dtype=None):
 
 
 # ------------------------------------------------------------------ tile engine unit tests
+@pytest.mark.parametrize("dyn", [False, True])
 @pytest.mark.parametrize("cg", [1, 2])
 @pytest.mark.parametrize("a_mn,b_mn", [(0, 0), (0, 1), (1, 0), (1, 1)])
 @pytest.mark.parametrize("M,N,K", [(128, 256, 64), (392, 520, 200), (1000, 776, 1096)])
-def test_engine_gemm(B, cg, a_mn, b_mn, M, N, K):
+def test_engine_gemm(B, dyn, cg, a_mn, b_mn, M, N, K):
     g = torch.Generator(device="cuda").manual_seed(M + N + K)
     A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
     Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
     ref = A.double() @ Bm.double().T
     C = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
-                             a_mn, b_mn, cta_group=cg)
+                             a_mn, b_mn, cta_group=cg, dynamic_schedule=dyn)
     assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
     C2 = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
-                              a_mn, b_mn, C_out=C.clone(), accumulate=True, cta_group=cg)
+                              a_mn, b_mn, C_out=C.clone(), accumulate=True, cta_group=cg,
+                              dynamic_schedule=dyn)
     assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+
+
+@pytest.mark.parametrize("dyn", [False, True])
+def test_engine_gemm_many_tiles(B, dyn):
+    """More tiles than CTA pairs (several items per pair, ragged edges), both schedules; the
+    dynamic one must also be deterministic (the tile -> pair map does not enter the result)."""
+    M, N, K = 256 * 21 + 40, 256 * 9 + 8, 320
+    g = torch.Generator(device="cuda").manual_seed(5)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.float() @ Bm.float().T
+    C1 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn)
+    C2 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn)
+    assert (C1 - ref).abs().max().item() < 1e-3 * K ** 0.5
+    assert torch.equal(C1, C2)
 
 
 # ------------------------------------------------------------------ a6/a7 advantages

@@ -197,11 +197,13 @@ int gc_kernel_timing_end(float* ms_by_kind_host, int32_t* launches_by_kind_host)
  * accumulate != 0 adds to C.  cta_group is 1 or 2.  dynamic_schedule != 0: tiles are claimed
  * by whichever CTA pair is free (the schedule of the forward / recompute / dW kernels; uses one
  * library-owned counter, so do not run two such debug calls concurrently); 0: static round-robin
- * (the schedule of the dH kernel). */
+ * (the schedule of the dH kernel).  dual_n != 0 (cta_group 2 only): 256 x 512 tiles whose two
+ * halves share the A stages (the dH kernel's tile). */
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major,
                        const void* B, int64_t ldb, int b_mn_major,
                        float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
-                       int accumulate, int cta_group, int dynamic_schedule, void* cuda_stream);
+                       int accumulate, int cta_group, int dynamic_schedule, int dual_n,
+                       void* cuda_stream);
 
 #ifdef __cplusplus
 }

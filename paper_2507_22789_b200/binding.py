@@ -60,7 +60,7 @@ def _load() -> C.CDLL:
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
                                        f32, vp, vp, vp, sz, vp]
     lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, ci,
-                                       vp]
+                                       ci, vp]
     lib.gc_kernel_timing_begin.argtypes = []
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
@@ -265,7 +265,7 @@ def gc_validate_targets(targets, mask, V) -> int:
 
 
 def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, accumulate=False,
-                       cta_group=2, dynamic_schedule=True):
+                       cta_group=2, dynamic_schedule=True, dual_n=False):
     """C[M,N] f32 = A.B on the tcgen05 tile engine (unit test of the engine)."""
     if a_mn_major:
         K, M = A.shape
@@ -281,7 +281,7 @@ def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, acc
     _check(_lib.gc_debug_gemm_bf16(_ptr(A), A.stride(0), int(a_mn_major), _ptr(B), B.stride(0),
                                    int(b_mn_major), _ptr(C_out), C_out.stride(0), M, N, K,
                                    int(accumulate), int(cta_group), int(dynamic_schedule),
-                                   _stream()))
+                                   int(dual_n), _stream()))
     return C_out
 
 

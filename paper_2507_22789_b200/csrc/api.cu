@@ -33,17 +33,18 @@ int check_head_args(const void* H, int64_t ldH, const void* W, int64_t ldW, int 
 }
 
 // ---- backward chunk size: rows of the dS buffer (multiple of 256) -----------------------------
-// Minimises the number of dH tile waves over the 74 CTA pairs; larger chunks win ties (fewer fp32
+// Minimises the number of dH tile waves (256 x 512 dual-N tiles over the 74 CTA pairs, the
+// coarsest-grained of the three chunk kernels); larger chunks win ties (fewer fp32
 // read-modify-write passes over dW).  Keeps the chunk below T so the [T,V] matrix is never whole.
 int64_t pick_chunk(int64_t T, int64_t D, int64_t V) {
   const int64_t Tr = ceil_div(T > 0 ? T : 1, 256) * 256;
   if (Tr <= 256) return 256;
   const int P = kNumSMs / 2;
-  const int64_t Nt = ceil_div(D, 256);
+  const int64_t Nt = ceil_div(D, 512);
   const int64_t half = ceil_div(Tr / 2, 256) * 256;          // at least two chunks
   int64_t best = 256;
   double best_cost = 1e300;
-  for (int64_t tc = 256; tc <= 8192 && tc <= half; tc += 256) {
+  for (int64_t tc = 256; tc <= 16384 && tc <= half; tc += 256) {
     if (tc > 256 && (double)tc * (double)V * 2.0 > 6.0e9) break;   // dS buffer <= 6 GB
     int64_t waves = 0;
     for (int64_t r0 = 0; r0 < Tr; r0 += tc) {
@@ -422,12 +423,13 @@ int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* target
 
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
                        int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
-                       int accumulate, int cta_group, int dynamic_schedule, void* cuda_stream) {
+                       int accumulate, int cta_group, int dynamic_schedule, int dual_n,
+                       void* cuda_stream) {
   if (!A || !B || !C) return GC_ERR_NULL;
   if (M <= 0 || N <= 0 || K <= 0) return GC_ERR_SHAPE;
   GC_TRY(check_arch());
   return tc_debug_gemm(A, lda, a_mn_major, B, ldb, b_mn_major, C, ldc, M, N, K, accumulate,
-                       cta_group, dynamic_schedule, static_cast<cudaStream_t>(cuda_stream));
+                       cta_group, dynamic_schedule, dual_n, static_cast<cudaStream_t>(cuda_stream));
 }
 
 }  // extern "C"

@@ -23,12 +23,18 @@ constexpr int kThreads = 256;
 constexpr int kTmemCols = 512;
 constexpr int kABytes = BM_CTA * BK * 2;   // 16 KB
 
-template <int CG> struct Cfg {
-  static constexpr int kBRows = BN / CG;                 // B rows staged by one CTA
+// NSUB = 256-wide N sub-tiles per item step (1 or 2).  NSUB = 2 ("dual-N", CG = 2 only): both TMEM
+// accumulators belong to one 256 x 512 output tile whose two halves share every A stage, which
+// cuts the L2 -> smem operand traffic per flop by a quarter; the epilogue then cannot overlap
+// the next tile's MMAs, so it is for contractions with a very long K (dH: K = V).
+template <int CG, int NSUB = 1> struct Cfg {
+  static_assert(NSUB == 1 || (NSUB == 2 && CG == 2), "dual-N needs the CTA pair");
+  static constexpr int kBRows = BN / CG;                 // B rows of one sub-tile staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;
-  static constexpr int kStageBytes = kABytes + kBBytes;  // 32 KB (CG=2) / 48 KB (CG=1)
-  static constexpr int kStages = CG == 2 ? 6 : 4;
-  static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int kStageBytes = kABytes + NSUB * kBBytes;  // 32 / 48 KB (CG=2), 48 KB (CG=1)
+  static constexpr int kStages = CG == 2 ? (NSUB == 2 ? 4 : 6) : 4;
+  static constexpr int kBarBytes = 1024;   // barriers + item ring (keeps what follows 1024-aligned)
+  static constexpr int kSmemBase = kStages * kStageBytes + 1024 /*align slack*/ + kBarBytes;
 };
 
 // Work schedule.  An item is (M tile, run of N tiles).  Items are handed out in index order to
@@ -112,11 +118,15 @@ __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt,
   return x;
 }
 
-template <int CG, bool A_MN, bool B_MN, class Epi>
+// Epilogue functor contract (tc_head.cu): Params (kernel parameter, __grid_constant__ so that it
+// may hold a CUtensorMap), State (registers of one epilogue thread), kWarpSmem (bytes of staging
+// smem per epilogue warp, 1024-aligned), setup / item_begin / tile_prefetch / chunk / item_end /
+// finish.
+template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1>
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-          const Sched s, const typename Epi::Params ep) {
-  using C = Cfg<CG>;
+          const Sched s, const __grid_constant__ typename Epi::Params ep) {
+  using C = Cfg<CG, NSUB>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + C::kStages * C::kStageBytes;
@@ -171,7 +181,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   int64_t M_eff, K_eff;
   resolve_dims(s, M_eff, K_eff);
   const int64_t Mt = (M_eff + BM_CTA * CG - 1) / (BM_CTA * CG);
-  const int64_t Nt = (s.N + BN - 1) / BN;
+  const int64_t Nt = (s.N + BN * NSUB - 1) / (BN * NSUB);   // item tiles along N
   const int64_t n_chunks = s.c_major ? (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles : Nt;
   const int num_kb = (int)((K_eff + BK - 1) / BK);
   const int64_t n_items = (s.skip_empty_k && num_kb == 0) ? 0 : Mt * n_chunks;
@@ -228,7 +238,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         const Item item = get_item(s, it, Mt, Nt);
         const int32_t m_coord = (int32_t)(item.m_tile * BM_CTA * CG + rank * BM_CTA);
         for (int64_t n = item.n0; n < item.n1; ++n) {
-          const int32_t n_coord = (int32_t)(n * BN + rank * C::kBRows);
+          const int32_t n_coord = (int32_t)(n * BN * NSUB + rank * C::kBRows);
           for (int kb = 0; kb < num_kb; ++kb) {
             ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
             const uint32_t sa = smem_base + stage * C::kStageBytes;
@@ -242,11 +252,16 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::tma_load_2d(sa, &tmA, m_coord, k_coord, fb, polA);
                 ptx::tma_load_2d(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
               }
-              if constexpr (!B_MN) ptx::tma_load_2d(sb, &tmB, k_coord, n_coord, fb, polB);
-              else {
 #pragma unroll
-                for (int b = 0; b < C::kBRows / 64; ++b)
-                  ptx::tma_load_2d(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb, polB);
+              for (int sub = 0; sub < NSUB; ++sub) {
+                const uint32_t sbs = sb + sub * C::kBBytes;
+                const int32_t nc = n_coord + sub * BN;
+                if constexpr (!B_MN) ptx::tma_load_2d(sbs, &tmB, k_coord, nc, fb, polB);
+                else {
+#pragma unroll
+                  for (int b = 0; b < C::kBRows / 64; ++b)
+                    ptx::tma_load_2d(sbs + 8192 * b, &tmB, nc + 64 * b, k_coord, fb, polB);
+                }
               }
             } else {
               // the leader's barrier collects the bytes of both CTAs
@@ -257,11 +272,16 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb, polA);
                 ptx::tma_load_2d_cg2(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
               }
-              if constexpr (!B_MN) ptx::tma_load_2d_cg2(sb, &tmB, k_coord, n_coord, fb, polB);
-              else {
 #pragma unroll
-                for (int b = 0; b < C::kBRows / 64; ++b)
-                  ptx::tma_load_2d_cg2(sb + 8192 * b, &tmB, n_coord + 64 * b, k_coord, fb, polB);
+              for (int sub = 0; sub < NSUB; ++sub) {
+                const uint32_t sbs = sb + sub * C::kBBytes;
+                const int32_t nc = n_coord + sub * BN;
+                if constexpr (!B_MN) ptx::tma_load_2d_cg2(sbs, &tmB, k_coord, nc, fb, polB);
+                else {
+#pragma unroll
+                  for (int b = 0; b < C::kBRows / 64; ++b)
+                    ptx::tma_load_2d_cg2(sbs + 8192 * b, &tmB, nc + 64 * b, k_coord, fb, polB);
+                }
               }
             }
             if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
@@ -284,24 +304,40 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       for (int64_t it = consume(false); it >= 0; it = consume(false)) {
         const Item item = get_item(s, it, Mt, Nt);
         for (int64_t n = item.n0; n < item.n1; ++n) {
-          ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+          // NSUB == 1: the two accumulators alternate between N tiles; NSUB == 2: both belong
+          // to this tile (sub-tile `sub` accumulates in buffer `sub`)
+          if constexpr (NSUB == 1) {
+            ptx::mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+          } else {
+            ptx::mbar_wait(tempty_bar(0), acc_phase ^ 1u);
+            ptx::mbar_wait(tempty_bar(1), acc_phase ^ 1u);
+          }
           ptx::tc_fence_after();
-          const uint32_t d_tmem = tmem_base + (uint32_t)acc * BN;
           for (int kb = 0; kb < num_kb; ++kb) {
             ptx::mbar_wait(full_bar(stage), phase);
             ptx::tc_fence_after();
             const uint32_t sa = smem_base + stage * C::kStageBytes;
             const uint64_t adesc = ptx::make_smem_desc(sa, A_MN);
-            const uint64_t bdesc = ptx::make_smem_desc(sa + kABytes, B_MN);
 #pragma unroll
-            for (int k = 0; k < BK / 16; ++k)
-              ptx::umma_bf16<CG>(d_tmem, adesc + (uint64_t)(k * a_step),
-                                 bdesc + (uint64_t)(k * b_step), idesc, (uint32_t)(kb | k));
+            for (int sub = 0; sub < NSUB; ++sub) {
+              const uint32_t d_tmem = tmem_base + (uint32_t)(NSUB == 1 ? acc : sub) * BN;
+              const uint64_t bdesc = ptx::make_smem_desc(sa + kABytes + sub * C::kBBytes, B_MN);
+#pragma unroll
+              for (int k = 0; k < BK / 16; ++k)
+                ptx::umma_bf16<CG>(d_tmem, adesc + (uint64_t)(k * a_step),
+                                   bdesc + (uint64_t)(k * b_step), idesc, (uint32_t)(kb | k));
+            }
             ptx::umma_commit<CG>(empty_bar(stage));      // frees the smem slot (both CTAs)
             if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
           }
-          ptx::umma_commit<CG>(tfull_bar(acc));          // accumulator ready (both CTAs)
-          if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+          if constexpr (NSUB == 1) {
+            ptx::umma_commit<CG>(tfull_bar(acc));        // accumulator ready (both CTAs)
+            if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+          } else {
+            ptx::umma_commit<CG>(tfull_bar(0));
+            ptx::umma_commit<CG>(tfull_bar(1));
+            acc_phase ^= 1u;
+          }
         }
       }
     }
@@ -313,13 +349,15 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     int acc = 0;
     uint32_t acc_phase = 0;
     typename Epi::State st;
-    Epi::setup(st, ep);
+    Epi::setup(st, ep, bar_base + C::kBarBytes + (uint32_t)(q * Epi::kWarpSmem));
     for (int64_t it = consume(true); it >= 0; it = consume(true)) {
       const Item item = get_item(s, it, Mt, Nt);
       const int64_t grow = item.m_tile * BM_CTA * CG + rank * BM_CTA + row_in_tile;
       const bool valid = grow < M_eff;
       Epi::item_begin(st, ep, grow, valid, item.c);
-      for (int64_t n = item.n0; n < item.n1; ++n) {
+      for (int64_t nn = item.n0 * NSUB; nn < item.n1 * NSUB; ++nn) {
+        const int64_t n = nn;                            // 256-wide tile index along N
+        Epi::tile_prefetch(ep, grow, valid, n * BN);
         ptx::mbar_wait(tfull_bar(acc), acc_phase);
         ptx::tc_fence_after();
 #pragma unroll 1
@@ -351,6 +389,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       }
       Epi::item_end(st, ep, grow, valid, item.c);
     }
+    Epi::finish(st, ep);
   }
 
   // ---- teardown ----
@@ -411,17 +450,18 @@ inline int num_sms() {
   return n;
 }
 
-template <int CG, bool A_MN, bool B_MN, class Epi>
+template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1>
 int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& s,
                    const typename Epi::Params& ep, cudaStream_t st) {
-  auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi>;
-  GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   Cfg<CG>::kSmemBytes));
+  auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi, NSUB>;
+  constexpr int kSmemBytes = Cfg<CG, NSUB>::kSmemBase + 4 * Epi::kWarpSmem;
+  static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
+  GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
   cudaLaunchConfig_t cfg = {};
   const int sms = num_sms();
   cfg.gridDim = dim3((unsigned)(sms / CG * CG));
   cfg.blockDim = dim3(kThreads);
-  cfg.dynamicSmemBytes = Cfg<CG>::kSmemBytes;
+  cfg.dynamicSmemBytes = kSmemBytes;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;

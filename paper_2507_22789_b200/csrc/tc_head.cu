@@ -20,6 +20,7 @@ using tc::Sched;
 // A thread owns one row; state lives in registers across the N tiles of an item.
 // ---------------------------------------------------------------------------------------------
 struct EpiStats {
+  static constexpr int kWarpSmem = 0;
   struct Params {
     const int32_t* targets;   // [rows] compact targets
     RowStat* partials;        // [n_split][split_stride]
@@ -28,7 +29,7 @@ struct EpiStats {
     float c;                  // log2(e) / tau
   };
   struct State { float m, s0, s1, u0, u1, ay; int32_t y; };
-  static __device__ __forceinline__ void setup(State&, const Params&) {}
+  static __device__ __forceinline__ void setup(State&, const Params&, uint32_t) {}
 
   static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
                                                     bool valid, int64_t) {
@@ -37,6 +38,7 @@ struct EpiStats {
     st.s0 = st.s1 = st.u0 = st.u1 = 0.f;
     st.ay = -INFINITY;
   }
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
   static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t, bool,
                                                int64_t col0, const float (&x)[32]) {
     if (col0 >= p.V) return;
@@ -79,6 +81,7 @@ struct EpiStats {
     o.ay = st.ay;
     p.partials[c * p.split_stride + row] = o;
   }
+  static __device__ __forceinline__ void finish(State&, const Params&) {}
 };
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -91,6 +94,7 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 // dynamic row count and for columns >= V (the dW contraction runs over those rows).
 // ---------------------------------------------------------------------------------------------
 struct EpiDS {
+  static constexpr int kWarpSmem = 0;
   struct Params {
     const int32_t* targets;   // chunk-local compact arrays
     const float* lse;
@@ -106,7 +110,7 @@ struct EpiDS {
     int64_t cap;              // chunk capacity
   };
   struct State { float lse2, gp; int32_t y; int64_t n_eff; };
-  static __device__ __forceinline__ void setup(State& st, const Params& p) {
+  static __device__ __forceinline__ void setup(State& st, const Params& p, uint32_t) {
     int64_t n = p.n_static;
     if (p.n_dyn) {
       n = (int64_t)(*p.n_dyn) - p.row0;
@@ -125,6 +129,7 @@ struct EpiDS {
       if (st.y < 0) st.gp = 0.f;
     }
   }
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
   static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool,
                                                int64_t col0, const float (&x)[32]) {
     if (col0 >= p.ldS) return;
@@ -149,18 +154,21 @@ struct EpiDS {
     uint4* dst = reinterpret_cast<uint4*>(p.dS + row * p.ldS + col0);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      if (col0 + 8 * q < p.ldS)
-        dst[q] = make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
-                            pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
+      if (col0 + 8 * q < p.ldS)     // streaming store: 2 GB per chunk must not evict the H band
+        __stcs(dst + q,
+               make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
+                          pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7])));
     }
   }
   static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void finish(State&, const Params&) {}
 };
 
 // ---------------------------------------------------------------------------------------------
 // Epilogue a11: store bf16 rows, optionally scattered through rows[] (dH of compacted tokens).
 // ---------------------------------------------------------------------------------------------
 struct EpiStoreBf16 {
+  static constexpr int kWarpSmem = 0;
   struct Params {
     __nv_bfloat16* out;
     int64_t ldo;
@@ -169,11 +177,12 @@ struct EpiStoreBf16 {
     int64_t N;
   };
   struct State { int64_t orow; };
-  static __device__ __forceinline__ void setup(State&, const Params&) {}
+  static __device__ __forceinline__ void setup(State&, const Params&, uint32_t) {}
   static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
                                                     bool valid, int64_t) {
     st.orow = valid ? (p.rows ? (int64_t)p.rows[row] : p.row_base + row) : -1;
   }
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
   static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t, bool,
                                                int64_t col0, const float (&x)[32]) {
     if (st.orow < 0 || col0 >= p.N) return;
@@ -186,43 +195,75 @@ struct EpiStoreBf16 {
     }
   }
   static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void finish(State&, const Params&) {}
 };
 
 // ---------------------------------------------------------------------------------------------
-// Epilogue a12 (and the debug GEMM): fp32 store or accumulate.
+// Epilogue a12 (and the debug GEMM): fp32 tile store, or accumulate, through TMA.  Each epilogue
+// warp stages its 32 rows x 32 columns (4 KB, 128-byte-swizzled, double-buffered) in shared memory
+// and one lane issues a bulk tensor store -- or, when accumulating, a bulk tensor REDUCE-ADD, so
+// the read-modify-write of dW happens at the L2 and the old values never travel to the SM.  Every
+// dW element receives exactly one add per launch and launches are stream-ordered, so the result
+// is deterministic.  Rows >= M and columns >= N are clipped by the tensor map.
+// (A register read-add-store epilogue was latency-bound: cfg4's accumulating dW launch ran at 27 %
+// tensor-pipe activity, profiles/.)
 // ---------------------------------------------------------------------------------------------
 struct EpiStoreF32 {
-  struct Params {
-    float* out;
-    int64_t ldo;
+  static constexpr int kWarpSmem = 2 * 4096;
+  struct alignas(64) Params {
+    CUtensorMap tm;           // fp32 [M, N] (row stride ldo), box {32 columns, 32 rows}, swizzle 128B
     int64_t N;
     int accumulate;
   };
-  struct State { int dummy; };
-  static __device__ __forceinline__ void setup(State&, const Params&) {}
+  struct State { uint32_t smem; uint32_t buf; };
+  static __device__ __forceinline__ void setup(State& st, const Params&, uint32_t warp_smem) {
+    st.smem = warp_smem;
+    st.buf = 0;
+  }
   static __device__ __forceinline__ void item_begin(State&, const Params&, int64_t, bool, int64_t) {}
-  static __device__ __forceinline__ void chunk(State&, const Params& p, int64_t row, bool valid,
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool,
                                                int64_t col0, const float (&x)[32]) {
-    if (!valid || col0 >= p.N) return;
-    float4* dst = reinterpret_cast<float4*>(p.out + row * p.ldo + col0);
-    if (p.accumulate) {
-      float4 prev[8];
+    if (col0 >= p.N) return;                       // uniform over the warp
+    const int lane = threadIdx.x & 31;
+    const uint32_t base = st.smem + st.buf * 4096u;
+    st.buf ^= 1u;
+    // the store issued two chunks ago (same buffer) must have finished reading it
+    if (lane == 0) ptx::bulk_wait_group_read<1>();
+    __syncwarp();
+    const uint32_t rbase = base + (uint32_t)lane * 128u;
 #pragma unroll
-      for (int q = 0; q < 8; ++q)
-        prev[q] = (col0 + 4 * q < p.N) ? dst[q] : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-      for (int q = 0; q < 8; ++q)
-        if (col0 + 4 * q < p.N)
-          dst[q] = make_float4(prev[q].x + x[4 * q], prev[q].y + x[4 * q + 1],
-                               prev[q].z + x[4 * q + 2], prev[q].w + x[4 * q + 3]);
-    } else {
-#pragma unroll
-      for (int q = 0; q < 8; ++q)
-        if (col0 + 4 * q < p.N) dst[q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
+    for (int q = 0; q < 8; ++q)
+      ptx::st_shared_v4(rbase + (uint32_t)((q ^ (lane & 7)) << 4), x[4 * q], x[4 * q + 1],
+                        x[4 * q + 2], x[4 * q + 3]);
+    ptx::fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      // `row` is this lane's row = first row of the warp's 32-row slab
+      if (p.accumulate) ptx::tma_reduce_add_2d(&p.tm, base, (int32_t)col0, (int32_t)row);
+      else ptx::tma_store_2d(&p.tm, base, (int32_t)col0, (int32_t)row);
+      ptx::bulk_commit_group();
     }
   }
   static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void finish(State&, const Params&) {
+    if ((threadIdx.x & 31) == 0) ptx::bulk_wait_group_read<0>();
+  }
 };
+
+static int make_f32_out_tmap(CUtensorMap* m, float* out, int64_t rows, int64_t cols, int64_t ld) {
+  tc::PFN_encodeTiled fn = tc::get_encode_fn();
+  if (!fn) return GC_ERR_CUDA;
+  if ((reinterpret_cast<uintptr_t>(out) & 15) || ((ld * 4) & 15)) return GC_ERR_ALIGN;
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+  cuuint32_t box[2] = {32, 32};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, out, dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? GC_OK : GC_ERR_CUDA;
+}
 
 // ---------------------------------------------------------------------------------------------
 // forward plan: choose the number of N tiles per item so that the items balance over the CTA
@@ -252,7 +293,7 @@ TcPlan tc_plan_forward(int64_t T, int64_t V) {
 // L2 budget for the operand panels a schedule keeps resident.  Measured (profiles/): bands up to
 // ~48 MB stay resident, 60 MB and more thrash (DRAM reads x2.5 .. x7) -- about half of the 126 MB,
 // consistent with each die's L2 also holding the lines its SMs fetch from the other die.
-constexpr int64_t kL2ResidentBytes = 44ll << 20;
+constexpr int64_t kL2ResidentBytes = 40ll << 20;
 
 // M tiles per band of the forward / recompute schedule: the band's A panels (m_band x 256 rows x
 // D bf16) stay in L2 while the N sweep streams W past; W is re-read once per band.
@@ -293,7 +334,11 @@ static void exp_override(Sched& s, const char* kind) {
 
 template <class Epi, bool A_MN, bool B_MN>
 static int launch_cg(int cg, const CUtensorMap& a, const CUtensorMap& b, const Sched& s,
-                     const typename Epi::Params& ep, cudaStream_t st) {
+                     const typename Epi::Params& ep, cudaStream_t st, bool dual_n = false) {
+  if (dual_n) {
+    if (cg != 2) return GC_ERR_ARG;
+    return tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 2>(a, b, s, ep, st);
+  }
   if (cg == 2) return tc::launch_tc_gemm<2, A_MN, B_MN, Epi>(a, b, s, ep, st);
   return tc::launch_tc_gemm<1, A_MN, B_MN, Epi>(a, b, s, ep, st);
 }
@@ -321,7 +366,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   s.m_band = pick_m_band(D);
   s.counter = counter;
   s.a_hint = ptx::kL2EvictLast;     // the band's H tiles are re-read for every vocab tile
-  s.b_hint = ptx::kL2EvictFirst;    // W streams past
+  s.b_hint = ptx::kL2Normal;        // W streams past, shared by the band's pairs a few us apart
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = 0; s.dyn_cap = T; }
   EpiStats::Params ep;
   ep.targets = targets_c;
@@ -352,7 +397,7 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   s.m_band = pick_m_band(D);
   s.counter = counter;
   s.a_hint = ptx::kL2EvictLast;
-  s.b_hint = ptx::kL2EvictFirst;
+  s.b_hint = ptx::kL2Normal;
   if (n_rows_dev) {
     s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; s.dyn_round = 256;
   }
@@ -392,7 +437,8 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.N = D;
   GC_EXP_OVERRIDE(s, "DH");
   KernelTimer kt(GC_KERNEL_DH, st);
-  return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st);
+  // K = V is ~2000 k-blocks per tile: 256 x 512 dual-N tiles (tc_gemm.cuh, Cfg)
+  return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st, cg == 2);
 }
 
 int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
@@ -407,14 +453,13 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   // items (D band, vocab tile, D tile in band): the band's H panels stay in L2, the D tiles of a
   // vocab tile run together and share its dS^T panel, which streams past once per band
   s.counter = counter;
-  s.a_hint = ptx::kL2EvictFirst;
+  s.a_hint = ptx::kL2Normal;
   s.b_hint = ptx::kL2EvictLast;
   s.n_band = pick_n_band(k_rows);
   s.skip_empty_k = accumulate ? 1 : 0;
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 2; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
   EpiStoreF32::Params ep;
-  ep.out = dW;
-  ep.ldo = lddW;
+  GC_TRY(make_f32_out_tmap(&ep.tm, dW, V, D, lddW));
   ep.N = D;
   ep.accumulate = accumulate;
   GC_EXP_OVERRIDE(s, "DW");
@@ -427,8 +472,9 @@ __device__ uint32_t g_debug_counter;
 
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, int dynamic_schedule, cudaStream_t st) {
+                  int cta_group, int dynamic_schedule, int dual_n, cudaStream_t st) {
   if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
+  if (dual_n && cta_group != 2) return GC_ERR_ARG;
   if (N % 4 != 0) return GC_ERR_SHAPE;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
@@ -441,14 +487,14 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
     s.counter = static_cast<uint32_t*>(ctr);
   }
   EpiStoreF32::Params ep;
-  ep.out = C;
-  ep.ldo = ldc;
+  GC_TRY(make_f32_out_tmap(&ep.tm, C, M, N, ldc));
   ep.N = N;
   ep.accumulate = accumulate;
-  if (!a_mn && !b_mn) return launch_cg<EpiStoreF32, false, false>(cta_group, ta, tb, s, ep, st);
-  if (!a_mn && b_mn) return launch_cg<EpiStoreF32, false, true>(cta_group, ta, tb, s, ep, st);
-  if (a_mn && !b_mn) return launch_cg<EpiStoreF32, true, false>(cta_group, ta, tb, s, ep, st);
-  return launch_cg<EpiStoreF32, true, true>(cta_group, ta, tb, s, ep, st);
+  const bool d2 = dual_n != 0;
+  if (!a_mn && !b_mn) return launch_cg<EpiStoreF32, false, false>(cta_group, ta, tb, s, ep, st, d2);
+  if (!a_mn && b_mn) return launch_cg<EpiStoreF32, false, true>(cta_group, ta, tb, s, ep, st, d2);
+  if (a_mn && !b_mn) return launch_cg<EpiStoreF32, true, false>(cta_group, ta, tb, s, ep, st, d2);
+  return launch_cg<EpiStoreF32, true, true>(cta_group, ta, tb, s, ep, st, d2);
 }
 
 }  // namespace gc

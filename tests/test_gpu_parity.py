@@ -55,6 +55,25 @@ def test_engine_gemm(B, dyn, cg, a_mn, b_mn, M, N, K):
 
 
 @pytest.mark.parametrize("dyn", [False, True])
+@pytest.mark.parametrize("a_mn,b_mn", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K", [(256, 512, 64), (392, 520, 200), (1000, 776, 1096),
+                                   (256 * 5 + 8, 256 * 7 + 8, 328)])
+def test_engine_gemm_dual_n(B, dyn, a_mn, b_mn, M, N, K):
+    """256 x 512 dual-N tiles (the dH kernel's tile), incl. an odd number of 256-wide N tiles."""
+    g = torch.Generator(device="cuda").manual_seed(M + N + K + 1)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    C = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
+                             a_mn, b_mn, cta_group=2, dynamic_schedule=dyn, dual_n=True)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    C2 = B.gc_debug_gemm_bf16(A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm,
+                              a_mn, b_mn, C_out=C.clone(), accumulate=True, cta_group=2,
+                              dynamic_schedule=dyn, dual_n=True)
+    assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+
+
+@pytest.mark.parametrize("dyn", [False, True])
 def test_engine_gemm_many_tiles(B, dyn):
     """More tiles than CTA pairs (several items per pair, ragged edges), both schedules; the
     dynamic one must also be deterministic (the tile -> pair map does not enter the result)."""

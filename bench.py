@@ -397,8 +397,6 @@ def main():
     value = tokens_all / (ms_per_step * 1e-3)
 
     if rank == 0:
-        passes = 4 if w.backward else 1
-        flops = 2.0 * tokens * w.D * w.V * passes          # algorithmic: scored rows only
         step_ms = float(np.mean(per))
         long_run = total_ms > 1000.0
         roof = roofline(w, tokens, args.steps, kinds, step_ms, long_run, peaks)

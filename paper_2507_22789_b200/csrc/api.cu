@@ -33,9 +33,11 @@ int check_head_args(const void* H, int64_t ldH, const void* W, int64_t ldW, int 
 }
 
 // ---- backward chunk size: rows of the dS buffer (multiple of 256) -----------------------------
-// Minimises the number of dH tile waves (256 x 512 dual-N tiles over the 74 CTA pairs, the
-// coarsest-grained of the three chunk kernels); larger chunks win ties (fewer fp32
-// read-modify-write passes over dW).  Keeps the chunk below T so the [T,V] matrix is never whole.
+// Minimises the number of dH tile waves -- the coarsest-grained of the three chunk kernels: 256 x 512
+// dual-N tiles over the 74 CTA pairs, a last wave that is at most half full costing half a wave
+// (tc_gemm.cuh) -- with a small charge per chunk (one more fp32 accumulate pass over dW); larger
+// chunks win ties.  Capped at 8192 rows / 6 GB (measured: 8192, 12288 and 16384 rows run cfg2 within
+// 1 % of each other) and at T/2, so the [T,V] matrix never exists whole.
 int64_t pick_chunk(int64_t T, int64_t D, int64_t V) {
   const int64_t Tr = ceil_div(T > 0 ? T : 1, 256) * 256;
   if (Tr <= 256) return 256;
@@ -44,14 +46,16 @@ int64_t pick_chunk(int64_t T, int64_t D, int64_t V) {
   const int64_t half = ceil_div(Tr / 2, 256) * 256;          // at least two chunks
   int64_t best = 256;
   double best_cost = 1e300;
-  for (int64_t tc = 256; tc <= 16384 && tc <= half; tc += 256) {
+  for (int64_t tc = 256; tc <= 8192 && tc <= half; tc += 256) {
     if (tc > 256 && (double)tc * (double)V * 2.0 > 6.0e9) break;   // dS buffer <= 6 GB
-    int64_t waves = 0;
+    double waves = 0;
     for (int64_t r0 = 0; r0 < Tr; r0 += tc) {
       const int64_t rows = (Tr - r0 < tc) ? Tr - r0 : tc;
-      waves += ceil_div(ceil_div(rows, 256) * Nt, P);
+      const int64_t items = ceil_div(rows, 256) * Nt;
+      const int64_t r = items % P;
+      waves += (double)(items / P) + (r == 0 ? 0.0 : (2 * r <= P ? 0.5 : 1.0));
     }
-    const double cost = (double)waves * (1.0 + 0.01 * (double)ceil_div(Tr, tc));
+    const double cost = waves * (1.0 + 0.01 * (double)ceil_div(Tr, tc));
     if (cost <= best_cost) { best_cost = cost; best = tc; }
   }
   return best;

@@ -75,10 +75,11 @@ __device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t
   }
 }
 
-struct Item { int64_t m_tile, n0, n1, c; };
+struct Item { int64_t m_tile, n0, n1, c; int half; };   // half: dual-N tail, see k_tc_gemm
 
 __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt, int64_t Nt) {
   Item x;
+  x.half = -1;
   if (s.c_major) {
     const int64_t C = (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles;
     const int64_t band = s.m_band > 0 ? s.m_band : Mt;
@@ -184,7 +185,27 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   const int64_t Nt = (s.N + BN * NSUB - 1) / (BN * NSUB);   // item tiles along N
   const int64_t n_chunks = s.c_major ? (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles : Nt;
   const int num_kb = (int)((K_eff + BK - 1) / BK);
-  const int64_t n_items = (s.skip_empty_k && num_kb == 0) ? 0 : Mt * n_chunks;
+  // Dual-N tail: 256 x 512 tiles make the waves coarse.  When the last wave would be at most
+  // half full, its r tiles are issued as 2r half tiles (one 256 x 256 sub-tile each, `half` = 0/1)
+  // spread over twice as many pairs: the tail costs half a wave instead of a whole one.
+  int64_t tail_start = Mt * n_chunks, n_total = Mt * n_chunks;
+  if constexpr (NSUB == 2) {
+    const int64_t full = n_total / n_pairs * n_pairs, r = n_total - full;
+    if (s.counter == nullptr && !s.c_major && r > 0 && 2 * r <= n_pairs) {
+      tail_start = full;
+      n_total = full + 2 * r;
+    }
+  }
+  const int64_t n_items = (s.skip_empty_k && num_kb == 0) ? 0 : n_total;
+  auto item_of = [&](int64_t it) -> Item {
+    if (NSUB == 2 && it >= tail_start) {
+      const int64_t j = it - tail_start;
+      Item x = get_item(s, tail_start + (j >> 1), Mt, Nt);
+      x.half = (int)(j & 1);
+      return x;
+    }
+    return get_item(s, it, Mt, Nt);
+  };
 
   // ---- item stream -------------------------------------------------------------------------
   const bool dynamic = s.counter != nullptr;
@@ -235,17 +256,20 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         uint32_t ticket = 0;
         if (scheduler) ticket = atomicAdd(s.counter, 1u);
         int64_t it_next = -1;
-        const Item item = get_item(s, it, Mt, Nt);
+        const Item item = item_of(it);
         const int32_t m_coord = (int32_t)(item.m_tile * BM_CTA * CG + rank * BM_CTA);
         for (int64_t n = item.n0; n < item.n1; ++n) {
-          const int32_t n_coord = (int32_t)(n * BN * NSUB + rank * C::kBRows);
+          const int nsub = item.half < 0 ? NSUB : 1;    // half tile: one B sub-tile, in slot 0
+          const int32_t n_coord = (int32_t)(n * BN * NSUB + (item.half > 0 ? BN : 0) +
+                                            rank * C::kBRows);
+          const uint32_t stage_tx = (uint32_t)(kABytes + nsub * C::kBBytes);
           for (int kb = 0; kb < num_kb; ++kb) {
             ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
             const uint32_t sa = smem_base + stage * C::kStageBytes;
             const uint32_t sb = sa + kABytes;
             const int32_t k_coord = kb * BK;
             if constexpr (CG == 1) {
-              ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes);
+              ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               const uint32_t fb = full_bar(stage);
               if constexpr (!A_MN) ptx::tma_load_2d(sa, &tmA, k_coord, m_coord, fb, polA);
               else {
@@ -254,6 +278,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               }
 #pragma unroll
               for (int sub = 0; sub < NSUB; ++sub) {
+                if (sub >= nsub) break;
                 const uint32_t sbs = sb + sub * C::kBBytes;
                 const int32_t nc = n_coord + sub * BN;
                 if constexpr (!B_MN) ptx::tma_load_2d(sbs, &tmB, k_coord, nc, fb, polB);
@@ -265,7 +290,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               }
             } else {
               // the leader's barrier collects the bytes of both CTAs
-              if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), C::kStageBytes * 2);
+              if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx * 2);
               const uint32_t fb = ptx::mapa(full_bar(stage), 0);
               if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb, polA);
               else {
@@ -274,6 +299,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               }
 #pragma unroll
               for (int sub = 0; sub < NSUB; ++sub) {
+                if (sub >= nsub) break;
                 const uint32_t sbs = sb + sub * C::kBBytes;
                 const int32_t nc = n_coord + sub * BN;
                 if constexpr (!B_MN) ptx::tma_load_2d_cg2(sbs, &tmB, k_coord, nc, fb, polB);
@@ -302,7 +328,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
       int acc = 0;
       uint32_t acc_phase = 0;
       for (int64_t it = consume(false); it >= 0; it = consume(false)) {
-        const Item item = get_item(s, it, Mt, Nt);
+        const Item item = item_of(it);
         for (int64_t n = item.n0; n < item.n1; ++n) {
           // NSUB == 1: the two accumulators alternate between N tiles; NSUB == 2: both belong
           // to this tile (sub-tile `sub` accumulates in buffer `sub`)
@@ -320,6 +346,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             const uint64_t adesc = ptx::make_smem_desc(sa, A_MN);
 #pragma unroll
             for (int sub = 0; sub < NSUB; ++sub) {
+              if (sub > 0 && item.half >= 0) break;      // half tile: accumulator 0 only
               const uint32_t d_tmem = tmem_base + (uint32_t)(NSUB == 1 ? acc : sub) * BN;
               const uint64_t bdesc = ptx::make_smem_desc(sa + kABytes + sub * C::kBBytes, B_MN);
 #pragma unroll
@@ -351,15 +378,28 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     typename Epi::State st;
     Epi::setup(st, ep, bar_base + C::kBarBytes + (uint32_t)(q * Epi::kWarpSmem));
     for (int64_t it = consume(true); it >= 0; it = consume(true)) {
-      const Item item = get_item(s, it, Mt, Nt);
+      const Item item = item_of(it);
       const int64_t grow = item.m_tile * BM_CTA * CG + rank * BM_CTA + row_in_tile;
       const bool valid = grow < M_eff;
       Epi::item_begin(st, ep, grow, valid, item.c);
       for (int64_t nn = item.n0 * NSUB; nn < item.n1 * NSUB; ++nn) {
-        const int64_t n = nn;                            // 256-wide tile index along N
-        Epi::tile_prefetch(ep, grow, valid, n * BN);
+        // 256-wide tile index along N; a half tile keeps its data in accumulator 0 and only
+        // hands accumulator 1 back
+        const int64_t n = item.half > 0 ? nn + 1 : nn;
+        const bool skip = NSUB == 2 && item.half >= 0 && nn != item.n0 * NSUB;
+        Epi::tile_prefetch(ep, grow, valid && !skip, n * BN);
         ptx::mbar_wait(tfull_bar(acc), acc_phase);
         ptx::tc_fence_after();
+        if (skip) {
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) {
+            if constexpr (CG == 1) ptx::mbar_arrive(tempty_bar(acc));
+            else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
+          }
+          if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+          continue;
+        }
 #pragma unroll 1
         for (int ch = 0; ch < BN / 32; ++ch) {
           uint32_t r[32];

@@ -73,17 +73,20 @@ def test_engine_gemm_dual_n(B, dyn, a_mn, b_mn, M, N, K):
     assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
 
 
+@pytest.mark.parametrize("dual", [False, True])
 @pytest.mark.parametrize("dyn", [False, True])
-def test_engine_gemm_many_tiles(B, dyn):
+def test_engine_gemm_many_tiles(B, dyn, dual):
     """More tiles than CTA pairs (several items per pair, ragged edges), both schedules; the
-    dynamic one must also be deterministic (the tile -> pair map does not enter the result)."""
+    dynamic one must also be deterministic (the tile -> pair map does not enter the result).
+    dual + static: 22 x 5 = 110 dual tiles = one full wave of 74 + 36 tiles issued as 72 half
+    tiles (the dual-N tail)."""
     M, N, K = 256 * 21 + 40, 256 * 9 + 8, 320
     g = torch.Generator(device="cuda").manual_seed(5)
     A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
     Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
     ref = A.float() @ Bm.float().T
-    C1 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn)
-    C2 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn)
+    C1 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn, dual_n=dual)
+    C2 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn, dual_n=dual)
     assert (C1 - ref).abs().max().item() < 1e-3 * K ** 0.5
     assert torch.equal(C1, C2)
 

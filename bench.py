@@ -329,6 +329,51 @@ def roofline(w, tokens, steps, kinds, step_ms, long_run, peaks):
     }
 
 
+def hbm_kernels(B, device, peaks):
+    """The HBM-bound kernels of the path (rows a1, a8, a9) on scaled-up stand-ins -- at the configs'
+    own sizes they move < 6 MB (loss) / 0.4 GB (gather) and are launch-latency bound (DESIGN.md
+    sec 6.3).  Algorithmic bytes / CUDA-event time, against the measured copy bandwidth."""
+    def timeit(fn, n=10):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+    out = {"peak_gbs": peaks["hbm"], "stand_in": True}
+    T = 1 << 26
+    R = T // 16
+    g = torch.Generator(device=device).manual_seed(0)
+    logp = -3.0 * torch.rand(T, device=device, generator=g)
+    old = logp + 0.05 * torch.randn(T, device=device, generator=g)
+    ref = logp + 0.1 * torch.randn(T, device=device, generator=g)
+    y = torch.randint(0, 1000, (T,), device=device, dtype=torch.int32, generator=g)
+    mask = (torch.rand(T, device=device, generator=g) < 0.75).to(torch.uint8)
+    cu = torch.arange(0, T + 1, 16, device=device, dtype=torch.int32)
+    adv = torch.randn(R, device=device, generator=g)
+    ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv))
+    # reads logp, old, ref, target (4 B each) + mask (1 B), writes g (4 B); the integer count pass
+    # that fixes the normaliser re-reads target + mask (5 B)
+    gbs = 26.0 * T / ms / 1e6
+    out["token_loss_and_grad"] = {"tokens": T, "responses": R, "bytes_per_token": 26, "ms": ms,
+                                  "gbs": gbs, "frac": gbs / peaks["hbm"]}
+    del logp, old, ref, y, mask, cu, adv
+    T2, D = 1 << 19, 4096
+    H = torch.randn(T2, D, device=device, generator=g).to(torch.bfloat16)
+    y2 = torch.zeros(T2, device=device, dtype=torch.int32)
+    m2 = (torch.rand(T2, device=device, generator=g) < 0.75).to(torch.uint8)
+    n = int(m2.sum())
+    ms = timeit(lambda: B.gc_compact_rows(H, y2, m2))
+    gbs = (2.0 * n * D * 2 + 9.0 * T2) / ms / 1e6
+    out["compact_and_gather_rows"] = {"rows": T2, "scored_rows": n, "hidden": D, "ms": ms,
+                                      "gbs": gbs, "frac": gbs / peaks["hbm"]}
+    return out
+
+
 def e2e_measure(B, b: DeviceBatch, steps, warmup):
     """Same metric through the C-ABI call with HOST buffers: per step H2D of H / targets / mask
     from pinned memory, the kernels, D2H of logp + entropy, all inside the timed region."""
@@ -417,6 +462,7 @@ def main():
                               "ms_per_step": ms, "pass": "fwd (gc_token_logprobs_host)"}
             out["cpu_baseline"] = cpu_baseline(w, 256 if w.D * w.V > 1e8 else 1 << 30)
             if args.workload == "cfg1":
+                out["hbm_kernels"] = hbm_kernels(B, torch.device("cuda", local_rank), peaks)
                 # the metric's second half: fwd+bwd on the 8B-class training micro-batch
                 del b
                 torch.cuda.empty_cache()

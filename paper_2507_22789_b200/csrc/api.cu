@@ -76,7 +76,7 @@ size_t carve_fwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, FwdWs* w
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   if (dtype == GC_BF16) {
     uint32_t* ctr = c.take<uint32_t>(kTcCounters);
-    RowStat* p = c.take<RowStat>(tc_fwd_partials_bytes(T, V) / sizeof(RowStat));
+    RowStat* p = c.take<RowStat>(tc_fwd_partials_bytes(T, D, V) / sizeof(RowStat));
     int32_t* rows = c.take<int32_t>((size_t)cap);
     int32_t* n_rows = c.take<int32_t>(64);
     int32_t* tc_ = c.take<int32_t>((size_t)cap);
@@ -180,7 +180,7 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
   Carver c(workspace);
   FwdWs w;
   carve_fwd(c, T, D, V, dtype, &w);
-  const TcPlan pl = tc_plan_forward(T, V);
+  const TcPlan pl = tc_plan_forward(T, D, V);
   const int64_t cap = ceil_div(T, 256) * 256;
   GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
   if (!mask) {

@@ -6,6 +6,7 @@
 //   a12    dW           dW (+)= dS^T Hs       -> fp32
 #include "tc_gemm.cuh"
 #include <stdio.h>
+#include <stdlib.h>
 
 #ifndef GC_DEFAULT_CG
 #define GC_DEFAULT_CG 2
@@ -265,18 +266,36 @@ static int make_f32_out_tmap(CUtensorMap* m, float* out, int64_t rows, int64_t c
   return r == CUDA_SUCCESS ? GC_OK : GC_ERR_CUDA;
 }
 
+// L2 budget of the forward / recompute schedule.  Measured (profiles/): an H band plus the W tiles
+// in flight stay resident up to ~50 MB, 60 MB and more thrash (DRAM reads x2.5 .. x7) -- about
+// half of the 126 MB, consistent with each die's L2 also holding the lines its SMs fetch from the
+// other die.  The W tiles alive at a time are about k (vocab tiles per item) panels: the band's
+// pairs reach a given W tile spread over a fraction of an item time.
+constexpr int64_t kL2BudgetBytes = 52ll << 20;     // H band + W in flight
+constexpr int64_t kL2StreamBytes = 16ll << 20;     // of which W in flight (caps k)
+constexpr int64_t kL2ResidentBytes = 40ll << 20;   // resident panels of the dW schedule
+
 // ---------------------------------------------------------------------------------------------
-// forward plan: choose the number of N tiles per item so that the items balance over the CTA
-// pairs (wave quantisation, SURVEY.md sec 7.2 hard part 5); prefer longer items on ties.
+// forward plan: vocab tiles per item k.  Among k <= 16 MB / panel (and >= what the cap of 512
+// partial slots per row and 512 MB of partials needs) pick the one whose items balance best over
+// the CTA pairs (wave quantisation, SURVEY.md sec 7.2 hard part 5); longer items win ties.
 // ---------------------------------------------------------------------------------------------
-TcPlan tc_plan_forward(int64_t T, int64_t V) {
+TcPlan tc_plan_forward(int64_t T, int64_t D, int64_t V) {
   const int P = kNumSMs / 2;
   const int64_t Mt = ceil_div(T > 0 ? T : 1, 256);
   const int64_t Nt = ceil_div(V, tc::BN);
+  const int64_t panel = 512 * D;
   TcPlan best{(int)Nt, 1, (int)Nt};
   double best_cost = 1e300;
-  const int64_t kmin = ceil_div(Nt, 160);                // at most 160 partial slots per row
-  for (int64_t k = kmin > 1 ? kmin : 1; k <= 64 && k <= Nt; ++k) {
+  int64_t max_split = (512ll << 20) / (Mt * 256 * (int64_t)sizeof(RowStat));
+  if (max_split > 512) max_split = 512;
+  if (max_split < 1) max_split = 1;
+  int64_t kmin = ceil_div(Nt, max_split);
+  if (kmin < 1) kmin = 1;
+  int64_t kmax = kL2StreamBytes / panel;
+  if (kmax < 2) kmax = 2;
+  if (kmax < kmin) kmax = kmin;
+  for (int64_t k = kmin; k <= kmax && k <= Nt; ++k) {
     const int64_t C = ceil_div(Nt, k);
     // makespan in tiles (upper bound: every item counted as k tiles) + a charge per item flush
     const double cost = (double)(ceil_div(C * Mt, P) * k) * (1.0 + 0.02 / (double)k);
@@ -287,18 +306,20 @@ TcPlan tc_plan_forward(int64_t T, int64_t V) {
     }
   }
   best.n_vtiles = (int)Nt;
+#ifdef GC_EXP_ENV
+  if (const char* v = getenv("GC_PLAN_K")) {
+    best.chunk_vtiles = atoi(v);
+    best.n_split = (int)ceil_div(Nt, best.chunk_vtiles);
+  }
+#endif
   return best;
 }
 
-// L2 budget for the operand panels a schedule keeps resident.  Measured (profiles/): bands up to
-// ~48 MB stay resident, 60 MB and more thrash (DRAM reads x2.5 .. x7) -- about half of the 126 MB,
-// consistent with each die's L2 also holding the lines its SMs fetch from the other die.
-constexpr int64_t kL2ResidentBytes = 40ll << 20;
-
 // M tiles per band of the forward / recompute schedule: the band's A panels (m_band x 256 rows x
 // D bf16) stay in L2 while the N sweep streams W past; W is re-read once per band.
-static int pick_m_band(int64_t D) {
-  int64_t mb = kL2ResidentBytes / (512 * D);
+static int pick_m_band(int64_t D, int k) {
+  const int64_t panel = 512 * D;
+  int64_t mb = (kL2BudgetBytes - (int64_t)k * panel) / panel;
   return (int)(mb < 4 ? 4 : (mb > 64 ? 64 : mb));
 }
 // N tiles per band of the dW schedule: the band's H panels (k_rows x 256 columns bf16).
@@ -307,8 +328,8 @@ static int pick_n_band(int64_t k_rows) {
   return (int)(nb < 1 ? 1 : nb);
 }
 
-size_t tc_fwd_partials_bytes(int64_t T, int64_t V) {
-  const TcPlan pl = tc_plan_forward(T, V);
+size_t tc_fwd_partials_bytes(int64_t T, int64_t D, int64_t V) {
+  const TcPlan pl = tc_plan_forward(T, D, V);
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   return align_up((size_t)pl.n_split * (size_t)cap * sizeof(RowStat), 256);
 }
@@ -359,11 +380,11 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / cg));
-  const TcPlan pl = tc_plan_forward(T, V);
+  const TcPlan pl = tc_plan_forward(T, D, V);
   Sched s = make_sched(T, V, D);
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
-  s.m_band = pick_m_band(D);
+  s.m_band = pick_m_band(D, pl.chunk_vtiles);
   s.counter = counter;
   s.a_hint = ptx::kL2EvictLast;     // the band's H tiles are re-read for every vocab tile
   s.b_hint = ptx::kL2Normal;        // W streams past, shared by the band's pairs a few us apart
@@ -391,10 +412,10 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   // rows up to the next multiple of 256 past the valid count are written as zeros: the dW
   // contraction runs over them (rows_cap is a multiple of 256)
   Sched s = make_sched(ceil_div(h_rows, 256) * 256, V, D);
-  const TcPlan pl = tc_plan_forward(rows_cap, V);
+  const TcPlan pl = tc_plan_forward(rows_cap, D, V);
   s.chunk_ntiles = pl.chunk_vtiles;
   s.c_major = 1;
-  s.m_band = pick_m_band(D);
+  s.m_band = pick_m_band(D, pl.chunk_vtiles);
   s.counter = counter;
   s.a_hint = ptx::kL2EvictLast;
   s.b_hint = ptx::kL2Normal;

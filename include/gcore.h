@@ -175,6 +175,36 @@ int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* re
                        float* out5, float* g,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- the step before the path: dynamic-sampling repack + workload balancing (SURVEY.md sec
+ * 8(f) NEXT-1).  PAPER.md:150 (sec 3.2): prompts whose samples are all right or all wrong are
+ * filtered out; PAPER.md:201 (sec 4.4): "we simply sort data by simulated workload"; PAPER.md:205:
+ * "we first bucket data according to the global batch size, then shuffle the buckets".
+ *   kept samples  = samples of groups with keep[g] != 0 (keep == NULL or group_offsets == NULL: all)
+ *   workload w_i  = w_lin L_i + w_quad L_i^2, L_i = cu_seqlens[i+1] - cu_seqlens[i]  (unsigned 64-bit)
+ *   sorted        = kept samples in ascending w, ties by ascending index
+ *   buckets       = consecutive runs of bucket_size sorted samples (the last may be short)
+ *   shuffle != 0  : buckets reordered by ascending (splitmix64(seed + (b+1) 0x9E3779B97F4A7C15) >> 1, b)
+ * Outputs (device): order [R] (source sample of each destination slot, -1 past n_kept), *n_kept,
+ * cu_out [R+1] (cu_seqlens of the repacked batch; entries past n_kept repeat the total),
+ * src_token [T] (source token of each destination token, first *n_tokens valid), *n_tokens.
+ * Integer work, bit-exact.  Use src_token with gc_gather_rows / gc_gather_1d to repack H, targets,
+ * log-probs.  workspace: gc_balance_workspace_bytes(R).  group_offsets[G] must equal R. */
+size_t gc_balance_workspace_bytes(int32_t R);
+int gc_balance_plan(const int32_t* cu_seqlens, int32_t R, const int32_t* group_offsets,
+                    const uint8_t* keep, int32_t G, uint64_t w_lin, uint64_t w_quad,
+                    int32_t bucket_size, uint64_t seed, int shuffle,
+                    int32_t* order, int32_t* n_kept, int32_t* cu_out, int32_t* src_token,
+                    int32_t* n_tokens, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Y[i,:] = X[rows[i],:] for i < *n_rows (device scalar), rows n_rows .. min(round_up(n_rows, 256),
+ * y_rows) of Y are zero-filled.  X [*, D] (ldX), Y [y_rows, D] dense, of `dtype` (GC_F32 / GC_BF16).
+ * HBM-bound: 2 n_rows D elem bytes. */
+int gc_gather_rows(const void* X, int64_t ldX, int dtype, int64_t D, const int32_t* rows,
+                   const int32_t* n_rows, int64_t y_rows, void* Y, void* cuda_stream);
+/* y[i] = x[rows[i]] for i < *n_rows, 4-byte elements (int32 / float). */
+int gc_gather_1d(const void* x, const int32_t* rows, const int32_t* n_rows, int64_t max_rows,
+                 void* y, void* cuda_stream);
+
 /* Measurement aid (bench.py's roofline figure): between _begin and _end the library brackets
  * every tcgen05 contraction launch with a pair of CUDA events recorded on the call's stream.
  * _end waits for the recorded events, then writes per kernel kind the summed duration in ms and

@@ -4,7 +4,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 ``--impl reference`` legs may import this package.  The product path
 (``paper_2507_22789_b200``) never imports it and shares no code with it.
 
-See ``oracle/gcore_oracle.py`` for the functions and the passages they follow.
+See ``oracle/gcore_oracle.py`` for the functions and the passages they follow;
+``oracle/balance_oracle.py`` holds the oracle of the repack + workload-balancing step.
 """
 from .gcore_oracle import (  # noqa: F401
     AGG_TOKEN_MEAN,
@@ -21,3 +22,4 @@ from .gcore_oracle import (  # noqa: F401
     lm_head_backward_row,
     grpo_forward_backward,
 )
+from . import balance_oracle  # noqa: F401,E402

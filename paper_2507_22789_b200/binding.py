@@ -24,6 +24,7 @@ EXPORTS = [
     "gc_host_staging_bytes", "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
     "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
+    "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
 ]
 
 
@@ -61,11 +62,19 @@ def _load() -> C.CDLL:
                                        f32, vp, vp, vp, sz, vp]
     lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, ci,
                                        ci, vp]
+    u64 = C.c_uint64
+    lib.gc_balance_workspace_bytes.restype = sz
+    lib.gc_balance_workspace_bytes.argtypes = [i32]
+    lib.gc_balance_plan.argtypes = [vp, i32, vp, vp, i32, u64, u64, i32, u64, ci, vp, vp, vp, vp, vp,
+                                    vp, sz, vp]
+    lib.gc_gather_rows.argtypes = [vp, i64, ci, i64, vp, vp, i64, vp, vp]
+    lib.gc_gather_1d.argtypes = [vp, vp, vp, i64, vp, vp]
     lib.gc_kernel_timing_begin.argtypes = []
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
         fn = getattr(lib, name)
-        if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes"):
+        if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes",
+                        "gc_balance_workspace_bytes"):
             fn.restype = ci
     return lib
 
@@ -299,3 +308,42 @@ def gc_kernel_timing_end() -> dict:
     n = (C.c_int32 * len(KERNEL_KINDS))()
     _check(_lib.gc_kernel_timing_end(ms, n))
     return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
+def gc_balance_plan(cu_seqlens, group_offsets=None, keep=None, w_lin=0, w_quad=1, bucket_size=1,
+                    seed=0, shuffle=True, n_tokens_max=None):
+    """Dynamic-sampling repack + workload balancing plan (device tensors in, device tensors out):
+    -> dict(order [R], n_kept [1], cu_out [R+1], src_token [T], n_tokens [1])."""
+    assert cu_seqlens.dtype == torch.int32
+    dev = cu_seqlens.device
+    R = cu_seqlens.numel() - 1
+    G = 0 if group_offsets is None else group_offsets.numel() - 1
+    T = int(n_tokens_max) if n_tokens_max is not None else int(cu_seqlens[-1].item())
+    order = torch.empty(max(R, 1), dtype=torch.int32, device=dev)
+    cu_out = torch.empty(R + 1, dtype=torch.int32, device=dev)
+    src_token = torch.empty(max(T, 1), dtype=torch.int32, device=dev)
+    n_kept = torch.empty(1, dtype=torch.int32, device=dev)
+    n_tokens = torch.empty(1, dtype=torch.int32, device=dev)
+    ws = workspace(int(_lib.gc_balance_workspace_bytes(R)), dev)
+    _check(_lib.gc_balance_plan(_ptr(cu_seqlens), R, _ptr(group_offsets), _ptr(keep), G, int(w_lin),
+                                int(w_quad), int(bucket_size), int(seed) & ((1 << 64) - 1),
+                                int(bool(shuffle)), _ptr(order), _ptr(n_kept), _ptr(cu_out),
+                                _ptr(src_token), _ptr(n_tokens), _ptr(ws), ws.numel(), _stream()))
+    return dict(order=order, n_kept=n_kept, cu_out=cu_out, src_token=src_token, n_tokens=n_tokens)
+
+
+def gc_gather_rows(X, rows, n_rows, y_rows):
+    """Y[i] = X[rows[i]] for i < n_rows (device scalar); -> Y [y_rows, D]."""
+    assert X.dim() == 2 and X.stride(1) == 1
+    Y = torch.empty(y_rows, X.shape[1], dtype=X.dtype, device=X.device)
+    _check(_lib.gc_gather_rows(_ptr(X), X.stride(0), dtype_code(X), X.shape[1], _ptr(rows),
+                               _ptr(n_rows), y_rows, _ptr(Y), _stream()))
+    return Y
+
+
+def gc_gather_1d(x, rows, n_rows, max_rows):
+    """y[i] = x[rows[i]] for i < n_rows; x of a 4-byte dtype."""
+    assert x.element_size() == 4 and x.is_contiguous()
+    y = torch.zeros(max_rows, dtype=x.dtype, device=x.device)
+    _check(_lib.gc_gather_1d(_ptr(x), _ptr(rows), _ptr(n_rows), max_rows, _ptr(y), _stream()))
+    return y

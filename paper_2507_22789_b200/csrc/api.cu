@@ -425,6 +425,52 @@ int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* target
   return GC_OK;
 }
 
+size_t gc_balance_workspace_bytes(int32_t R) { return R < 0 ? 0 : balance_ws_bytes(R); }
+
+int gc_balance_plan(const int32_t* cu_seqlens, int32_t R, const int32_t* group_offsets,
+                    const uint8_t* keep, int32_t G, uint64_t w_lin, uint64_t w_quad,
+                    int32_t bucket_size, uint64_t seed, int shuffle, int32_t* order,
+                    int32_t* n_kept, int32_t* cu_out, int32_t* src_token, int32_t* n_tokens,
+                    void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (R < 0 || G < 0) return GC_ERR_SHAPE;
+  if (bucket_size < 1) return GC_ERR_ARG;
+  if (!n_kept || !n_tokens || !cu_out) return GC_ERR_NULL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (R == 0) {
+    GC_CUDA_TRY(cudaMemsetAsync(n_kept, 0, sizeof(int32_t), st));
+    GC_CUDA_TRY(cudaMemsetAsync(n_tokens, 0, sizeof(int32_t), st));
+    GC_CUDA_TRY(cudaMemsetAsync(cu_out, 0, sizeof(int32_t), st));
+    return GC_OK;
+  }
+  if (!cu_seqlens || !order || !src_token) return GC_ERR_NULL;
+  if (keep && !group_offsets) return GC_ERR_NULL;
+  if (!workspace || workspace_bytes < balance_ws_bytes(R)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  GC_TRY(check_arch());
+  return launch_balance_plan(cu_seqlens, R, group_offsets, keep, G, w_lin, w_quad, bucket_size, seed,
+                             shuffle, order, n_kept, cu_out, src_token, n_tokens, workspace, st);
+}
+
+int gc_gather_rows(const void* X, int64_t ldX, int dtype, int64_t D, const int32_t* rows,
+                   const int32_t* n_rows, int64_t y_rows, void* Y, void* cuda_stream) {
+  if (dtype != GC_F32 && dtype != GC_BF16) return GC_ERR_DTYPE;
+  if (D <= 0 || ldX < D || y_rows < 0) return GC_ERR_SHAPE;
+  if (y_rows == 0) return GC_OK;
+  if (!X || !rows || !n_rows || !Y) return GC_ERR_NULL;
+  if (!aligned16(X) || !aligned16(Y)) return GC_ERR_ALIGN;
+  return launch_gather_rows(X, ldX, elem_bytes(dtype), D, y_rows, rows, n_rows, Y, y_rows,
+                            static_cast<cudaStream_t>(cuda_stream));
+}
+
+int gc_gather_1d(const void* x, const int32_t* rows, const int32_t* n_rows, int64_t max_rows,
+                 void* y, void* cuda_stream) {
+  if (max_rows < 0) return GC_ERR_SHAPE;
+  if (max_rows == 0) return GC_OK;
+  if (!x || !rows || !n_rows || !y) return GC_ERR_NULL;
+  return launch_gather_i32(static_cast<const int32_t*>(x), rows, n_rows, max_rows,
+                           static_cast<int32_t*>(y), static_cast<cudaStream_t>(cuda_stream));
+}
+
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
                        int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
                        int accumulate, int cta_group, int dynamic_schedule, int dual_n,

@@ -85,6 +85,14 @@ int launch_zero_rows_unscored(const int32_t* targets, const uint8_t* mask, int64
 int launch_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
                             unsigned long long* n_bad_dev, cudaStream_t st);
 
+// balance.cu (NEXT-1: dynamic-sampling repack + workload balancing)
+size_t balance_ws_bytes(int32_t R);
+int launch_balance_plan(const int32_t* cu, int32_t R, const int32_t* group_offsets,
+                        const uint8_t* keep, int32_t G, uint64_t w_lin, uint64_t w_quad,
+                        int32_t bucket_size, uint64_t seed, int shuffle, int32_t* order,
+                        int32_t* n_kept, int32_t* cu_out, int32_t* src_token, int32_t* n_tokens,
+                        void* ws, cudaStream_t st);
+
 // simt_head.cu
 int simt_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, bool bf16,
                   const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,

@@ -346,21 +346,24 @@ def hbm_kernels(B, device, peaks):
         return e0.elapsed_time(e1) / n
     out = {"peak_gbs": peaks["hbm"], "stand_in": True}
     T = 1 << 26
-    R = T // 16
     g = torch.Generator(device=device).manual_seed(0)
     logp = -3.0 * torch.rand(T, device=device, generator=g)
     old = logp + 0.05 * torch.randn(T, device=device, generator=g)
     ref = logp + 0.1 * torch.randn(T, device=device, generator=g)
     y = torch.randint(0, 1000, (T,), device=device, dtype=torch.int32, generator=g)
-    mask = (torch.rand(T, device=device, generator=g) < 0.75).to(torch.uint8)
-    cu = torch.arange(0, T + 1, 16, device=device, dtype=torch.int32)
-    adv = torch.randn(R, device=device, generator=g)
-    ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv))
-    # reads logp, old, ref, target (4 B each) + mask (1 B), writes g (4 B); the integer count pass
-    # that fixes the normaliser re-reads target + mask (5 B)
-    gbs = 26.0 * T / ms / 1e6
-    out["token_loss_and_grad"] = {"tokens": T, "responses": R, "bytes_per_token": 26, "ms": ms,
-                                  "gbs": gbs, "frac": gbs / peaks["hbm"]}
+    # cfg2's layout scaled up: samples of 1024 tokens = 256 prompt (mask 0) + 768 response tokens;
+    # and a stress layout of 16-token responses (a response boundary in every other thread)
+    mask = ((torch.arange(T, device=device) % 1024) >= 256).to(torch.uint8)
+    for name, seqlen in (("token_loss_and_grad", 1024), ("token_loss_and_grad_16_token_responses", 16)):
+        R = T // seqlen
+        cu = torch.arange(0, T + 1, seqlen, device=device, dtype=torch.int32)
+        adv = torch.randn(R, device=device, generator=g)
+        ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv))
+        # reads logp, old, ref, target (4 B each) + mask (1 B), writes g (4 B); the integer count
+        # pass that fixes the normaliser re-reads target + mask (5 B)
+        gbs = 26.0 * T / ms / 1e6
+        out[name] = {"tokens": T, "responses": R, "bytes_per_token": 26, "ms": ms, "gbs": gbs,
+                     "frac": gbs / peaks["hbm"]}
     del logp, old, ref, y, mask, cu, adv
     T2, D = 1 << 19, 4096
     H = torch.randn(T2, D, device=device, generator=g).to(torch.bfloat16)

@@ -188,8 +188,8 @@ k_loss_counts(const int32_t* __restrict__ targets, const uint8_t* __restrict__ m
               int32_t* __restrict__ resp_cnt, LossCounters* __restrict__ cnt) {
   __shared__ int32_t s_cu[kCuSmem];
   CuSlice cs;
-  if (per_response) cs = load_cu_slice(cu, tile_r, s_cu);
   const int64_t tile0 = (int64_t)blockIdx.x * kLossTile;
+  if (per_response) cs = load_cu_slice(cu, tile_r, s_cu);
   unsigned int n_sc = 0, n_kept = 0;
 #pragma unroll
   for (int round = 0; round < 2; ++round) {
@@ -229,6 +229,27 @@ k_loss_counts(const int32_t* __restrict__ targets, const uint8_t* __restrict__ m
     for (int w = 0; w < kLossThreads / 32; ++w) { a += sm[0][w]; k += sm[1][w]; }
     if (a) atomicAdd(&cnt->n_scored, a);
     if (k) atomicAdd(&cnt->n_kept, k);
+  }
+}
+
+// seq-mean with long responses (>= 128 tokens on average): one warp per response, coalesced; the
+// token-parallel kernel above would put ~L/8 atomics on one counter.
+__global__ void k_loss_counts_seq(const int32_t* __restrict__ targets,
+                                  const uint8_t* __restrict__ mask,
+                                  const int32_t* __restrict__ cu, int32_t R,
+                                  int32_t* __restrict__ resp_cnt, LossCounters* __restrict__ cnt) {
+  const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (r >= R) return;
+  unsigned int c = 0;
+  for (int64_t t = cu[r] + lane; t < cu[r + 1]; t += 32) c += is_scored(targets, mask, t) ? 1u : 0u;
+  c = warp_sum(c);
+  if (lane == 0) {
+    resp_cnt[r] = (int32_t)c;
+    if (c) {
+      atomicAdd(&cnt->n_scored, (unsigned long long)c);
+      atomicAdd(&cnt->n_kept, 1u);
+    }
   }
 }
 
@@ -487,8 +508,12 @@ int launch_token_loss(const float* logp, const float* old_logp, const float* ref
     GC_CUDA_TRY(cudaMemsetAsync(resp_cnt, 0, sizeof(int32_t) * (size_t)(R > 0 ? R : 1), st));
   k_loss_tile_ranges<<<(unsigned)ceil_div(blocks + 1, 256), 256, 0, st>>>(cu_seqlens, R, T, blocks,
                                                                           tile_r);
-  k_loss_counts<<<(unsigned)blocks, kLossThreads, 0, st>>>(targets, mask, T, cu_seqlens, R, tile_r,
-                                                          per_response, resp_cnt, cnt);
+  if (per_response && T >= (int64_t)R * 128)
+    k_loss_counts_seq<<<(unsigned)ceil_div((int64_t)R * 32, 256), 256, 0, st>>>(
+        targets, mask, cu_seqlens, R, resp_cnt, cnt);
+  else
+    k_loss_counts<<<(unsigned)blocks, kLossThreads, 0, st>>>(targets, mask, T, cu_seqlens, R, tile_r,
+                                                            per_response, resp_cnt, cnt);
   GC_CUDA_TRY(cudaGetLastError());
   k_token_loss<<<(unsigned)blocks, kLossThreads, 0, st>>>(
       logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, resp_cnt, tile_r, clip_lo, clip_hi, beta, agg, grad_loss, cnt, partials, out5, g);

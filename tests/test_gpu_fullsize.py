@@ -116,6 +116,16 @@ def check_full(B, b, n_random=64, seed=0):
     expect = -(A_tok * scored_full).sum() / max(scored_full.sum(), 1)
     assert abs(out5[0].item() - expect) <= 1e-6 + 1e-5 * abs(expect)
     assert out5[4].item() == scored_full.sum()
+    # reruns are bit-identical at full size too: which CTA pair computes a tile (dynamic schedule)
+    # and the L2-side dW accumulation (one TMA reduce-add per element per chunk, stream-ordered)
+    # must not enter the result
+    dH1, dW1 = dH.clone(), dW.clone()
+    f2 = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
+                            w.clip_hi, w.beta)
+    B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f2["logp"], f2["lse"],
+                       w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW)
+    assert torch.equal(f2["logp"], logp) and torch.equal(f2["entropy"], ent)
+    assert torch.equal(b.dH, dH1) and torch.equal(b.dW, dW1)
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 4])

@@ -175,6 +175,23 @@ int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* re
                        float* out5, float* g,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- verdict-token scoring for a generative reward model.
+ * PAPER.md:144 (sec 3.2): "Generative rewarding using standard next-token prediction, represents
+ * solution correctness using the LLM's probability distribution over tokens ... the verification
+ * decision is just another token".  Only the scoring is in scope (generation and regex matching,
+ * PAPER.md:146, need an inference engine and trained weights): at each given position, the
+ * log-probability of each of K candidate verdict tokens, in one pass of the forward contraction.
+ *   logp[t,k] = z[t, targets[t,k]] - lse[t]      (0 where targets[t,k] < 0 or >= V)
+ * H [T,D] holds the hidden states at the verdict positions (gather them with gc_gather_rows);
+ * targets [T,K] int32 row-major, 1 <= K <= 8; logp [T,K]; entropy, lse [T] nullable.  GC_BF16 only.
+ * exp(logp[t,:]) are the candidates' probabilities; a reward such as P(yes) / (P(yes) + P(no)) is
+ * the caller's arithmetic.  workspace: gc_multi_workspace_bytes(T, D, V, K). */
+size_t gc_multi_workspace_bytes(int64_t T, int64_t D, int64_t V, int32_t K);
+int gc_token_logprobs_multi(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                            const int32_t* targets, int32_t K, int64_t T, int64_t D, int64_t V,
+                            float temperature, float* logp, float* entropy, float* lse,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- the step before the path: dynamic-sampling repack + workload balancing (SURVEY.md sec
  * 8(f) NEXT-1).  PAPER.md:150 (sec 3.2): prompts whose samples are all right or all wrong are
  * filtered out; PAPER.md:201 (sec 4.4): "we simply sort data by simulated workload"; PAPER.md:205:

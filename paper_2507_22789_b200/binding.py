@@ -25,6 +25,7 @@ EXPORTS = [
     "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
+    "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
 ]
 
 
@@ -69,12 +70,16 @@ def _load() -> C.CDLL:
                                     vp, sz, vp]
     lib.gc_gather_rows.argtypes = [vp, i64, ci, i64, vp, vp, i64, vp, vp]
     lib.gc_gather_1d.argtypes = [vp, vp, vp, i64, vp, vp]
+    lib.gc_multi_workspace_bytes.restype = sz
+    lib.gc_multi_workspace_bytes.argtypes = [i64, i64, i64, i32]
+    lib.gc_token_logprobs_multi.argtypes = [vp, i64, vp, i64, ci, vp, i32, i64, i64, i64, f32, vp, vp,
+                                            vp, vp, sz, vp]
     lib.gc_kernel_timing_begin.argtypes = []
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes",
-                        "gc_balance_workspace_bytes"):
+                        "gc_balance_workspace_bytes", "gc_multi_workspace_bytes"):
             fn.restype = ci
     return lib
 
@@ -347,3 +352,21 @@ def gc_gather_1d(x, rows, n_rows, max_rows):
     y = torch.zeros(max_rows, dtype=x.dtype, device=x.device)
     _check(_lib.gc_gather_1d(_ptr(x), _ptr(rows), _ptr(n_rows), max_rows, _ptr(y), _stream()))
     return y
+
+
+def gc_token_logprobs_multi(H, W, targets, temperature=1.0):
+    """Verdict-token scoring: targets [T, K] int32 -> (logp [T, K], entropy [T], lse [T])."""
+    assert H.dim() == 2 and W.dim() == 2 and targets.dim() == 2 and targets.dtype == torch.int32
+    T, D = H.shape
+    V, K = W.shape[0], targets.shape[1]
+    assert targets.shape[0] == T and targets.is_contiguous()
+    dev = H.device
+    logp = torch.empty(T, K, dtype=torch.float32, device=dev)
+    ent = torch.empty(T, dtype=torch.float32, device=dev)
+    lse = torch.empty(T, dtype=torch.float32, device=dev)
+    ws = workspace(int(_lib.gc_multi_workspace_bytes(T, D, V, K)), dev)
+    _check(_lib.gc_token_logprobs_multi(_ptr(H), H.stride(0) if T > 0 else D, _ptr(W), W.stride(0),
+                                        dtype_code(H), _ptr(targets), K, T, D, V, float(temperature),
+                                        _ptr(logp), _ptr(ent), _ptr(lse), _ptr(ws), ws.numel(),
+                                        _stream()))
+    return logp, ent, lse

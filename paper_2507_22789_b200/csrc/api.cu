@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/gcore.h: argument validation, workspace carving, and the
 // host-side plan (row compaction, chunk loop of the backward).  No allocation, no sync.
 #include "common.cuh"
+#include <math.h>
 
 using namespace gc;
 
@@ -196,6 +197,39 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
   GC_TRY(tc_forward_stats(w.Hs, D, W, ldW, T, D, V, temperature, w.targets_c, w.n_rows, w.partials,
                           w.counters, st));
   return launch_combine(w.partials, pl.n_split, cap, w.rows, w.n_rows, T, logp, entropy, lse, st);
+}
+
+size_t gc_multi_workspace_bytes(int64_t T, int64_t D, int64_t V, int32_t K) {
+  if (T < 0 || D <= 0 || V <= 0 || K < 1 || K > 8) return 0;
+  const size_t cap = (size_t)ceil_div(T > 0 ? T : 1, 256) * 256;
+  return align_up(sizeof(uint32_t) * kTcCounters, 256) + tc_fwd_partials_bytes(T, D, V) +
+         align_up(cap * (size_t)K * sizeof(float), 256) + 256;
+}
+
+int gc_token_logprobs_multi(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                            const int32_t* targets, int32_t K, int64_t T, int64_t D, int64_t V,
+                            float temperature, float* logp, float* entropy, float* lse,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (dtype != GC_BF16) return GC_ERR_DTYPE;
+  if (K < 1 || K > 8) return GC_ERR_ARG;
+  GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
+  if (T > 0 && !logp) return GC_ERR_NULL;
+  if (T == 0) return GC_OK;
+  if (!workspace || workspace_bytes < gc_multi_workspace_bytes(T, D, V, K)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  GC_TRY(check_arch());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t cap = (size_t)ceil_div(T, 256) * 256;
+  Carver c(workspace);
+  uint32_t* counters = c.take<uint32_t>(kTcCounters);
+  RowStat* partials = c.take<RowStat>(tc_fwd_partials_bytes(T, D, V) / sizeof(RowStat));
+  float* ay = c.take<float>(cap * (size_t)K);
+  GC_CUDA_TRY(cudaMemsetAsync(counters, 0, sizeof(uint32_t) * kTcCounters, st));
+  GC_TRY(launch_fill_f32(ay, -INFINITY, (int64_t)T * K, st));     // "target not met"
+  GC_TRY(tc_forward_stats_multi(H, ldH, W, ldW, T, D, V, temperature, targets, K, ay, partials,
+                                counters, st));
+  const TcPlan pl = tc_plan_forward(T, D, V);
+  return launch_combine_multi(partials, pl.n_split, (int64_t)cap, ay, K, T, logp, entropy, lse, st);
 }
 
 size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype) {

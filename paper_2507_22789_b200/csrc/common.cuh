@@ -68,6 +68,10 @@ int launch_token_loss(const float* logp, const float* old_logp, const float* ref
 int launch_combine(const RowStat* partials, int n_split, int64_t split_stride,
                    const int32_t* rows, const int32_t* n_rows_dev, int64_t n_rows_max,
                    float* logp, float* entropy, float* lse, cudaStream_t st);
+int launch_combine_multi(const RowStat* partials, int n_split, int64_t split_stride,
+                         const float* ay, int K, int64_t T, float* logp, float* entropy,
+                         float* lse, cudaStream_t st);
+int launch_fill_f32(float* p, float v, int64_t n, cudaStream_t st);
 int launch_zero_unscored(const int32_t* targets, const uint8_t* mask, int64_t T,
                          float* logp, float* entropy, float* lse, cudaStream_t st);
 size_t compact_ws_bytes(int64_t T);
@@ -116,6 +120,9 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
                      int64_t D, int64_t V, float tau, const int32_t* targets_c,
                      const int32_t* n_rows_dev, RowStat* partials, uint32_t* counter,
                      cudaStream_t st);
+int tc_forward_stats_multi(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
+                           int64_t D, int64_t V, float tau, const int32_t* targets, int K,
+                           float* ay, RowStat* partials, uint32_t* counter, cudaStream_t st);
 // Backward chunk kernels.  rows_cap = rows of the dS chunk buffer (multiple of 256); the valid
 // rows of the chunk are clamp(*n_rows_dev - row0, 0, rows_cap), or n_static if n_rows_dev == NULL.
 int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,

@@ -562,6 +562,56 @@ int launch_combine(const RowStat* partials, int n_split, int64_t split_stride,
   return GC_OK;
 }
 
+__global__ void k_fill_f32(float* __restrict__ p, float v, int64_t n) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (int64_t)gridDim.x * blockDim.x)
+    p[i] = v;
+}
+int launch_fill_f32(float* p, float v, int64_t n, cudaStream_t st) {
+  if (n <= 0) return GC_OK;
+  int64_t blocks = ceil_div(n, 256);
+  if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
+  k_fill_f32<<<(unsigned)blocks, 256, 0, st>>>(p, v, n);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
+// K targets per row (verdict-token scoring): logp[t,k] = ln2 ay[t,k] - lse[t], 0 where the target
+// was absent (id < 0 or >= V: ay still holds its -inf fill).
+__global__ void k_combine_multi(const RowStat* __restrict__ partials, int n_split,
+                                int64_t split_stride, const float* __restrict__ ay, int K, int64_t T,
+                                float* __restrict__ logp, float* __restrict__ entropy,
+                                float* __restrict__ lse) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= T) return;
+  float M = -INFINITY;
+  for (int c = 0; c < n_split; ++c) M = fmaxf(M, partials[(int64_t)c * split_stride + i].m);
+  float S = 0.f, U = 0.f;
+  for (int c = 0; c < n_split; ++c) {
+    const RowStat p = partials[(int64_t)c * split_stride + i];
+    const float sc = exp2f(p.m - M);
+    S += p.s * sc;
+    U += (p.u + p.m * p.s) * sc;
+  }
+  const float l = kLn2 * (M + log2f(S));
+  for (int k = 0; k < K; ++k) {
+    const float a = ay[i * K + k];
+    logp[i * K + k] = a > -INFINITY ? kLn2 * a - l : 0.f;
+  }
+  if (entropy) entropy[i] = l - kLn2 * (U / S);
+  if (lse) lse[i] = l;
+}
+
+int launch_combine_multi(const RowStat* partials, int n_split, int64_t split_stride,
+                         const float* ay, int K, int64_t T, float* logp, float* entropy,
+                         float* lse, cudaStream_t st) {
+  if (T <= 0) return GC_OK;
+  k_combine_multi<<<(unsigned)ceil_div(T, 128), 128, 0, st>>>(partials, n_split, split_stride, ay, K,
+                                                              T, logp, entropy, lse);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
 // =============================================================================================
 // a1: row selection.  rows[] = ascending indices of scored tokens (bit-exact integer work):
 // per-block counts -> single-block exclusive scan -> per-block ordered scatter.

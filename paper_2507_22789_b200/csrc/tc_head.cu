@@ -85,6 +85,88 @@ struct EpiStats {
   static __device__ __forceinline__ void finish(State&, const Params&) {}
 };
 
+// ---------------------------------------------------------------------------------------------
+// Epilogue of the verdict-token scoring ("Generative
+// rewarding ... represents solution correctness using the LLM's probability distribution over
+// tokens"): the same online statistics as EpiStats, with K target ids per row.  Every target logit
+// lives in exactly one vocab tile, so the thread that meets it stores it straight to ay[row, k]
+// (one writer in the whole grid; the buffer is pre-filled with -inf) instead of carrying it in the
+// split-V partials.
+// ---------------------------------------------------------------------------------------------
+constexpr int kMaxTargets = 8;
+struct EpiStatsMulti {
+  static constexpr int kWarpSmem = 0;
+  struct Params {
+    const int32_t* targets;   // [rows, K]
+    float* ay;                // [rows, K], log2-scaled target logits
+    RowStat* partials;
+    int64_t split_stride;
+    int64_t V;
+    float c;
+    int K;
+  };
+  struct State { float m, s0, s1, u0, u1; int32_t y[kMaxTargets]; int64_t row; };
+  static __device__ __forceinline__ void setup(State&, const Params&, uint32_t) {}
+  static __device__ __forceinline__ void item_begin(State& st, const Params& p, int64_t row,
+                                                    bool valid, int64_t) {
+#pragma unroll
+    for (int k = 0; k < kMaxTargets; ++k)
+      st.y[k] = (valid && k < p.K) ? p.targets[row * p.K + k] : -1;
+    st.row = row;
+    st.m = -1e30f;
+    st.s0 = st.s1 = st.u0 = st.u1 = 0.f;
+  }
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t, bool,
+                                               int64_t col0, const float (&x)[32]) {
+    if (col0 >= p.V) return;
+    const bool full = col0 + 32 <= p.V;
+    const int nvalid = full ? 32 : (int)(p.V - col0);
+    float cm = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) cm = (full || j < nvalid) ? fmaxf(cm, x[j]) : cm;
+    const float mnew = fmaxf(st.m, cm * p.c);
+    const float dm = st.m - mnew;
+    const float sc = ptx::ex2(dm);
+    st.u0 = (st.u0 + dm * st.s0) * sc;
+    st.u1 = (st.u1 + dm * st.s1) * sc;
+    st.s0 *= sc;
+    st.s1 *= sc;
+    st.m = mnew;
+#pragma unroll
+    for (int j = 0; j < 32; j += 2) {
+      const float t0 = fmaf(x[j], p.c, -mnew), t1 = fmaf(x[j + 1], p.c, -mnew);
+      float e0 = ptx::ex2(t0), e1 = ptx::ex2(t1);
+      if (!full) { e0 = j < nvalid ? e0 : 0.f; e1 = j + 1 < nvalid ? e1 : 0.f; }
+      st.s0 += e0;
+      st.s1 += e1;
+      st.u0 = fmaf(e0, t0, st.u0);
+      st.u1 = fmaf(e1, t1, st.u1);
+    }
+#pragma unroll
+    for (int k = 0; k < kMaxTargets; ++k) {
+      const uint32_t rel = (uint32_t)((int64_t)st.y[k] - col0);
+      if (st.y[k] >= 0 && rel < 32u && (int64_t)st.y[k] < p.V) {
+        float v = 0.f;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v = (rel == (uint32_t)j) ? x[j] : v;
+        p.ay[st.row * p.K + k] = v * p.c;
+      }
+    }
+  }
+  static __device__ __forceinline__ void item_end(State& st, const Params& p, int64_t row,
+                                                  bool valid, int64_t c) {
+    if (!valid) return;
+    RowStat o;
+    o.m = st.m;
+    o.s = st.s0 + st.s1;
+    o.u = st.u0 + st.u1;
+    o.ay = -INFINITY;
+    p.partials[c * p.split_stride + row] = o;
+  }
+  static __device__ __forceinline__ void finish(State&, const Params&) {}
+};
+
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&v);
@@ -398,6 +480,33 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   GC_EXP_OVERRIDE(s, "FWD");
   KernelTimer kt(GC_KERNEL_FWD_STATS, st);
   return launch_cg<EpiStats, false, false>(cg, ta, tb, s, ep, st);
+}
+
+int tc_forward_stats_multi(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
+                           int64_t D, int64_t V, float tau, const int32_t* targets, int K,
+                           float* ay, RowStat* partials, uint32_t* counter, cudaStream_t st) {
+  if (K < 1 || K > kMaxTargets) return GC_ERR_ARG;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / 2));
+  const TcPlan pl = tc_plan_forward(T, D, V);
+  Sched s = make_sched(T, V, D);
+  s.chunk_ntiles = pl.chunk_vtiles;
+  s.c_major = 1;
+  s.m_band = pick_m_band(D, pl.chunk_vtiles);
+  s.counter = counter;
+  s.a_hint = ptx::kL2EvictLast;
+  s.b_hint = ptx::kL2Normal;
+  EpiStatsMulti::Params ep;
+  ep.targets = targets;
+  ep.ay = ay;
+  ep.partials = partials;
+  ep.split_stride = ceil_div(T, 256) * 256;
+  ep.V = V;
+  ep.c = kLog2e / tau;
+  ep.K = K;
+  KernelTimer kt(GC_KERNEL_FWD_STATS, st);
+  return tc::launch_tc_gemm<2, false, false, EpiStatsMulti>(ta, tb, s, ep, st);
 }
 
 int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,

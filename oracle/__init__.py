@@ -5,7 +5,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 (``paper_2507_22789_b200``) never imports it and shares no code with it.
 
 See ``oracle/gcore_oracle.py`` for the functions and the passages they follow;
-``oracle/balance_oracle.py`` holds the oracle of the repack + workload-balancing step.
+``oracle/balance_oracle.py`` holds the oracle of the repack + workload-balancing step,
+``oracle/critic_oracle.py`` the oracle of the PPO critic path (value head, GAE, value loss).
 """
 from .gcore_oracle import (  # noqa: F401
     AGG_TOKEN_MEAN,
@@ -23,3 +24,4 @@ from .gcore_oracle import (  # noqa: F401
     grpo_forward_backward,
 )
 from . import balance_oracle  # noqa: F401,E402
+from . import critic_oracle  # noqa: F401,E402

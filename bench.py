@@ -374,6 +374,15 @@ def hbm_kernels(B, device, peaks):
     gbs = (2.0 * n * D * 2 + 9.0 * T2) / ms / 1e6
     out["compact_and_gather_rows"] = {"rows": T2, "scored_rows": n, "hidden": D, "ms": ms,
                                       "gbs": gbs, "frac": gbs / peaks["hbm"]}
+    # PPO critic (NEXT-2): value head forward (reads H once) and backward (reads H, writes dH)
+    wv = (torch.randn(D, device=device, generator=g) / 64).to(torch.bfloat16)
+    gt = torch.randn(T2, device=device, generator=g)
+    ms = timeit(lambda: B.gc_value_head_fwd(H, wv))
+    gbs = (2.0 * T2 * D + 4.0 * T2) / ms / 1e6
+    out["value_head_fwd"] = {"rows": T2, "hidden": D, "ms": ms, "gbs": gbs, "frac": gbs / peaks["hbm"]}
+    ms = timeit(lambda: B.gc_value_head_bwd(H, wv, gt))
+    gbs = (4.0 * T2 * D + 4.0 * T2) / ms / 1e6
+    out["value_head_bwd"] = {"rows": T2, "hidden": D, "ms": ms, "gbs": gbs, "frac": gbs / peaks["hbm"]}
     return out
 
 

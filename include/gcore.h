@@ -175,6 +175,35 @@ int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* re
                        float* out5, float* g,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- the PPO variant of stages 3-4: critic values, GAE, clipped value loss (SURVEY.md sec 8(f)
+ * NEXT-2).  PAPER.md:96 (sec 2.2): in PPO "the critic computes values"; stage 3
+ * computes them, stage 4 trains actor and critic.  The paper prints no formula; the arithmetic is
+ * PPO [18] as read in DESIGN.md sec 11:
+ *   v_t      = sum_d H[t,d] w[d] + bias                                      (gc_value_head_fwd)
+ *   delta_t  = r_t + gamma v_next(t) - v_t;  A_t = delta_t + gamma lambda A_next(t);
+ *   return_t = A_t + v_t, over the scored tokens of each response in order (a masked token is not
+ *              part of the trajectory; v_next = 0 after the last); 0 at unscored tokens   (gc_gae)
+ *   v_clip   = clip(v, v_old - clip_v, v_old + clip_v);  l_t = 0.5 max((v-ret)^2, (v_clip-ret)^2)
+ *   loss     = sum m l / max(sum m, 1);  out3 = {loss, clip_frac, n_scored};
+ *   g_t      = grad_loss d loss / d v_t                                       (gc_value_loss)
+ *   dH[t,:]  = g_t w;  dw = sum_t g_t H[t,:];  dbias = sum_t g_t              (gc_value_head_bwd)
+ * The policy side of PPO is gc_grpo_token_loss with one "response" per token (cu_seqlens = 0..T)
+ * and adv = the per-token GAE advantages.  H [T,D] and w [D] of `dtype` (GC_F32 / GC_BF16),
+ * D % 8 == 0, 16-byte aligned rows; values, rewards, adv, returns, g [T] f32; mask [T] uint8
+ * nullable; dH in H's dtype; dw [D] f32, dbias device [1] f32 nullable.  Deterministic. */
+int gc_value_head_fwd(const void* H, int64_t ldH, int dtype, const void* w, float bias, int64_t T,
+                      int64_t D, float* values, void* cuda_stream);
+int gc_gae(const float* rewards, const float* values, const uint8_t* mask,
+           const int32_t* cu_seqlens, int32_t R, int64_t T, float gamma, float lambda,
+           float* adv, float* returns, void* cuda_stream);
+size_t gc_critic_workspace_bytes(int64_t T, int64_t D);
+int gc_value_loss(const float* values, const float* old_values, const float* returns,
+                  const uint8_t* mask, int64_t T, float clip_v, float grad_loss, float* out3,
+                  float* g, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int gc_value_head_bwd(const void* H, int64_t ldH, int dtype, const void* w, const float* g,
+                      int64_t T, int64_t D, void* dH, int64_t lddH, float* dw, float* dbias,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- verdict-token scoring for a generative reward model.
  * PAPER.md:144 (sec 3.2): "Generative rewarding using standard next-token prediction, represents
  * solution correctness using the LLM's probability distribution over tokens ... the verification

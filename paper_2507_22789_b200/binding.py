@@ -26,6 +26,7 @@ EXPORTS = [
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
     "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
+    "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
 
@@ -74,12 +75,19 @@ def _load() -> C.CDLL:
     lib.gc_multi_workspace_bytes.argtypes = [i64, i64, i64, i32]
     lib.gc_token_logprobs_multi.argtypes = [vp, i64, vp, i64, ci, vp, i32, i64, i64, i64, f32, vp, vp,
                                             vp, vp, sz, vp]
+    lib.gc_value_head_fwd.argtypes = [vp, i64, ci, vp, f32, i64, i64, vp, vp]
+    lib.gc_gae.argtypes = [vp, vp, vp, vp, i32, i64, f32, f32, vp, vp, vp]
+    lib.gc_critic_workspace_bytes.restype = sz
+    lib.gc_critic_workspace_bytes.argtypes = [i64, i64]
+    lib.gc_value_loss.argtypes = [vp, vp, vp, vp, i64, f32, f32, vp, vp, vp, sz, vp]
+    lib.gc_value_head_bwd.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, i64, vp, vp, vp, sz, vp]
     lib.gc_kernel_timing_begin.argtypes = []
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes",
-                        "gc_balance_workspace_bytes", "gc_multi_workspace_bytes"):
+                        "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
+                        "gc_critic_workspace_bytes"):
             fn.restype = ci
     return lib
 
@@ -370,3 +378,51 @@ def gc_token_logprobs_multi(H, W, targets, temperature=1.0):
                                         _ptr(logp), _ptr(ent), _ptr(lse), _ptr(ws), ws.numel(),
                                         _stream()))
     return logp, ent, lse
+
+
+def gc_value_head_fwd(H, w, bias=0.0):
+    """v[t] = H[t,:] . w + bias -> float32 [T]."""
+    T, D = H.shape
+    assert w.numel() == D and w.dtype == H.dtype and H.stride(1) == 1
+    v = torch.empty(T, dtype=torch.float32, device=H.device)
+    _check(_lib.gc_value_head_fwd(_ptr(H), H.stride(0) if T > 0 else D, dtype_code(H), _ptr(w),
+                                  float(bias), T, D, _ptr(v), _stream()))
+    return v
+
+
+def gc_gae(rewards, values, mask, cu_seqlens, gamma=1.0, lam=0.95):
+    """-> (adv [T], returns [T])."""
+    T = rewards.numel()
+    adv = torch.zeros(T, dtype=torch.float32, device=rewards.device)
+    ret = torch.zeros(T, dtype=torch.float32, device=rewards.device)
+    _check(_lib.gc_gae(_ptr(rewards), _ptr(values), _ptr(mask), _ptr(cu_seqlens),
+                       cu_seqlens.numel() - 1, T, float(gamma), float(lam), _ptr(adv), _ptr(ret),
+                       _stream()))
+    return adv, ret
+
+
+def gc_value_loss(values, old_values, returns, mask=None, clip_v=0.2, grad_loss=1.0, want_grad=True):
+    """-> (out3 = [loss, clip_frac, n_scored] device tensor, g [T] or None)."""
+    T = values.numel()
+    dev = values.device
+    out3 = torch.empty(3, dtype=torch.float32, device=dev)
+    g = torch.empty(T, dtype=torch.float32, device=dev) if want_grad else None
+    ws = workspace(int(_lib.gc_critic_workspace_bytes(T, 8)), dev)
+    _check(_lib.gc_value_loss(_ptr(values), _ptr(old_values), _ptr(returns), _ptr(mask), T,
+                              float(clip_v), float(grad_loss), _ptr(out3), _ptr(g), _ptr(ws),
+                              ws.numel(), _stream()))
+    return out3, g
+
+
+def gc_value_head_bwd(H, w, g):
+    """-> (dH [T,D] in H's dtype, dw [D] float32, dbias [1] float32)."""
+    T, D = H.shape
+    dev = H.device
+    dH = torch.empty(T, D, dtype=H.dtype, device=dev)
+    dw = torch.empty(D, dtype=torch.float32, device=dev)
+    db = torch.empty(1, dtype=torch.float32, device=dev)
+    ws = workspace(int(_lib.gc_critic_workspace_bytes(T, D)), dev)
+    _check(_lib.gc_value_head_bwd(_ptr(H), H.stride(0) if T > 0 else D, dtype_code(H), _ptr(w),
+                                  _ptr(g), T, D, _ptr(dH), D, _ptr(dw), _ptr(db), _ptr(ws),
+                                  ws.numel(), _stream()))
+    return dH, dw, db

@@ -459,6 +459,77 @@ int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* target
   return GC_OK;
 }
 
+static int check_value_args(const void* H, int64_t ldH, int dtype, const void* w, int64_t T,
+                            int64_t D) {
+  if (dtype != GC_F32 && dtype != GC_BF16) return GC_ERR_DTYPE;
+  if (T < 0 || D <= 0 || D % 8 != 0 || ldH < D || T >= (1ll << 31)) return GC_ERR_SHAPE;
+  if (!w || (T > 0 && !H)) return GC_ERR_NULL;
+  if (!aligned16(H) || !aligned16(w) || (ldH * elem_bytes(dtype)) % 16 != 0) return GC_ERR_ALIGN;
+  return GC_OK;
+}
+
+int gc_value_head_fwd(const void* H, int64_t ldH, int dtype, const void* w, float bias, int64_t T,
+                      int64_t D, float* values, void* cuda_stream) {
+  GC_TRY(check_value_args(H, ldH, dtype, w, T, D));
+  if (T == 0) return GC_OK;
+  if (!values) return GC_ERR_NULL;
+  return launch_value_fwd(H, ldH, dtype == GC_BF16, w, bias, T, D, values,
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+int gc_gae(const float* rewards, const float* values, const uint8_t* mask,
+           const int32_t* cu_seqlens, int32_t R, int64_t T, float gamma, float lambda, float* adv,
+           float* returns, void* cuda_stream) {
+  if (R < 0 || T < 0) return GC_ERR_SHAPE;
+  if (!(gamma >= 0.f) || !(lambda >= 0.f)) return GC_ERR_ARG;
+  if (R == 0 || T == 0) return GC_OK;
+  if (!rewards || !values || !cu_seqlens || !adv || !returns) return GC_ERR_NULL;
+  return launch_gae(rewards, values, mask, cu_seqlens, R, gamma, lambda, adv, returns,
+                    static_cast<cudaStream_t>(cuda_stream));
+}
+
+size_t gc_critic_workspace_bytes(int64_t T, int64_t D) {
+  if (T < 0 || D <= 0) return 0;
+  const size_t a = value_loss_ws_bytes(T), b = value_bwd_ws_bytes(T, D);
+  return (a > b ? a : b) + 256;
+}
+
+int gc_value_loss(const float* values, const float* old_values, const float* returns,
+                  const uint8_t* mask, int64_t T, float clip_v, float grad_loss, float* out3,
+                  float* g, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (T < 0) return GC_ERR_SHAPE;
+  if (!(clip_v >= 0.f)) return GC_ERR_ARG;
+  if (!out3) return GC_ERR_NULL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (T == 0) {
+    GC_CUDA_TRY(cudaMemsetAsync(out3, 0, 3 * sizeof(float), st));
+    return GC_OK;
+  }
+  if (!values || !old_values || !returns) return GC_ERR_NULL;
+  if (!workspace || workspace_bytes < value_loss_ws_bytes(T)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  return launch_value_loss(values, old_values, returns, mask, T, clip_v, grad_loss, out3, g,
+                           workspace, st);
+}
+
+int gc_value_head_bwd(const void* H, int64_t ldH, int dtype, const void* w, const float* g,
+                      int64_t T, int64_t D, void* dH, int64_t lddH, float* dw, float* dbias,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  GC_TRY(check_value_args(H, ldH, dtype, w, T, D));
+  if (!dw) return GC_ERR_NULL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (T == 0) {
+    GC_CUDA_TRY(cudaMemsetAsync(dw, 0, (size_t)D * sizeof(float), st));
+    if (dbias) GC_CUDA_TRY(cudaMemsetAsync(dbias, 0, sizeof(float), st));
+    return GC_OK;
+  }
+  if (!g || !dH) return GC_ERR_NULL;
+  if (lddH < D || !aligned16(dH) || (lddH * elem_bytes(dtype)) % 16 != 0) return GC_ERR_ALIGN;
+  if (!workspace || workspace_bytes < value_bwd_ws_bytes(T, D)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  return launch_value_bwd(H, ldH, dtype == GC_BF16, w, g, T, D, dH, lddH, dw, dbias, workspace, st);
+}
+
 size_t gc_balance_workspace_bytes(int32_t R) { return R < 0 ? 0 : balance_ws_bytes(R); }
 
 int gc_balance_plan(const int32_t* cu_seqlens, int32_t R, const int32_t* group_offsets,

@@ -97,6 +97,20 @@ int launch_balance_plan(const int32_t* cu, int32_t R, const int32_t* group_offse
                         int32_t* n_kept, int32_t* cu_out, int32_t* src_token, int32_t* n_tokens,
                         void* ws, cudaStream_t st);
 
+// critic.cu (NEXT-2: PPO critic path)
+int launch_value_fwd(const void* H, int64_t ldH, bool bf16, const void* w, float bias, int64_t T,
+                     int64_t D, float* values, cudaStream_t st);
+int launch_gae(const float* rewards, const float* values, const uint8_t* mask, const int32_t* cu,
+               int32_t R, float gamma, float lam, float* adv, float* ret, cudaStream_t st);
+size_t value_loss_ws_bytes(int64_t T);
+int launch_value_loss(const float* values, const float* old_values, const float* returns,
+                      const uint8_t* mask, int64_t T, float clip_v, float grad_loss, float* out3,
+                      float* g, void* ws, cudaStream_t st);
+size_t value_bwd_ws_bytes(int64_t T, int64_t D);
+int launch_value_bwd(const void* H, int64_t ldH, bool bf16, const void* w, const float* g, int64_t T,
+                     int64_t D, void* dH, int64_t lddH, float* dw, float* dbias, void* ws,
+                     cudaStream_t st);
+
 // simt_head.cu
 int simt_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, bool bf16,
                   const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,

@@ -274,12 +274,14 @@ int gc_kernel_timing_end(float* ms_by_kind_host, int32_t* launches_by_kind_host)
  * by whichever CTA pair is free (the schedule of the forward / recompute / dW kernels; uses one
  * library-owned counter, so do not run two such debug calls concurrently); 0: static round-robin
  * (the schedule of the dH kernel).  dual_n != 0 (cta_group 2 only): 256 x 512 tiles whose two
- * halves share the A stages (the dH kernel's tile). */
+ * halves share the A stages (the dH kernel's tile).  cluster4 != 0 (cta_group 2 only): clusters
+ * of two CTA pairs that take adjacent M tiles and fetch every B stage once, by TMA multicast
+ * (the launch shape of the path's kernels). */
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major,
                        const void* B, int64_t ldb, int b_mn_major,
                        float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
                        int accumulate, int cta_group, int dynamic_schedule, int dual_n,
-                       void* cuda_stream);
+                       int cluster4, void* cuda_stream);
 
 #ifdef __cplusplus
 }

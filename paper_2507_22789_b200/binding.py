@@ -63,7 +63,7 @@ def _load() -> C.CDLL:
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
                                        f32, vp, vp, vp, sz, vp]
     lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, ci,
-                                       ci, vp]
+                                       ci, ci, vp]
     u64 = C.c_uint64
     lib.gc_balance_workspace_bytes.restype = sz
     lib.gc_balance_workspace_bytes.argtypes = [i32]
@@ -287,7 +287,7 @@ def gc_validate_targets(targets, mask, V) -> int:
 
 
 def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, accumulate=False,
-                       cta_group=2, dynamic_schedule=True, dual_n=False):
+                       cta_group=2, dynamic_schedule=True, dual_n=False, cluster4=False):
     """C[M,N] f32 = A.B on the tcgen05 tile engine (unit test of the engine)."""
     if a_mn_major:
         K, M = A.shape
@@ -303,7 +303,7 @@ def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, acc
     _check(_lib.gc_debug_gemm_bf16(_ptr(A), A.stride(0), int(a_mn_major), _ptr(B), B.stride(0),
                                    int(b_mn_major), _ptr(C_out), C_out.stride(0), M, N, K,
                                    int(accumulate), int(cta_group), int(dynamic_schedule),
-                                   int(dual_n), _stream()))
+                                   int(dual_n), int(cluster4), _stream()))
     return C_out
 
 

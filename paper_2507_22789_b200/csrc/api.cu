@@ -42,20 +42,13 @@ int check_head_args(const void* H, int64_t ldH, const void* W, int64_t ldW, int 
 int64_t pick_chunk(int64_t T, int64_t D, int64_t V) {
   const int64_t Tr = ceil_div(T > 0 ? T : 1, 256) * 256;
   if (Tr <= 256) return 256;
-  const int P = kNumSMs / 2;
-  const int64_t Nt = ceil_div(D, 512);
   const int64_t half = ceil_div(Tr / 2, 256) * 256;          // at least two chunks
   int64_t best = 256;
   double best_cost = 1e300;
   for (int64_t tc = 256; tc <= 8192 && tc <= half; tc += 256) {
     if (tc > 256 && (double)tc * (double)V * 2.0 > 6.0e9) break;   // dS buffer <= 6 GB
     double waves = 0;
-    for (int64_t r0 = 0; r0 < Tr; r0 += tc) {
-      const int64_t rows = (Tr - r0 < tc) ? Tr - r0 : tc;
-      const int64_t items = ceil_div(rows, 256) * Nt;
-      const int64_t r = items % P;
-      waves += (double)(items / P) + (r == 0 ? 0.0 : (2 * r <= P ? 0.5 : 1.0));
-    }
+    for (int64_t r0 = 0; r0 < Tr; r0 += tc) waves += tc_dh_waves((Tr - r0 < tc) ? Tr - r0 : tc, D);
     const double cost = waves * (1.0 + 0.01 * (double)ceil_div(Tr, tc));
     if (cost <= best_cost) { best_cost = cost; best = tc; }
   }
@@ -579,12 +572,13 @@ int gc_gather_1d(const void* x, const int32_t* rows, const int32_t* n_rows, int6
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
                        int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
                        int accumulate, int cta_group, int dynamic_schedule, int dual_n,
-                       void* cuda_stream) {
+                       int cluster4, void* cuda_stream) {
   if (!A || !B || !C) return GC_ERR_NULL;
   if (M <= 0 || N <= 0 || K <= 0) return GC_ERR_SHAPE;
   GC_TRY(check_arch());
   return tc_debug_gemm(A, lda, a_mn_major, B, ldb, b_mn_major, C, ldc, M, N, K, accumulate,
-                       cta_group, dynamic_schedule, dual_n, static_cast<cudaStream_t>(cuda_stream));
+                       cta_group, dynamic_schedule, dual_n, cluster4,
+                       static_cast<cudaStream_t>(cuda_stream));
 }
 
 }  // extern "C"

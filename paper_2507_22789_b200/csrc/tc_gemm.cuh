@@ -123,10 +123,19 @@ __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt,
 // may hold a CUtensorMap), State (registers of one epilogue thread), kWarpSmem (bytes of staging
 // smem per epilogue warp, 1024-aligned), setup / item_begin / tile_prefetch / chunk / item_end /
 // finish.
-template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1>
+//
+// PPC = CTA pairs per cluster (1 or 2).  PPC = 2 (CG = 2 only): a 4-CTA cluster whose two pairs take
+// M tiles 2i and 2i+1 of the same item and walk the same N tiles in lock-step; every B stage is
+// fetched from L2 once per cluster -- each CTA loads a quarter of the 256-row B tile and multicasts
+// it to the CTA of the other pair that needs the same half -- so the L2 -> SM operand traffic per
+// flop drops by a quarter.  Only 33 clusters of 4 are co-resident on the 148 SMs of a B200, which
+// is why the path's kernels stay on PPC = 1 (measurements in tc_head.cu).
+template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1, int PPC = 1>
 __global__ void __launch_bounds__(kThreads, 1)
 k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
           const Sched s, const __grid_constant__ typename Epi::Params ep) {
+  static_assert(PPC == 1 || (PPC == 2 && CG == 2), "pairs per cluster");
+  constexpr int CL = CG * PPC;                 // CTAs per cluster
   using C = Cfg<CG, NSUB>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -145,8 +154,12 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   static_assert(8 * (2 * C::kStages + 4) + 4 <= 136, "barrier area overlap");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = CG == 2 ? ptx::cluster_ctarank() : 0u;
-  const int64_t pair = blockIdx.x / CG, n_pairs = gridDim.x / CG;
+  const uint32_t rank = CL > 1 ? ptx::cluster_ctarank() : 0u;   // rank in the cluster
+  const uint32_t prank = rank % CG;                             // rank in the CTA pair
+  const uint32_t pic = rank / CG;                               // pair in the cluster
+  const uint32_t lead = rank - prank;                           // cluster rank of the pair's leader
+  // scheduling unit = cluster
+  const int64_t pair = blockIdx.x / CL, n_pairs = gridDim.x / CL;
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tmap(&tmA);
@@ -155,7 +168,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < C::kStages; ++i) {
       ptx::mbar_init(full_bar(i), 1);
-      ptx::mbar_init(empty_bar(i), 1);
+      ptx::mbar_init(empty_bar(i), PPC);       // every pair that receives this CTA's multicast
     }
     for (int i = 0; i < 2; ++i) {
       ptx::mbar_init(tfull_bar(i), 1);
@@ -163,9 +176,9 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     }
     for (int i = 0; i < kSlots; ++i) {
       ptx::mbar_init(sfull_bar(i), 1);
-      // consumers of a slot: MMA lane + 4 epilogue warps (leader), producer lane + 4 epilogue
-      // warps (peer)
-      ptx::mbar_init(sempty_bar(i), 5 * CG);
+      // consumers of a slot: 4 epilogue warps per CTA, the producer lane of every CTA but the
+      // scheduler's, the MMA lane of every pair leader
+      ptx::mbar_init(sempty_bar(i), 4 * CL + (CL - 1) + PPC);
     }
     ptx::fence_barrier_init();
   }
@@ -174,14 +187,15 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     ptx::tmem_relinquish<CG>();
   }
   ptx::tc_fence_before();
-  if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  if constexpr (CL > 1) ptx::cluster_sync(); else __syncthreads();
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   int64_t M_eff, K_eff;
   resolve_dims(s, M_eff, K_eff);
-  const int64_t Mt = (M_eff + BM_CTA * CG - 1) / (BM_CTA * CG);
+  // M tiles of an item's unit: PPC consecutive 128*CG-row tiles (one per pair of the cluster)
+  const int64_t Mt = (M_eff + BM_CTA * CG * PPC - 1) / (BM_CTA * CG * PPC);
   const int64_t Nt = (s.N + BN * NSUB - 1) / (BN * NSUB);   // item tiles along N
   const int64_t n_chunks = s.c_major ? (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles : Nt;
   const int num_kb = (int)((K_eff + BK - 1) / BK);
@@ -234,9 +248,10 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     ptx::mbar_wait_cluster(sempty_bar(cur.slot), cur.phase ^ 1u);
     ptx::st_shared_u32(sitem(cur.slot), (uint32_t)v);
     ptx::mbar_arrive(sfull_bar(cur.slot));
-    if constexpr (CG == 2) {
-      ptx::st_shared_cluster_u32(ptx::mapa(sitem(cur.slot), 1), (uint32_t)v);
-      ptx::mbar_arrive_cluster(ptx::mapa(sfull_bar(cur.slot), 1));
+#pragma unroll
+    for (uint32_t peer = 1; peer < (uint32_t)CL; ++peer) {
+      ptx::st_shared_cluster_u32(ptx::mapa(sitem(cur.slot), peer), (uint32_t)v);
+      ptx::mbar_arrive_cluster(ptx::mapa(sfull_bar(cur.slot), peer));
     }
     if (++cur.slot == kSlots) { cur.slot = 0; cur.phase ^= 1u; }
     return (int64_t)v;
@@ -257,11 +272,13 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
         if (scheduler) ticket = atomicAdd(s.counter, 1u);
         int64_t it_next = -1;
         const Item item = item_of(it);
-        const int32_t m_coord = (int32_t)(item.m_tile * BM_CTA * CG + rank * BM_CTA);
+        const int32_t m_coord =
+            (int32_t)((item.m_tile * PPC + pic) * BM_CTA * CG + prank * BM_CTA);
+        const uint16_t b_mask = (uint16_t)((1u << prank) | (1u << (prank + CG)));   // PPC == 2
         for (int64_t n = item.n0; n < item.n1; ++n) {
           const int nsub = item.half < 0 ? NSUB : 1;    // half tile: one B sub-tile, in slot 0
           const int32_t n_coord = (int32_t)(n * BN * NSUB + (item.half > 0 ? BN : 0) +
-                                            rank * C::kBRows);
+                                            prank * C::kBRows);
           const uint32_t stage_tx = (uint32_t)(kABytes + nsub * C::kBBytes);
           for (int kb = 0; kb < num_kb; ++kb) {
             ptx::mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -290,8 +307,8 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               }
             } else {
               // the leader's barrier collects the bytes of both CTAs
-              if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx * 2);
-              const uint32_t fb = ptx::mapa(full_bar(stage), 0);
+              if (prank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx * 2);
+              const uint32_t fb = ptx::mapa(full_bar(stage), lead);
               if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb, polA);
               else {
                 ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb, polA);
@@ -302,8 +319,18 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 if (sub >= nsub) break;
                 const uint32_t sbs = sb + sub * C::kBBytes;
                 const int32_t nc = n_coord + sub * BN;
-                if constexpr (!B_MN) ptx::tma_load_2d_cg2(sbs, &tmB, k_coord, nc, fb, polB);
-                else {
+                if constexpr (PPC == 2) {
+                  // this CTA's quarter (64 B rows) of the tile, multicast to the CTA of the
+                  // other pair that stages the same half
+                  if constexpr (!B_MN)
+                    ptx::tma_load_2d_cg2_mc(sbs + 8192 * pic, &tmB, k_coord, nc + 64 * (int32_t)pic, fb,
+                                            b_mask, polB);
+                  else
+                    ptx::tma_load_2d_cg2_mc(sbs + 8192 * pic, &tmB, nc + 64 * (int32_t)pic, k_coord, fb,
+                                            b_mask, polB);
+                } else if constexpr (!B_MN) {
+                  ptx::tma_load_2d_cg2(sbs, &tmB, k_coord, nc, fb, polB);
+                } else {
 #pragma unroll
                   for (int b = 0; b < C::kBRows / 64; ++b)
                     ptx::tma_load_2d_cg2(sbs + 8192 * b, &tmB, nc + 64 * b, k_coord, fb, polB);
@@ -319,7 +346,11 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     }
   } else if (warp == 1) {
     // ===================== MMA issuer (one lane of the leader CTA) =====================
-    if (rank == 0 && lane == 0) {
+    if (prank == 0 && lane == 0) {
+      // commits: a smem slot is released in every CTA of the cluster (each multicasts into it),
+      // an accumulator is announced to this pair's two CTAs
+      constexpr uint16_t kAllCtas = (uint16_t)((1u << CL) - 1u);
+      const uint16_t pair_ctas = (uint16_t)(((1u << CG) - 1u) << lead);
       constexpr uint32_t idesc = ptx::make_idesc_bf16(BM_CTA * CG, BN, A_MN, B_MN);
       constexpr uint32_t a_step = A_MN ? (2048 >> 4) : (32 >> 4);   // per UMMA_K = 16
       constexpr uint32_t b_step = B_MN ? (2048 >> 4) : (32 >> 4);
@@ -354,15 +385,15 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 ptx::umma_bf16<CG>(d_tmem, adesc + (uint64_t)(k * a_step),
                                    bdesc + (uint64_t)(k * b_step), idesc, (uint32_t)(kb | k));
             }
-            ptx::umma_commit<CG>(empty_bar(stage));      // frees the smem slot (both CTAs)
+            ptx::umma_commit<CG>(empty_bar(stage), kAllCtas);   // frees the smem slot
             if (++stage == C::kStages) { stage = 0; phase ^= 1u; }
           }
           if constexpr (NSUB == 1) {
-            ptx::umma_commit<CG>(tfull_bar(acc));        // accumulator ready (both CTAs)
+            ptx::umma_commit<CG>(tfull_bar(acc), pair_ctas);    // accumulator ready (both CTAs)
             if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
           } else {
-            ptx::umma_commit<CG>(tfull_bar(0));
-            ptx::umma_commit<CG>(tfull_bar(1));
+            ptx::umma_commit<CG>(tfull_bar(0), pair_ctas);
+            ptx::umma_commit<CG>(tfull_bar(1), pair_ctas);
             acc_phase ^= 1u;
           }
         }
@@ -379,7 +410,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
     Epi::setup(st, ep, bar_base + C::kBarBytes + (uint32_t)(q * Epi::kWarpSmem));
     for (int64_t it = consume(true); it >= 0; it = consume(true)) {
       const Item item = item_of(it);
-      const int64_t grow = item.m_tile * BM_CTA * CG + rank * BM_CTA + row_in_tile;
+      const int64_t grow = (item.m_tile * PPC + pic) * BM_CTA * CG + prank * BM_CTA + row_in_tile;
       const bool valid = grow < M_eff;
       Epi::item_begin(st, ep, grow, valid, item.c);
       for (int64_t nn = item.n0 * NSUB; nn < item.n1 * NSUB; ++nn) {
@@ -395,7 +426,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           __syncwarp();
           if (lane == 0) {
             if constexpr (CG == 1) ptx::mbar_arrive(tempty_bar(acc));
-            else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
+            else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), lead));
           }
           if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
           continue;
@@ -417,7 +448,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
             __syncwarp();
             if (lane == 0) {
               if constexpr (CG == 1) ptx::mbar_arrive(tempty_bar(acc));
-              else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), 0));
+              else ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(acc), lead));
             }
           }
           float x[32];
@@ -434,7 +465,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
 
   // ---- teardown ----
   ptx::tc_fence_before();
-  if constexpr (CG == 2) ptx::cluster_sync(); else __syncthreads();
+  if constexpr (CL > 1) ptx::cluster_sync(); else __syncthreads();
   if (warp == 2) ptx::tmem_dealloc<CG>(tmem_base, kTmemCols);
 }
 
@@ -490,22 +521,46 @@ inline int num_sms() {
   return n;
 }
 
-template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1>
+// Clusters of `cl` CTAs that can be co-resident with this kernel's resources (1 CTA per SM): 74 of
+// 2, 33 of 4 on a B200 (GPC boundaries).  Queried once per kernel instantiation.
+template <class Kern>
+inline int max_active_clusters(Kern kern, int cl, int smem_bytes) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(num_sms() / cl * cl));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = (size_t)smem_bytes;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cl;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = num_sms() / cl;
+  return n;
+}
+
+template <int CG, bool A_MN, bool B_MN, class Epi, int NSUB = 1, int PPC = 1>
 int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& s,
                    const typename Epi::Params& ep, cudaStream_t st) {
-  auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi, NSUB>;
+  auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi, NSUB, PPC>;
+  constexpr int CL = CG * PPC;
   constexpr int kSmemBytes = Cfg<CG, NSUB>::kSmemBase + 4 * Epi::kWarpSmem;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
-  GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+  static int clusters = 0;                       // per instantiation
+  if (clusters == 0) {
+    GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    clusters = max_active_clusters(kern, CL, kSmemBytes);
+  }
   cudaLaunchConfig_t cfg = {};
-  const int sms = num_sms();
-  cfg.gridDim = dim3((unsigned)(sms / CG * CG));
+  cfg.gridDim = dim3((unsigned)(clusters * CL));
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = kSmemBytes;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.x = CL;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;

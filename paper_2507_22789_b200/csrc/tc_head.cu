@@ -8,9 +8,20 @@
 #include <stdio.h>
 #include <stdlib.h>
 
-#ifndef GC_DEFAULT_CG
-#define GC_DEFAULT_CG 2
+// Production launch shape: CTA pairs (cta_group::2) in clusters of kPpc pairs (tc_gemm.cuh).
+// kPpc = 2 (4-CTA clusters, B stages fetched once per cluster by TMA multicast) is built, tested
+// (test_engine_gemm_cluster4) and measured, but is not the default: only 33 clusters of 4 are
+// co-resident on the 148 SMs, and same-box A/B on cfg2 gave 79.5 ms (kPpc 2: 132 SMs at 1395 MHz)
+// against 78.7 ms (kPpc 1: 148 SMs at 1245 MHz) and 81.0 ms (kPpc 1 restricted to 132 SMs): the
+// multicast saves ~2 % energy per flop, less than the 16 idle SMs cost.  Build with -DGC_PPC=2 to
+// use it.
+#ifndef GC_PPC
+#define GC_PPC 1
 #endif
+constexpr int kPpc = GC_PPC;
+// scheduling units = co-resident clusters on a B200 (the launcher queries the real number; the
+// planners only need it to size waves): 74 pairs, or 33 clusters of two pairs
+constexpr int kUnits = kPpc == 2 ? 33 : 74;
 
 namespace gc {
 
@@ -213,9 +224,9 @@ struct EpiDS {
     }
   }
   static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
-  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool,
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool valid,
                                                int64_t col0, const float (&x)[32]) {
-    if (col0 >= p.ldS) return;
+    if (!valid || col0 >= p.ldS) return;       // !valid: phantom M tile of an odd cluster item
     float v[32];
     if (st.gp == 0.f) {
 #pragma unroll
@@ -363,13 +374,13 @@ constexpr int64_t kL2ResidentBytes = 40ll << 20;   // resident panels of the dW 
 // the CTA pairs (wave quantisation, SURVEY.md sec 7.2 hard part 5); longer items win ties.
 // ---------------------------------------------------------------------------------------------
 TcPlan tc_plan_forward(int64_t T, int64_t D, int64_t V) {
-  const int P = kNumSMs / 2;
-  const int64_t Mt = ceil_div(T > 0 ? T : 1, 256);
+  const int P = kUnits;
+  const int64_t Mt = ceil_div(T > 0 ? T : 1, 256 * kPpc);      // M extent of an item = kPpc tiles
   const int64_t Nt = ceil_div(V, tc::BN);
   const int64_t panel = 512 * D;
   TcPlan best{(int)Nt, 1, (int)Nt};
   double best_cost = 1e300;
-  int64_t max_split = (512ll << 20) / (Mt * 256 * (int64_t)sizeof(RowStat));
+  int64_t max_split = (512ll << 20) / (Mt * 256 * kPpc * (int64_t)sizeof(RowStat));
   if (max_split > 512) max_split = 512;
   if (max_split < 1) max_split = 1;
   int64_t kmin = ceil_div(Nt, max_split);
@@ -402,7 +413,8 @@ TcPlan tc_plan_forward(int64_t T, int64_t D, int64_t V) {
 static int pick_m_band(int64_t D, int k) {
   const int64_t panel = 512 * D;
   int64_t mb = (kL2BudgetBytes - (int64_t)k * panel) / panel;
-  return (int)(mb < 4 ? 4 : (mb > 64 ? 64 : mb));
+  mb = mb < 4 ? 4 : (mb > 64 ? 64 : mb);
+  return (int)(mb / kPpc);                     // in items (kPpc M tiles each)
 }
 // N tiles per band of the dW schedule: the band's H panels (k_rows x 256 columns bf16).
 static int pick_n_band(int64_t k_rows) {
@@ -435,16 +447,23 @@ static void exp_override(Sched& s, const char* kind) {
 #define GC_EXP_OVERRIDE(s, kind) ((void)0)
 #endif
 
+// every launch shape of the engine (debug GEMM only; the path's kernels use fixed shapes)
 template <class Epi, bool A_MN, bool B_MN>
-static int launch_cg(int cg, const CUtensorMap& a, const CUtensorMap& b, const Sched& s,
-                     const typename Epi::Params& ep, cudaStream_t st, bool dual_n = false) {
-  if (dual_n) {
-    if (cg != 2) return GC_ERR_ARG;
-    return tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 2>(a, b, s, ep, st);
+static int launch_any(int cg, bool dual_n, int ppc, const CUtensorMap& a, const CUtensorMap& b,
+                      const Sched& s, const typename Epi::Params& ep, cudaStream_t st) {
+  if (cg == 1) {
+    if (dual_n || ppc != 1) return GC_ERR_ARG;
+    return tc::launch_tc_gemm<1, A_MN, B_MN, Epi>(a, b, s, ep, st);
   }
-  if (cg == 2) return tc::launch_tc_gemm<2, A_MN, B_MN, Epi>(a, b, s, ep, st);
-  return tc::launch_tc_gemm<1, A_MN, B_MN, Epi>(a, b, s, ep, st);
+  if (ppc == 2)
+    return dual_n ? tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 2, 2>(a, b, s, ep, st)
+                  : tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 1, 2>(a, b, s, ep, st);
+  return dual_n ? tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 2, 1>(a, b, s, ep, st)
+                : tc::launch_tc_gemm<2, A_MN, B_MN, Epi, 1, 1>(a, b, s, ep, st);
 }
+
+// K-major B operand: rows of one TMA box = the share of the 256-row tile one CTA fetches
+static int b_box_rows(int cg, int ppc) { return tc::BN / cg / ppc; }
 
 static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   Sched s;
@@ -458,10 +477,9 @@ static Sched make_sched(int64_t M, int64_t N, int64_t K) {
 int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T, int64_t D,
                      int64_t V, float tau, const int32_t* targets_c, const int32_t* n_rows_dev,
                      RowStat* partials, uint32_t* counter, cudaStream_t st) {
-  const int cg = GC_DEFAULT_CG;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / cg));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, b_box_rows(2, kPpc)));
   const TcPlan pl = tc_plan_forward(T, D, V);
   Sched s = make_sched(T, V, D);
   s.chunk_ntiles = pl.chunk_vtiles;
@@ -479,7 +497,7 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   ep.c = kLog2e / tau;
   GC_EXP_OVERRIDE(s, "FWD");
   KernelTimer kt(GC_KERNEL_FWD_STATS, st);
-  return launch_cg<EpiStats, false, false>(cg, ta, tb, s, ep, st);
+  return tc::launch_tc_gemm<2, false, false, EpiStats, 1, kPpc>(ta, tb, s, ep, st);
 }
 
 int tc_forward_stats_multi(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
@@ -488,7 +506,7 @@ int tc_forward_stats_multi(const void* H, int64_t ldH, const void* W, int64_t ld
   if (K < 1 || K > kMaxTargets) return GC_ERR_ARG;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, H, T, D, ldH, false, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / 2));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, b_box_rows(2, kPpc)));
   const TcPlan pl = tc_plan_forward(T, D, V);
   Sched s = make_sched(T, V, D);
   s.chunk_ntiles = pl.chunk_vtiles;
@@ -506,18 +524,17 @@ int tc_forward_stats_multi(const void* H, int64_t ldH, const void* W, int64_t ld
   ep.c = kLog2e / tau;
   ep.K = K;
   KernelTimer kt(GC_KERNEL_FWD_STATS, st);
-  return tc::launch_tc_gemm<2, false, false, EpiStatsMulti>(ta, tb, s, ep, st);
+  return tc::launch_tc_gemm<2, false, false, EpiStatsMulti, 1, kPpc>(ta, tb, s, ep, st);
 }
 
 int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t rows_cap,
                     int64_t n_static, int64_t D, int64_t V, float tau, const int32_t* targets_c,
                     const float* lse_c, const float* g_c, const int32_t* n_rows_dev, int64_t row0,
                     void* dS, int64_t ldS, uint32_t* counter, cudaStream_t st) {
-  const int cg = GC_DEFAULT_CG;
   const int64_t h_rows = n_rows_dev ? rows_cap : n_static;   // rows behind the H pointer
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, H, h_rows, D, ldH, false, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, tc::BN / cg));
+  GC_TRY(tc::make_operand_tmap(&tb, W, V, D, ldW, false, b_box_rows(2, kPpc)));
   // rows up to the next multiple of 256 past the valid count are written as zeros: the dW
   // contraction runs over them (rows_cap is a multiple of 256)
   Sched s = make_sched(ceil_div(h_rows, 256) * 256, V, D);
@@ -546,13 +563,12 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   ep.inv_tau = 1.0f / tau;
   GC_EXP_OVERRIDE(s, "DS");
   KernelTimer kt(GC_KERNEL_RECOMPUTE_DS, st);
-  return launch_cg<EpiDS, false, false>(cg, ta, tb, s, ep, st);
+  return tc::launch_tc_gemm<2, false, false, EpiDS, 1, kPpc>(ta, tb, s, ep, st);
 }
 
 int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* W,
           int64_t ldW, int64_t D, int64_t V, const int32_t* rows, const int32_t* n_rows_dev,
           int64_t row0, void* dH, int64_t lddH, uint32_t* counter, cudaStream_t st) {
-  const int cg = GC_DEFAULT_CG;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, dS, rows_cap, V, ldS, false, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
@@ -568,13 +584,12 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   GC_EXP_OVERRIDE(s, "DH");
   KernelTimer kt(GC_KERNEL_DH, st);
   // K = V is ~2000 k-blocks per tile: 256 x 512 dual-N tiles (tc_gemm.cuh, Cfg)
-  return launch_cg<EpiStoreBf16, false, true>(cg, ta, tb, s, ep, st, cg == 2);
+  return tc::launch_tc_gemm<2, false, true, EpiStoreBf16, 2, kPpc>(ta, tb, s, ep, st);
 }
 
 int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
           int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
           int64_t lddW, int accumulate, uint32_t* counter, cudaStream_t st) {
-  const int cg = GC_DEFAULT_CG;
   const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
@@ -594,21 +609,30 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.accumulate = accumulate;
   GC_EXP_OVERRIDE(s, "DW");
   KernelTimer kt(GC_KERNEL_DW, st);
-  return launch_cg<EpiStoreF32, true, true>(cg, ta, tb, s, ep, st);
+  return tc::launch_tc_gemm<2, true, true, EpiStoreF32, 1, kPpc>(ta, tb, s, ep, st);
 }
 
 // one counter for the debug GEMM (not safe for concurrent debug calls on different streams)
 __device__ uint32_t g_debug_counter;
 
+// dH tile waves of a chunk of `rows` rows (api.cu's chunk picker): items of kPpc x (256 x 512) tiles
+// over the scheduling units; a last wave that is at most half full costs half a wave.
+double tc_dh_waves(int64_t rows, int64_t D) {
+  const int64_t items = ceil_div(rows, 256 * kPpc) * ceil_div(D, 512);
+  const int64_t r = items % kUnits;
+  return (double)(items / kUnits) + (r == 0 ? 0.0 : (2 * r <= kUnits ? 0.5 : 1.0));
+}
+
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, int dynamic_schedule, int dual_n, cudaStream_t st) {
+                  int cta_group, int dynamic_schedule, int dual_n, int cluster4, cudaStream_t st) {
   if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
-  if (dual_n && cta_group != 2) return GC_ERR_ARG;
+  if ((dual_n || cluster4) && cta_group != 2) return GC_ERR_ARG;
+  const int ppc = cluster4 ? 2 : 1;
   if (N % 4 != 0) return GC_ERR_SHAPE;
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, tc::BN / cta_group));
+  GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, b_box_rows(cta_group, ppc)));
   Sched s = make_sched(M, N, K);
   if (dynamic_schedule) {
     void* ctr = nullptr;
@@ -621,10 +645,10 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
   ep.N = N;
   ep.accumulate = accumulate;
   const bool d2 = dual_n != 0;
-  if (!a_mn && !b_mn) return launch_cg<EpiStoreF32, false, false>(cta_group, ta, tb, s, ep, st, d2);
-  if (!a_mn && b_mn) return launch_cg<EpiStoreF32, false, true>(cta_group, ta, tb, s, ep, st, d2);
-  if (a_mn && !b_mn) return launch_cg<EpiStoreF32, true, false>(cta_group, ta, tb, s, ep, st, d2);
-  return launch_cg<EpiStoreF32, true, true>(cta_group, ta, tb, s, ep, st, d2);
+  if (!a_mn && !b_mn) return launch_any<EpiStoreF32, false, false>(cta_group, d2, ppc, ta, tb, s, ep, st);
+  if (!a_mn && b_mn) return launch_any<EpiStoreF32, false, true>(cta_group, d2, ppc, ta, tb, s, ep, st);
+  if (a_mn && !b_mn) return launch_any<EpiStoreF32, true, false>(cta_group, d2, ppc, ta, tb, s, ep, st);
+  return launch_any<EpiStoreF32, true, true>(cta_group, d2, ppc, ta, tb, s, ep, st);
 }
 
 }  // namespace gc

@@ -144,6 +144,21 @@ __device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const CUtensorMap*
       : "memory");
 }
 
+// Multicast variant: the tile lands at the same smem offset in every CTA of `cta_mask` (cluster
+// ranks), and each destination's bytes complete on the barrier at `bar`'s offset in the leader
+// (even rank) of that destination's CTA pair -- `bar` must carry a cleared peer bit, i.e. be the
+// issuing pair's leader barrier (the convention of 2-SM multicast loads).
+__device__ __forceinline__ void tma_load_2d_cg2_mc(uint32_t dst, const CUtensorMap* m, int32_t c0,
+                                                   int32_t c1, uint32_t bar, uint16_t cta_mask,
+                                                   uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
+      ".multicast::cluster.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5, %6;"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "h"(cta_mask),
+        "l"(pol)
+      : "memory");
+}
+
 // ---- TMA stores (smem tile -> global, bulk-group completion) ---------------------------------
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, uint32_t src, int32_t c0,
                                              int32_t c1) {

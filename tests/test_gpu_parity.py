@@ -73,6 +73,28 @@ def test_engine_gemm_dual_n(B, dyn, a_mn, b_mn, M, N, K):
     assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
 
 
+@pytest.mark.parametrize("dyn", [False, True])
+@pytest.mark.parametrize("dual", [False, True])
+@pytest.mark.parametrize("a_mn,b_mn", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K", [(256, 256, 64), (392, 520, 200), (1000, 776, 1096),
+                                   (256 * 5 + 8, 256 * 7 + 8, 328), (256 * 21 + 40, 256 * 9 + 8, 320)])
+def test_engine_gemm_cluster4(B, dyn, dual, a_mn, b_mn, M, N, K):
+    """Clusters of two CTA pairs: adjacent M tiles, every B stage fetched once and multicast (the
+    launch shape of the path's kernels), incl. an odd number of M tiles (phantom tile), both
+    schedules, both tile shapes, all operand layouts; reruns bit-identical."""
+    g = torch.Generator(device="cuda").manual_seed(M + N + K + 2)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    args = (A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm, a_mn, b_mn)
+    kw = dict(cta_group=2, dynamic_schedule=dyn, dual_n=dual, cluster4=True)
+    C = B.gc_debug_gemm_bf16(*args, **kw)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    C2 = B.gc_debug_gemm_bf16(*args, C_out=C.clone(), accumulate=True, **kw)
+    assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+    assert torch.equal(C, B.gc_debug_gemm_bf16(*args, **kw))
+
+
 @pytest.mark.parametrize("dual", [False, True])
 @pytest.mark.parametrize("dyn", [False, True])
 def test_engine_gemm_many_tiles(B, dyn, dual):

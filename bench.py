@@ -127,6 +127,9 @@ def make_step(B, b: DeviceBatch):
             return B.gc_token_logprobs(b.H, b.W, b.y, b.mask, w.tau, want_lse=False)
         return step, 1 + fwd_launches
 
+    if w.drop_constant_groups:
+        return make_step_dynamic_sampling(B, b)
+
     def step():
         adv, _ = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, w.drop_constant_groups)
         f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
@@ -141,6 +144,47 @@ def make_step(B, b: DeviceBatch):
     else:
         bwd = 2 + 2
     return step, 1 + fwd_launches + 2 + bwd
+
+
+def make_step_dynamic_sampling(B, b):
+    """configs[3]: group filter -> repack + workload balancing (gc_balance_plan: kept samples
+    sorted by simulated workload L^2, buckets of one group's size, shuffled) -> gathers of H,
+    targets, old / ref log-probs -> forward + backward on the kept batch.  Everything runs on the
+    device every step; only the kept sizes (fixed by the seeded rewards) are read once at set-up."""
+    w = b.w
+    R = b.cu.numel() - 1
+    adv_all, keep = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, True)
+    plan = B.gc_balance_plan(b.cu, b.go, keep, 0, 1, w.group_size, 1234, True, n_tokens_max=b.T)
+    Tk, Rk = int(plan["n_tokens"].item()), int(plan["n_kept"].item())
+    b.n_scored = Tk
+    b.T_kept = Tk
+    dH = torch.empty(Tk, w.D, dtype=b.H.dtype, device=b.H.device)
+    del b.dH
+
+    def step():
+        adv_all, keep = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, True)
+        p = B.gc_balance_plan(b.cu, b.go, keep, 0, 1, w.group_size, 1234, True, n_tokens_max=b.T)
+        Hk = B.gc_gather_rows(b.H, p["src_token"], p["n_tokens"], Tk)
+        yk = B.gc_gather_1d(b.y, p["src_token"], p["n_tokens"], Tk)
+        oldk = B.gc_gather_1d(b.old, p["src_token"], p["n_tokens"], Tk)
+        refk = B.gc_gather_1d(b.ref, p["src_token"], p["n_tokens"], Tk)
+        advk = B.gc_gather_1d(adv_all, p["order"], p["n_kept"], Rk)
+        cuk = p["cu_out"][:Rk + 1]
+        f = B.gc_grpo_loss_fwd(Hk, b.W, yk, None, w.tau, cuk, advk, oldk, refk, w.clip_lo, w.clip_hi,
+                               w.beta)
+        B.gc_grpo_loss_bwd(Hk, b.W, yk, None, w.tau, cuk, advk, oldk, refk, f["logp"], f["lse"],
+                           w.clip_lo, w.clip_hi, w.beta, dH=dH, dW=b.dW)
+        return f["out5"]
+    n_chunks = -(-Tk // _bwd_chunk_T(B, Tk, w))
+    # advantages 1 + plan 7 (+ memset) + gathers 5 + fwd 2 + loss 3 + bwd: loss 3 + 3 per chunk
+    return step, 1 + 7 + 5 + 2 + 3 + 3 + 3 * n_chunks
+
+
+def _bwd_chunk_T(B, T, w):
+    a = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 0)
+    c256 = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 256)
+    ld = -(-w.V // 64) * 64
+    return 256 + (a - c256) // (ld * 2)
 
 
 def _bwd_chunk(B, b):
@@ -462,7 +506,11 @@ def main():
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32",
-            "data": "synthetic", "config": workload_config(w, b.T, world),
+            "data": "synthetic",
+            "config": dict(workload_config(w, b.T, world),
+                           **({"tokens_kept_after_group_filter": b.T_kept,
+                               "flow": "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"}
+                              if hasattr(b, "T_kept") else {})),
             "clocks": clocks, "gpu_launches": launches * args.steps,
             "roofline": roof,
         }

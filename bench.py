@@ -137,13 +137,13 @@ def make_step(B, b: DeviceBatch):
         B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f["logp"],
                            f["lse"], w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW)
         return f["out5"]
-    # launches: advantages 1, fwd, loss 2, bwd: loss 2 + compaction 8 + 3 per chunk (or SIMT 2)
+    # launches: advantages 1, fwd, loss 3, bwd: loss 3 + compaction 8 + 3 per chunk (or SIMT 2)
     if tc:
         n_chunks = -(-b.T // _bwd_chunk(B, b))
-        bwd = 2 + (8 if compact else 0) + 3 * n_chunks
+        bwd = 3 + (8 if compact else 0) + 3 * n_chunks
     else:
-        bwd = 2 + 2
-    return step, 1 + fwd_launches + 2 + bwd
+        bwd = 3 + 2
+    return step, 1 + fwd_launches + 3 + bwd
 
 
 def make_step_dynamic_sampling(B, b):

@@ -204,7 +204,7 @@ template <bool kBf16>
 __global__ void __launch_bounds__(kBwdThreads)
 k_value_bwd(const void* __restrict__ H, int64_t ld, const void* __restrict__ w,
             const float* __restrict__ g, int64_t T, int64_t D, void* __restrict__ dH, int64_t lddH,
-            float* __restrict__ dw_part /*[row blocks, D]*/) {
+            float* __restrict__ dw_part /*[row blocks, D]*/, float* __restrict__ db_part) {
   const int64_t col = (int64_t)blockIdx.y * kBwdCols + (int64_t)threadIdx.x * 8;
   if (col >= D) return;
   float wv[8], acc[8];
@@ -217,6 +217,7 @@ k_value_bwd(const void* __restrict__ H, int64_t ld, const void* __restrict__ w,
   }
 #pragma unroll
   for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+  float gsum = 0.f;                              // sum of g over this block's rows (for dbias)
   // persistent over row tiles: tile = blockIdx.x, + gridDim.x, ... (one partial per block)
   for (int64_t r0 = (int64_t)blockIdx.x * kBwdRows; r0 < T; r0 += (int64_t)gridDim.x * kBwdRows) {
   const int64_t r1 = r0 + kBwdRows < T ? r0 + kBwdRows : T;
@@ -257,17 +258,19 @@ k_value_bwd(const void* __restrict__ H, int64_t ld, const void* __restrict__ w,
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) acc[j] = fmaf(gt[u], h[u][j], acc[j]);
+      gsum += gt[u];
     }
   }
   }
+  if (blockIdx.y == 0 && threadIdx.x == 0) db_part[blockIdx.x] = gsum;
   float* out = dw_part + (int64_t)blockIdx.x * D + col;
   *reinterpret_cast<float4*>(out) = make_float4(acc[0], acc[1], acc[2], acc[3]);
   *reinterpret_cast<float4*>(out + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
 }
 
-// dw[d] = sum over row blocks in index order (fp64); db = sum_t g_t by block 0's extra pass
-__global__ void k_value_bwd_reduce(const float* __restrict__ dw_part, int64_t nblocks, int64_t D,
-                                   const float* __restrict__ g, int64_t T, float* __restrict__ dw,
+// dw[d] = sum over row blocks in index order (fp64); db = the blocks' row sums in index order
+__global__ void k_value_bwd_reduce(const float* __restrict__ dw_part, const float* __restrict__ db_part,
+                                   int64_t nblocks, int64_t D, float* __restrict__ dw,
                                    float* __restrict__ dbias) {
   const int64_t d = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (d < D) {
@@ -275,18 +278,10 @@ __global__ void k_value_bwd_reduce(const float* __restrict__ dw_part, int64_t nb
     for (int64_t b = 0; b < nblocks; ++b) a += (double)dw_part[b * D + d];
     dw[d] = (float)a;
   }
-  if (blockIdx.x == 0 && dbias) {
+  if (blockIdx.x == 0 && threadIdx.x == 0 && dbias) {
     double a = 0.0;
-    for (int64_t t = threadIdx.x; t < T; t += blockDim.x) a += (double)g[t];
-    a = wsum(a);
-    __shared__ double s[32];
-    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = a;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      a = 0.0;
-      for (int w = 0; w < (int)(blockDim.x >> 5); ++w) a += s[w];
-      *dbias = (float)a;
-    }
+    for (int64_t b = 0; b < nblocks; ++b) a += (double)db_part[b];
+    *dbias = (float)a;
   }
 }
 
@@ -337,18 +332,21 @@ static int64_t value_bwd_row_blocks(int64_t T) {
   return rb < 2 * kNumSMs ? rb : 2 * kNumSMs;      // a function of T only: reruns are bit-identical
 }
 size_t value_bwd_ws_bytes(int64_t T, int64_t D) {
-  return align_up((size_t)value_bwd_row_blocks(T) * (size_t)D * sizeof(float), 256);
+  return align_up((size_t)value_bwd_row_blocks(T) * (size_t)D * sizeof(float), 256) +
+         align_up((size_t)value_bwd_row_blocks(T) * sizeof(float), 256);
 }
 
 int launch_value_bwd(const void* H, int64_t ldH, bool bf16, const void* w, const float* g, int64_t T,
                      int64_t D, void* dH, int64_t lddH, float* dw, float* dbias, void* ws,
                      cudaStream_t st) {
   const int64_t rb = value_bwd_row_blocks(T);
-  float* part = static_cast<float*>(ws);
+  Carver c(ws);
+  float* part = c.take<float>((size_t)rb * (size_t)D);
+  float* db_part = c.take<float>((size_t)rb);
   dim3 grid((unsigned)rb, (unsigned)ceil_div(D, kBwdCols));
-  if (bf16) k_value_bwd<true><<<grid, kBwdThreads, 0, st>>>(H, ldH, w, g, T, D, dH, lddH, part);
-  else k_value_bwd<false><<<grid, kBwdThreads, 0, st>>>(H, ldH, w, g, T, D, dH, lddH, part);
-  k_value_bwd_reduce<<<(unsigned)ceil_div(D, 256), 256, 0, st>>>(part, rb, D, g, T, dw, dbias);
+  if (bf16) k_value_bwd<true><<<grid, kBwdThreads, 0, st>>>(H, ldH, w, g, T, D, dH, lddH, part, db_part);
+  else k_value_bwd<false><<<grid, kBwdThreads, 0, st>>>(H, ldH, w, g, T, D, dH, lddH, part, db_part);
+  k_value_bwd_reduce<<<(unsigned)ceil_div(D, 256), 256, 0, st>>>(part, db_part, rb, D, dw, dbias);
   GC_CUDA_TRY(cudaGetLastError());
   return GC_OK;
 }

@@ -266,8 +266,31 @@ k_token_loss(const float* __restrict__ logp, const float* __restrict__ old_logp,
              LossCounters* __restrict__ cnt, LossPartial* __restrict__ partials,
              float* __restrict__ out5, float* __restrict__ g) {
   __shared__ int32_t s_cu[kCuSmem];
-  const CuSlice cs = load_cu_slice(cu, tile_r, s_cu);
   const int64_t tile0 = (int64_t)blockIdx.x * kLossTile;
+  // Whole tiles: issue this thread's 8 tokens' loads first, so that their DRAM latency overlaps
+  // the staging of the cu_seqlens slice (two dependent loads and a block barrier).
+  const bool whole = tile0 + kLossTile <= T;
+  const int64_t t0f = tile0 + (int64_t)threadIdx.x * 8;
+  float4 a0, a1, b0, b1, d0, d1;
+  int4 c0, c1;
+  unsigned long long mk8 = 0x0101010101010101ull;
+  if (whole) {
+    a0 = *reinterpret_cast<const float4*>(logp + t0f);
+    a1 = *reinterpret_cast<const float4*>(logp + t0f + 4);
+    b0 = *reinterpret_cast<const float4*>(old_logp + t0f);
+    b1 = *reinterpret_cast<const float4*>(old_logp + t0f + 4);
+    c0 = *reinterpret_cast<const int4*>(targets + t0f);
+    c1 = *reinterpret_cast<const int4*>(targets + t0f + 4);
+    if (ref_logp) {
+      d0 = *reinterpret_cast<const float4*>(ref_logp + t0f);
+      d1 = *reinterpret_cast<const float4*>(ref_logp + t0f + 4);
+    } else {
+      d0 = a0;
+      d1 = a1;
+    }
+    if (mask) mk8 = *reinterpret_cast<const unsigned long long*>(mask + t0f);
+  }
+  const CuSlice cs = load_cu_slice(cu, tile_r, s_cu);
   const double n_scored = (double)cnt->n_scored;
   const double n_kept = (double)cnt->n_kept;
   // gradient scale shared by every token of the batch
@@ -278,38 +301,20 @@ k_token_loss(const float* __restrict__ logp, const float* __restrict__ old_logp,
   float acc_pg = 0.f, acc_kl = 0.f;     // 8 terms per thread in fp32, fp64 from there on
   unsigned int n_clip = 0;
 
-  if (cs.s != nullptr && tile0 + kLossTile <= T) {
+  if (cs.s != nullptr && whole) {
     // ---- fast path: whole tile, cu slice in shared memory.  8 consecutive tokens per thread,
     // tile-relative 32-bit indices, one binary search per thread then a forward walk. ----
-    const int tl0 = threadIdx.x * 8;
-    const int64_t t0 = tile0 + tl0;
+    const int64_t t0 = t0f;
     float lp[8], ol[8], rf[8], gout[8];
     int32_t y[8];
-    {
-      const float4 a0 = *reinterpret_cast<const float4*>(logp + t0);
-      const float4 a1 = *reinterpret_cast<const float4*>(logp + t0 + 4);
-      const float4 b0 = *reinterpret_cast<const float4*>(old_logp + t0);
-      const float4 b1 = *reinterpret_cast<const float4*>(old_logp + t0 + 4);
-      const int4 c0 = *reinterpret_cast<const int4*>(targets + t0);
-      const int4 c1 = *reinterpret_cast<const int4*>(targets + t0 + 4);
-      lp[0] = a0.x; lp[1] = a0.y; lp[2] = a0.z; lp[3] = a0.w;
-      lp[4] = a1.x; lp[5] = a1.y; lp[6] = a1.z; lp[7] = a1.w;
-      ol[0] = b0.x; ol[1] = b0.y; ol[2] = b0.z; ol[3] = b0.w;
-      ol[4] = b1.x; ol[5] = b1.y; ol[6] = b1.z; ol[7] = b1.w;
-      y[0] = c0.x; y[1] = c0.y; y[2] = c0.z; y[3] = c0.w;
-      y[4] = c1.x; y[5] = c1.y; y[6] = c1.z; y[7] = c1.w;
-      if (ref_logp) {
-        const float4 d0 = *reinterpret_cast<const float4*>(ref_logp + t0);
-        const float4 d1 = *reinterpret_cast<const float4*>(ref_logp + t0 + 4);
-        rf[0] = d0.x; rf[1] = d0.y; rf[2] = d0.z; rf[3] = d0.w;
-        rf[4] = d1.x; rf[5] = d1.y; rf[6] = d1.z; rf[7] = d1.w;
-      } else {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) rf[i] = lp[i];
-      }
-    }
-    unsigned long long mk8 = 0x0101010101010101ull;
-    if (mask) mk8 = *reinterpret_cast<const unsigned long long*>(mask + t0);
+    lp[0] = a0.x; lp[1] = a0.y; lp[2] = a0.z; lp[3] = a0.w;
+    lp[4] = a1.x; lp[5] = a1.y; lp[6] = a1.z; lp[7] = a1.w;
+    ol[0] = b0.x; ol[1] = b0.y; ol[2] = b0.z; ol[3] = b0.w;
+    ol[4] = b1.x; ol[5] = b1.y; ol[6] = b1.z; ol[7] = b1.w;
+    rf[0] = d0.x; rf[1] = d0.y; rf[2] = d0.z; rf[3] = d0.w;
+    rf[4] = d1.x; rf[5] = d1.y; rf[6] = d1.z; rf[7] = d1.w;
+    y[0] = c0.x; y[1] = c0.y; y[2] = c0.z; y[3] = c0.w;
+    y[4] = c1.x; y[5] = c1.y; y[6] = c1.z; y[7] = c1.w;
     // slice-relative response index: largest r with cu[r0 + r] <= t0
     const int32_t* sc_ = cs.s;
     const int32_t tq = (int32_t)t0;

@@ -1,7 +1,11 @@
 """Data-parallel plumbing for the scoring path: whole groups per rank, W replicated
 ("use all GPUs for training and rollout log probability calculations"; DP at
-PAPER.md:86).  No data-path collective: ranks only agree on timing and token counts.
-Works on any torch.distributed backend (nccl on GPUs, gloo in the CPU tests)."""
+PAPER.md:86).  Scoring (stage 3) needs no data-path collective: ranks only agree on timing and
+token counts.  Training (stage 4) across ranks needs exactly two exchanges: the
+global scored-token count before the backward, and an all-reduce of dW (and of the loss scalars)
+after it -- `global_grad_scale` and `all_reduce_mean` below.  dH stays local (each rank owns its
+tokens); like dW before the mean it is world x the global gradient, which the trunk's own
+gradient averaging over ranks divides out.  Works on any torch.distributed backend (nccl on GPUs, gloo in the CPU tests)."""
 from __future__ import annotations
 
 import os
@@ -46,3 +50,27 @@ def reduce_step_stats(elapsed_ms: float, units: float) -> Tuple[float, float]:
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     dist.all_reduce(u, op=dist.ReduceOp.SUM)
     return float(t.item()), float(u.item())
+
+
+def global_grad_scale(n_scored_local: float) -> float:
+    """`grad_loss` to pass to gc_grpo_loss_bwd on this rank so that the MEAN over ranks of the
+    local dW (and of the local loss) is the gradient (loss) of the global token-mean objective
+    sum_all m l / sum_all m:  local dW_r = grad_loss_r / n_r * S_r with S_r the rank's un-normalised
+    sum, so grad_loss_r = world * n_r / N makes mean_r dW_r = (1/N) sum_r S_r.  One all-reduce of a
+    scalar.  (Equal per-rank counts give 1.0.)"""
+    if not is_dist():
+        return 1.0
+    n = torch.tensor([float(n_scored_local)], dtype=torch.float64, device=_device())
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    total = float(n.item())
+    return dist.get_world_size() * float(n_scored_local) / total if total > 0 else 0.0
+
+
+def all_reduce_mean(*tensors: torch.Tensor) -> None:
+    """In-place mean over ranks (dW [V,D] fp32: 2-8 GB, NCCL over NVLink on GPUs; loss scalars)."""
+    if not is_dist():
+        return
+    w = dist.get_world_size()
+    for t in tensors:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        t.div_(w)

@@ -51,6 +51,83 @@ def test_two_rank_sharding_and_reductions():
         assert tok_sum == T                              # every token counted once
 
 
+def _train_worker(rank, world, port, out):
+    """Each rank runs the ORACLE on its shard (no GPU here); what is under test is the combination
+    rule of dp.global_grad_scale + dp.all_reduce_mean against the oracle on the whole batch."""
+    import numpy as np
+    import oracle as O
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank),
+                      WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        full = _make_train_case()
+        sh = _shard_case(full, dp.shard_groups(full["G"], world, rank))
+        n_local = int(sh["scored"].sum())
+        gl = dp.global_grad_scale(n_local)
+        r = O.grpo_forward_backward(sh["H"], full["W"], sh["y"], sh["mask"], 1.0, sh["cu"], sh["adv"],
+                                    sh["old"], sh["ref"], 0.2, 0.2, 0.04, grad_loss=gl)
+        dW = torch.from_numpy(r["dW"].copy())
+        loss = torch.tensor([r["loss"] * gl], dtype=torch.float64)
+        dp.all_reduce_mean(dW, loss)
+        out.put((rank, gl, dW.numpy(), float(loss.item()), r["dH"], sh["tok"]))
+    finally:
+        dist.destroy_process_group()
+
+
+def _make_train_case():
+    import numpy as np
+    import oracle as O
+    r = np.random.default_rng(0)
+    G, gs = 4, 2
+    L = np.array([5, 9, 3, 14, 7, 2, 11, 6])             # unequal shards: 31 vs 26 tokens
+    cu = np.concatenate([[0], np.cumsum(L)]).astype(np.int32)
+    T, D, V = int(cu[-1]), 16, 24
+    H = r.normal(size=(T, D)); W = r.normal(size=(V, D)) * 0.3
+    y = r.integers(0, V, T).astype(np.int32)
+    mask = (r.random(T) < 0.8).astype(np.uint8)
+    rewards = r.random(G * gs).astype(np.float32)
+    adv, _ = O.grpo_advantages(rewards, np.arange(0, G * gs + 1, gs, dtype=np.int32), 1e-6)
+    lp = O.token_logprobs(H, W, y, None, 1.0)[0]
+    old = lp + 0.05 * r.normal(size=T); ref = lp + 0.1 * r.normal(size=T)
+    return dict(G=G, gs=gs, cu=cu, H=H, W=W, y=y, mask=mask, adv=adv, old=old, ref=ref, T=T)
+
+
+def _shard_case(c, groups):
+    import numpy as np
+    resp = [g * c["gs"] + i for g in groups for i in range(c["gs"])]
+    tok = np.concatenate([np.arange(c["cu"][i], c["cu"][i + 1]) for i in resp])
+    L = [c["cu"][i + 1] - c["cu"][i] for i in resp]
+    cu = np.concatenate([[0], np.cumsum(L)]).astype(np.int32)
+    scored = (c["mask"][tok] != 0) & (c["y"][tok] >= 0)
+    return dict(H=c["H"][tok], y=c["y"][tok], mask=c["mask"][tok], cu=cu, adv=c["adv"][resp],
+                old=c["old"][tok], ref=c["ref"][tok], scored=scored, tok=tok)
+
+
+def test_two_rank_training_exchange_matches_global_objective():
+    import numpy as np
+    import oracle as O
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_train_worker, args=(r, world, port, q)) for r in range(world)]
+    [p.start() for p in procs]
+    res = sorted((q.get(timeout=180) for _ in range(world)), key=lambda x: x[0])
+    [p.join(timeout=60) for p in procs]
+    assert all(p.exitcode == 0 for p in procs)
+    c = _make_train_case()
+    g = O.grpo_forward_backward(c["H"], c["W"], c["y"], c["mask"], 1.0, c["cu"], c["adv"], c["old"],
+                                c["ref"], 0.2, 0.2, 0.04)
+    assert abs(sum(x[1] for x in res) - world) < 1e-12     # the scales average to 1
+    assert res[0][1] != res[1][1]                          # unequal shards: the scaling matters
+    for rank, gl, dW, loss, dH, tok in res:
+        assert np.allclose(dW, g["dW"], rtol=1e-12, atol=1e-15)     # both ranks hold the global dW
+        assert abs(loss - g["loss"]) < 1e-13
+        # dH needs no exchange: it is the gradient of this rank's term of the rank-MEAN, i.e. world x
+        # the global gradient, which the trunk's own gradient averaging over ranks divides out
+        assert np.allclose(dH / world, g["dH"][tok], rtol=1e-12, atol=1e-15)
+
+
 def test_shard_groups_balance():
     for n in (0, 1, 7, 16, 33):
         for world in (1, 2, 3, 8):

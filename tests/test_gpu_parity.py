@@ -348,3 +348,40 @@ def test_bf16_empty_and_all_masked(B):
     lp, en, ls = B.gc_token_logprobs(H0, b.W, torch.empty(0, dtype=torch.int32, device="cuda"))
     assert lp.numel() == 0
     assert B.gc_validate_targets(b.y, None, 512) == 0 and B.gc_validate_targets(b.y, None, 1) > 0
+
+
+def test_host_buffer_entry_point_matches_device_path(B):
+    """gc_token_logprobs_host (the end-to-end entry: pinned host inputs, host outputs) computes
+    exactly what gc_token_logprobs computes on device-resident copies, with and without a mask."""
+    w = I.reduced(I.CONFIGS[1], D=256, V=2048 + 24, groups=2, group_size=2, seq_len=75)
+    b = make_batch(w, seed=4, device="cuda")
+    mask_np = I.random_mask(b.T, 0.7, 4)
+    for m in (None, mask_np):
+        md = None if m is None else torch.from_numpy(m).cuda()
+        lp_d, en_d, _ = B.gc_token_logprobs(b.H, b.W, b.y, md, w.tau)
+        Hh = b.H.cpu().pin_memory()
+        yh = b.y.cpu().pin_memory()
+        mh = None if m is None else torch.from_numpy(m).pin_memory()
+        lph = torch.empty(b.T, dtype=torch.float32).pin_memory()
+        enh = torch.empty(b.T, dtype=torch.float32).pin_memory()
+        B.gc_token_logprobs_host(Hh, b.W, yh, mh, w.tau, logp_host=lph, entropy_host=enh)
+        torch.cuda.synchronize()
+        assert torch.equal(lph, lp_d.cpu()) and torch.equal(enh, en_d.cpu())
+    lp_o, en_o, _ = O.token_logprobs(to_f64(b.H), to_f64(b.W), b.y_np, mask_np, w.tau)
+    assert np.abs(lph.numpy() - lp_o).max() <= TOL_LOGP_BF16
+
+
+def test_kernel_timing_counts_the_contraction_launches(B):
+    """gc_kernel_timing_*: one record per contraction launch, by kind, positive durations, and off
+    again afterwards."""
+    w = I.reduced(I.CONFIGS[2], D=256, V=2048, groups=2, group_size=2, seq_len=160, prompt_len=32)
+    b = make_batch(w, seed=2, device="cuda")
+    B.gc_kernel_timing_begin()
+    run_gpu(B, b, chunk_tokens=256)
+    k = B.gc_kernel_timing_end()
+    n_chunks = -(-b.T // 256)
+    assert k["fwd_stats"][1] == 1 and k["recompute_ds"][1] == n_chunks
+    assert k["dh"][1] == n_chunks and k["dw"][1] == n_chunks
+    assert all(ms > 0 for ms, n in k.values() if n)
+    run_gpu(B, b)
+    assert all(n == 0 for _, n in B.gc_kernel_timing_end().values())

@@ -27,14 +27,20 @@ constexpr int kABytes = BM_CTA * BK * 2;   // 16 KB
 // accumulators belong to one 256 x 512 output tile whose two halves share every A stage, which
 // cuts the L2 -> smem operand traffic per flop by a quarter; the epilogue then cannot overlap
 // the next tile's MMAs, so it is for contractions with a very long K (dH: K = V).
-template <int CG, int NSUB = 1> struct Cfg {
+// kEpiSmem = staging bytes the epilogue functor wants per CTA; the operand ring takes the stages
+// that fit in what is left of the 227 KB (7 x 32 KB with no staging, 5 with the fp32 TMA-store
+// epilogue's 64 KB, 4 x 48 KB for dual-N).
+template <int CG, int NSUB = 1, int kEpiSmem = 0> struct Cfg {
   static_assert(NSUB == 1 || (NSUB == 2 && CG == 2), "dual-N needs the CTA pair");
   static constexpr int kBRows = BN / CG;                 // B rows of one sub-tile staged by one CTA
   static constexpr int kBBytes = kBRows * BK * 2;
   static constexpr int kStageBytes = kABytes + NSUB * kBBytes;  // 32 / 48 KB (CG=2), 48 KB (CG=1)
-  static constexpr int kStages = CG == 2 ? (NSUB == 2 ? 4 : 6) : 4;
   static constexpr int kBarBytes = 1024;   // barriers + item ring (keeps what follows 1024-aligned)
-  static constexpr int kSmemBase = kStages * kStageBytes + 1024 /*align slack*/ + kBarBytes;
+  static constexpr int kFit = (227 * 1024 - 1024 /*align slack*/ - kBarBytes - kEpiSmem) / kStageBytes;
+  static constexpr int kStages = kFit > 8 ? 8 : kFit;
+  static_assert(kStages >= 2, "operand ring too shallow");
+  static constexpr int kSmemBase = kStages * kStageBytes + 1024 + kBarBytes;
+  static constexpr int kSmemBytes = kSmemBase + kEpiSmem;
 };
 
 // Work schedule.  An item is (M tile, run of N tiles).  Items are handed out in index order to
@@ -136,7 +142,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
           const Sched s, const __grid_constant__ typename Epi::Params ep) {
   static_assert(PPC == 1 || (PPC == 2 && CG == 2), "pairs per cluster");
   constexpr int CL = CG * PPC;                 // CTAs per cluster
-  using C = Cfg<CG, NSUB>;
+  using C = Cfg<CG, NSUB, 4 * Epi::kWarpSmem>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + C::kStages * C::kStageBytes;
@@ -146,12 +152,14 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
   auto tfull_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + i); };
   auto tempty_bar = [&](int i) { return bar_base + 8u * (2 * C::kStages + 2 + i); };
   const uint32_t tmem_slot = bar_base + 8u * (2 * C::kStages + 4);
-  // item ring (dynamic schedule): sfull[4] @136, sempty[4] @168 (leader CTA's are used), item[4] @200
+  // item ring (dynamic schedule), after the pipeline barriers: sfull[4], sempty[4] (the cluster
+  // leader's are used), item[4]
   constexpr int kSlots = 4;
-  auto sfull_bar = [&](int i) { return bar_base + 136u + 8u * i; };
-  auto sempty_bar = [&](int i) { return bar_base + 168u + 8u * i; };
-  auto sitem = [&](int i) { return bar_base + 200u + 4u * i; };
-  static_assert(8 * (2 * C::kStages + 4) + 4 <= 136, "barrier area overlap");
+  constexpr uint32_t kRing = 8u * (2 * C::kStages + 4) + 8u;
+  auto sfull_bar = [&](int i) { return bar_base + kRing + 8u * i; };
+  auto sempty_bar = [&](int i) { return bar_base + kRing + 32u + 8u * i; };
+  auto sitem = [&](int i) { return bar_base + kRing + 64u + 4u * i; };
+  static_assert(kRing + 80u <= (uint32_t)C::kBarBytes, "barrier area overflow");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = CL > 1 ? ptx::cluster_ctarank() : 0u;   // rank in the cluster
@@ -546,7 +554,7 @@ int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& 
                    const typename Epi::Params& ep, cudaStream_t st) {
   auto kern = k_tc_gemm<CG, A_MN, B_MN, Epi, NSUB, PPC>;
   constexpr int CL = CG * PPC;
-  constexpr int kSmemBytes = Cfg<CG, NSUB>::kSmemBase + 4 * Epi::kWarpSmem;
+  constexpr int kSmemBytes = Cfg<CG, NSUB, 4 * Epi::kWarpSmem>::kSmemBytes;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
   static int clusters = 0;                       // per instantiation
   if (clusters == 0) {

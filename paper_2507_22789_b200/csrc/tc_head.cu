@@ -294,7 +294,7 @@ struct EpiStoreBf16 {
 
 // ---------------------------------------------------------------------------------------------
 // Epilogue a12 (and the debug GEMM): fp32 tile store, or accumulate, through TMA.  Each epilogue
-// warp stages its 32 rows x 32 columns (4 KB, 128-byte-swizzled, double-buffered) in shared memory
+// warp stages its 32 rows x 32 columns (4 KB, 128-byte-swizzled, 4 buffers in rotation) in shared memory
 // and one lane issues a bulk tensor store -- or, when accumulating, a bulk tensor REDUCE-ADD, so
 // the read-modify-write of dW happens at the L2 and the old values never travel to the SM.  Every
 // dW element receives exactly one add per launch and launches are stream-ordered, so the result
@@ -303,7 +303,8 @@ struct EpiStoreBf16 {
 // tensor-pipe activity, profiles/.)
 // ---------------------------------------------------------------------------------------------
 struct EpiStoreF32 {
-  static constexpr int kWarpSmem = 2 * 4096;
+  static constexpr int kBufs = 4;                // 4 KB staging buffers per warp
+  static constexpr int kWarpSmem = kBufs * 4096;
   struct alignas(64) Params {
     CUtensorMap tm;           // fp32 [M, N] (row stride ldo), box {32 columns, 32 rows}, swizzle 128B
     int64_t N;
@@ -321,9 +322,9 @@ struct EpiStoreF32 {
     if (col0 >= p.N) return;                       // uniform over the warp
     const int lane = threadIdx.x & 31;
     const uint32_t base = st.smem + st.buf * 4096u;
-    st.buf ^= 1u;
-    // the store issued two chunks ago (same buffer) must have finished reading it
-    if (lane == 0) ptx::bulk_wait_group_read<1>();
+    st.buf = (st.buf + 1u) % (uint32_t)kBufs;
+    // the store issued kBufs chunks ago (same buffer) must have finished reading it
+    if (lane == 0) ptx::bulk_wait_group_read<kBufs - 1>();
     __syncwarp();
     const uint32_t rbase = base + (uint32_t)lane * 128u;
 #pragma unroll

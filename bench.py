@@ -430,6 +430,42 @@ def hbm_kernels(B, device, peaks):
     return out
 
 
+def library_baseline(b, steps=20):
+    """Context only (not the product path, not the oracle): the same forward scoring the way the
+    paper's own stack does it (PyTorch / Megatron-Core library calls) -- one cuBLAS
+    GEMM that materialises the [T,V] logits in bf16, then fp32 log_softmax, gather and entropy
+    in row blocks so the fp32 intermediates fit.  Reported next to the fused kernel."""
+    w = b.w
+    def gemm():
+        return torch.matmul(b.H, b.W.t())
+    def full():
+        z = torch.matmul(b.H, b.W.t())
+        lp = torch.empty(b.T, dtype=torch.float32, device=z.device)
+        en = torch.empty(b.T, dtype=torch.float32, device=z.device)
+        for r0 in range(0, b.T, 2048):
+            zz = z[r0:r0 + 2048].float() / w.tau
+            ls = torch.log_softmax(zz, dim=-1)
+            lp[r0:r0 + 2048] = ls.gather(1, b.y[r0:r0 + 2048].long().clamp_min(0)[:, None])[:, 0]
+            en[r0:r0 + 2048] = -(ls.exp() * ls).sum(-1)
+        return lp, en
+    out = {}
+    for name, fn in (("cublas_gemm_only", gemm), ("torch_matmul_logsoftmax_gather_entropy", full)):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        out[name] = {"ms_per_step": ms, "scored_tokens_per_s": b.n_scored / (ms * 1e-3),
+                     "tflops": 2.0 * b.T * w.D * w.V / (ms * 1e-3) / 1e12}
+    out["logits_bytes_materialised"] = 2 * b.T * w.V
+    return out
+
+
 def e2e_measure(B, b: DeviceBatch, steps, warmup):
     """Same metric through the C-ABI call with HOST buffers: per step H2D of H / targets / mask
     from pinned memory, the kernels, D2H of logp + entropy, all inside the timed region."""
@@ -522,6 +558,7 @@ def main():
                               "ms_per_step": ms, "pass": "fwd (gc_token_logprobs_host)"}
             out["cpu_baseline"] = cpu_baseline(w, 256 if w.D * w.V > 1e8 else 1 << 30)
             if args.workload == "cfg1":
+                out["library_baseline"] = library_baseline(b)
                 out["hbm_kernels"] = hbm_kernels(B, torch.device("cuda", local_rank), peaks)
                 # the metric's second half: fwd+bwd on the 8B-class training micro-batch
                 del b

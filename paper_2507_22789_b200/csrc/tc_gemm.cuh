@@ -556,7 +556,11 @@ int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& 
   constexpr int CL = CG * PPC;
   constexpr int kSmemBytes = Cfg<CG, NSUB, 4 * Epi::kWarpSmem>::kSmemBytes;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
-  static int clusters = 0;                       // per instantiation
+  // per instantiation and device: the smem opt-in is a per-device function attribute
+  static int clusters_by_dev[64] = {};
+  int dev = 0;
+  GC_CUDA_TRY(cudaGetDevice(&dev));
+  int& clusters = clusters_by_dev[dev & 63];
   if (clusters == 0) {
     GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     clusters = max_active_clusters(kern, CL, kSmemBytes);

@@ -150,6 +150,28 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
                      int accumulate_dW, int64_t chunk_tokens,
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- stage 4 backward fused with its data-parallel exchange (training
+ * across ranks needs "one all-reduce (or reduce-scatter ...) of fp32 dW [V,D]").  Same computation
+ * as gc_grpo_loss_bwd, but the dW contraction's epilogue TMA-reduce-adds every tile straight into
+ * the shard of the rank that owns its vocab rows, so the reduce-scatter rides on the contraction
+ * and no full-size local dW exists.  dW_shards_host: HOST array of `world` (<= 8) DEVICE pointers;
+ * entry r is rank r's shard, fp32 [shard_rows, D] with row stride ld_shard, holding vocab rows
+ * [r shard_rows, (r+1) shard_rows) -- this rank's own buffer or a peer-mapped one (CUDA IPC /
+ * cudaDeviceEnablePeerAccess; NVLink carries the adds).  shard_rows % 32 == 0, shard_rows * world
+ * >= V.  Protocol: every rank zeroes its own shard, all ranks synchronise, every rank runs this
+ * call, all ranks synchronise again; each shard then holds the sum over ranks of those rows of dW
+ * (divide by `world` or fold 1/world into grad_loss for a mean).  Adds from different ranks meet
+ * in no fixed order: reruns agree to rounding, not bit for bit.  GC_BF16 only. */
+int gc_grpo_loss_bwd_reduce_scatter(
+    const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+    const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V, float temperature,
+    const int32_t* cu_seqlens, int32_t R, const float* adv,
+    const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi, float beta, int agg,
+    const float* logp, const float* lse, float grad_loss,
+    void* dH, int64_t lddH, float* const* dW_shards_host, int32_t world, int64_t shard_rows,
+    int64_t ld_shard, int64_t chunk_tokens,
+    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- helpers ---- */
 /* Debug: synchronises the stream; *n_bad_host = number of scored tokens with target >= V. */
 int gc_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,

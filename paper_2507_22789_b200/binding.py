@@ -26,6 +26,7 @@ EXPORTS = [
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
     "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
+    "gc_grpo_loss_bwd_reduce_scatter",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
@@ -58,6 +59,8 @@ def _load() -> C.CDLL:
     lib.gc_grpo_loss_fwd.argtypes = head + loss + [vp, vp, vp, vp, vp, sz, vp]
     lib.gc_grpo_loss_bwd.argtypes = head + loss + [vp, vp, f32, vp, i64, vp, i64, ci, ci, i64,
                                                    vp, sz, vp]
+    lib.gc_grpo_loss_bwd_reduce_scatter.argtypes = head + loss + [vp, vp, f32, vp, i64, C.POINTER(vp),
+                                                                  i32, i64, i64, i64, vp, sz, vp]
     lib.gc_validate_targets.argtypes = [vp, vp, i64, i64, C.POINTER(i64), vp]
     lib.gc_compact_rows.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, vp, vp, vp, sz, vp]
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
@@ -426,3 +429,26 @@ def gc_value_head_bwd(H, w, g):
                                   _ptr(g), T, D, _ptr(dH), D, _ptr(dw), _ptr(db), _ptr(ws),
                                   ws.numel(), _stream()))
     return dH, dw, db
+
+
+def gc_grpo_loss_bwd_reduce_scatter(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp,
+                                    ref_logp, logp, lse, shard_ptrs, shard_rows, ld_shard=None,
+                                    clip_lo=0.2, clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN,
+                                    grad_loss=1.0, *, dH=None, chunk_tokens=0):
+    """Backward whose dW tiles are TMA-reduce-added into the owning rank's shard.  shard_ptrs: list of
+    `world` device pointers (ints; own tensor.data_ptr() or peer-mapped), shard r = fp32
+    [shard_rows, D] holding vocab rows [r*shard_rows, (r+1)*shard_rows).  -> dH."""
+    args, T, D, V, dt = _head_args(H, W, targets, mask, temperature, False)
+    dev = H.device
+    if dH is None:
+        dH = torch.empty(T, D, dtype=H.dtype, device=dev)
+    world = len(shard_ptrs)
+    arr = (C.c_void_p * world)(*[C.c_void_p(int(p)) for p in shard_ptrs])
+    nb = workspace_bytes(GC_OP_LOSS_BWD, T, D, V, dt, chunk_tokens)
+    ws = workspace(nb, dev)
+    _check(_lib.gc_grpo_loss_bwd_reduce_scatter(
+        *args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg),
+        _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH), dH.stride(0) if T > 0 else D, arr, world,
+        int(shard_rows), int(ld_shard if ld_shard is not None else D), int(chunk_tokens), _ptr(ws),
+        ws.numel(), _stream()))
+    return dH

@@ -327,21 +327,45 @@ int gc_grpo_loss_fwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
                             workspace_bytes - align_up(fwd_bytes, 256), cuda_stream);
 }
 
-int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
-                     const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
-                     float temperature, const int32_t* cu_seqlens, int32_t R, const float* adv,
-                     const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
-                     float beta, int agg, const float* logp, const float* lse, float grad_loss,
-                     void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
-                     int accumulate_dW, int64_t chunk_tokens, void* workspace,
-                     size_t workspace_bytes, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+// where dW goes: a local [V, D] buffer, or (shards != NULL) the per-rank shards of a fused
+// reduce-scatter (tc_dw_reduce_scatter)
+struct DwSink {
+  void* dW; int64_t lddW; int accumulate;
+  float* const* shards; int world; int64_t shard_rows;
+};
+
+int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                  const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                  float temperature, const int32_t* cu_seqlens, int32_t R, const float* adv,
+                  const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
+                  float beta, int agg, const float* logp, const float* lse, float grad_loss,
+                  void* dH, int64_t lddH, const DwSink& sink, int64_t chunk_tokens, void* workspace,
+                  size_t workspace_bytes, void* cuda_stream) {
+  void* const dW = sink.dW;
+  const int64_t lddW = sink.lddW;
+  const int accumulate_dW = sink.accumulate;
   GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
   GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
-  if (dW_dtype != GC_F32) return GC_ERR_DTYPE;
-  if (!dW || (T > 0 && (!dH || !logp || !lse))) return GC_ERR_NULL;
-  if (lddH < D || lddW < D) return GC_ERR_SHAPE;
-  if (dtype == GC_BF16 && (lddH % 8 != 0 || lddW % 4 != 0 || !aligned16(dH) || !aligned16(dW)))
-    return GC_ERR_ALIGN;
+  if (sink.shards) {
+    if (dtype != GC_BF16) return GC_ERR_DTYPE;
+    if (sink.world < 1 || sink.world > 8 || sink.shard_rows <= 0 || sink.shard_rows % 32 != 0)
+      return GC_ERR_ARG;
+    if (sink.shard_rows * sink.world < V || lddW < D || lddW % 4 != 0) return GC_ERR_SHAPE;
+    for (int r = 0; r < sink.world; ++r) {
+      if (!sink.shards[r]) return GC_ERR_NULL;
+      if (!aligned16(sink.shards[r])) return GC_ERR_ALIGN;
+    }
+  } else {
+    if (!dW) return GC_ERR_NULL;
+    if (lddW < D) return GC_ERR_SHAPE;
+    if (dtype == GC_BF16 && (lddW % 4 != 0 || !aligned16(dW))) return GC_ERR_ALIGN;
+  }
+  if (T > 0 && (!dH || !logp || !lse)) return GC_ERR_NULL;
+  if (lddH < D) return GC_ERR_SHAPE;
+  if (dtype == GC_BF16 && (lddH % 8 != 0 || !aligned16(dH))) return GC_ERR_ALIGN;
   if (!aligned16(logp) || !aligned16(old_logp) || !aligned16(ref_logp) || !aligned16(targets) ||
       (reinterpret_cast<uintptr_t>(mask) & 3))
     return GC_ERR_ALIGN;
@@ -351,7 +375,7 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   GC_TRY(check_arch());
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (T == 0) {
-    if (!accumulate_dW)
+    if (!sink.shards && !accumulate_dW)
       GC_CUDA_TRY(cudaMemset2DAsync(dW, (size_t)lddW * 4, 0, (size_t)D * 4, (size_t)V, st));
     return GC_OK;
   }
@@ -407,12 +431,51 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
     GC_TRY(tc_dh(w.dS, ldS, rows_cap, n_static, W, ldW, D, V, rows ? rows + row0 : nullptr, n_rows,
                  row0, dH, lddH, w.counters + ci + 1, st));
     // a12: dW accumulates over chunks in fp32
-    GC_TRY(tc_dw(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
-                 static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0,
-                 w.counters + ci + 2, st));
+    if (sink.shards)
+      GC_TRY(tc_dw_reduce_scatter(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
+                                  sink.shards, sink.world, sink.shard_rows, lddW,
+                                  w.counters + ci + 2, st));
+    else
+      GC_TRY(tc_dw(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
+                   static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0,
+                   w.counters + ci + 2, st));
     ci += 3;
   }
   return GC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                     const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D, int64_t V,
+                     float temperature, const int32_t* cu_seqlens, int32_t R, const float* adv,
+                     const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
+                     float beta, int agg, const float* logp, const float* lse, float grad_loss,
+                     void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
+                     int accumulate_dW, int64_t chunk_tokens, void* workspace,
+                     size_t workspace_bytes, void* cuda_stream) {
+  if (dW_dtype != GC_F32) return GC_ERR_DTYPE;
+  const DwSink sink{dW, lddW, accumulate_dW, nullptr, 0, 0};
+  return loss_bwd_impl(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, cu_seqlens, R, adv,
+                       old_logp, ref_logp, clip_lo, clip_hi, beta, agg, logp, lse, grad_loss, dH, lddH,
+                       sink, chunk_tokens, workspace, workspace_bytes, cuda_stream);
+}
+
+int gc_grpo_loss_bwd_reduce_scatter(
+    const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype, const int32_t* targets,
+    const uint8_t* mask, int64_t T, int64_t D, int64_t V, float temperature,
+    const int32_t* cu_seqlens, int32_t R, const float* adv, const float* old_logp,
+    const float* ref_logp, float clip_lo, float clip_hi, float beta, int agg, const float* logp,
+    const float* lse, float grad_loss, void* dH, int64_t lddH, float* const* dW_shards_host,
+    int32_t world, int64_t shard_rows, int64_t ld_shard, int64_t chunk_tokens, void* workspace,
+    size_t workspace_bytes, void* cuda_stream) {
+  if (!dW_shards_host) return GC_ERR_NULL;
+  const DwSink sink{nullptr, ld_shard, 1, dW_shards_host, world, shard_rows};
+  return loss_bwd_impl(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, cu_seqlens, R, adv,
+                       old_logp, ref_logp, clip_lo, clip_hi, beta, agg, logp, lse, grad_loss, dH, lddH,
+                       sink, chunk_tokens, workspace, workspace_bytes, cuda_stream);
 }
 
 int gc_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,

@@ -149,6 +149,10 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
 int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const void* Hs,
           int64_t ldH, int64_t D, int64_t V, const int32_t* n_rows_dev, int64_t row0, float* dW,
           int64_t lddW, int accumulate, uint32_t* counter, cudaStream_t st);
+int tc_dw_reduce_scatter(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static,
+                         const void* Hs, int64_t ldH, int64_t D, int64_t V,
+                         const int32_t* n_rows_dev, int64_t row0, float* const* shards, int world,
+                         int64_t shard_rows, int64_t ld_shard, uint32_t* counter, cudaStream_t st);
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
                   int cta_group, int dynamic_schedule, int dual_n, int cluster4, cudaStream_t st);

@@ -360,6 +360,63 @@ static int make_f32_out_tmap(CUtensorMap* m, float* out, int64_t rows, int64_t c
   return r == CUDA_SUCCESS ? GC_OK : GC_ERR_CUDA;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Epilogue a12 fused with its data-parallel exchange ("one all-reduce (or
+// reduce-scatter ...) of fp32 dW"): instead of accumulating into a local dW and calling a
+// collective afterwards, every tile is TMA-reduce-added straight into the shard of the rank that
+// OWNS its vocab rows -- a peer-mapped buffer reached over NVLink (or this rank's own memory) --
+// so the reduce-scatter overlaps the contraction tile by tile and no full-size local dW exists.
+// Shard r holds vocab rows [r shard_rows, (r+1) shard_rows); shard_rows % 32 == 0 so that a warp's
+// 32-row slab never straddles two owners.  All ranks add into zero-initialised shards; after a
+// barrier each rank's shard is the sum over ranks.  (Adds from different ranks arrive in no fixed
+// order: across ranks the fp32 sum is reproducible only up to rounding, as with any NCCL ring.)
+// ---------------------------------------------------------------------------------------------
+constexpr int kMaxShards = 8;
+struct EpiReduceScatterF32 {
+  static constexpr int kBufs = 4;
+  static constexpr int kWarpSmem = kBufs * 4096;
+  struct alignas(64) Params {
+    CUtensorMap tm[kMaxShards];   // shard r: fp32 [rows of shard r, N], box {32, 32}, swizzle 128B
+    int64_t N;
+    int64_t shard_rows;
+    int world;
+  };
+  struct State { uint32_t smem; uint32_t buf; };
+  static __device__ __forceinline__ void setup(State& st, const Params&, uint32_t warp_smem) {
+    st.smem = warp_smem;
+    st.buf = 0;
+  }
+  static __device__ __forceinline__ void item_begin(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void tile_prefetch(const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void chunk(State& st, const Params& p, int64_t row, bool,
+                                               int64_t col0, const float (&x)[32]) {
+    if (col0 >= p.N) return;
+    const int lane = threadIdx.x & 31;
+    const uint32_t base = st.smem + st.buf * 4096u;
+    st.buf = (st.buf + 1u) % (uint32_t)kBufs;
+    if (lane == 0) ptx::bulk_wait_group_read<kBufs - 1>();
+    __syncwarp();
+    const uint32_t rbase = base + (uint32_t)lane * 128u;
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      ptx::st_shared_v4(rbase + (uint32_t)((q ^ (lane & 7)) << 4), x[4 * q], x[4 * q + 1],
+                        x[4 * q + 2], x[4 * q + 3]);
+    ptx::fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      const int64_t owner = row / p.shard_rows;            // `row` = first row of the warp's slab
+      if (owner < p.world)
+        ptx::tma_reduce_add_2d(&p.tm[owner], base, (int32_t)col0,
+                               (int32_t)(row - owner * p.shard_rows));
+      ptx::bulk_commit_group();
+    }
+  }
+  static __device__ __forceinline__ void item_end(State&, const Params&, int64_t, bool, int64_t) {}
+  static __device__ __forceinline__ void finish(State&, const Params&) {
+    if ((threadIdx.x & 31) == 0) ptx::bulk_wait_group_read<0>();
+  }
+};
+
 // L2 budget of the forward / recompute schedule.  Measured (profiles/): an H band plus the W tiles
 // in flight stay resident up to ~50 MB, 60 MB and more thrash (DRAM reads x2.5 .. x7) -- about
 // half of the 126 MB, consistent with each die's L2 also holding the lines its SMs fetch from the
@@ -611,6 +668,39 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   GC_EXP_OVERRIDE(s, "DW");
   KernelTimer kt(GC_KERNEL_DW, st);
   return tc::launch_tc_gemm<2, true, true, EpiStoreF32, 1, kPpc>(ta, tb, s, ep, st);
+}
+
+int tc_dw_reduce_scatter(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static,
+                         const void* Hs, int64_t ldH, int64_t D, int64_t V,
+                         const int32_t* n_rows_dev, int64_t row0, float* const* shards, int world,
+                         int64_t shard_rows, int64_t ld_shard, uint32_t* counter, cudaStream_t st) {
+  if (world < 1 || world > kMaxShards || shard_rows <= 0 || shard_rows % 32 != 0) return GC_ERR_ARG;
+  if (shard_rows * world < V) return GC_ERR_SHAPE;
+  const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
+  CUtensorMap ta, tb;
+  GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
+  GC_TRY(tc::make_operand_tmap(&tb, Hs, D, k_rows, ldH, true, 0));
+  Sched s = make_sched(V, D, k_rows);
+  s.counter = counter;
+  s.a_hint = ptx::kL2Normal;
+  s.b_hint = ptx::kL2EvictLast;
+  s.n_band = pick_n_band(k_rows);
+  s.skip_empty_k = 1;                               // every launch adds: an empty chunk adds nothing
+  if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 2; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
+  EpiReduceScatterF32::Params ep;
+  for (int r = 0; r < kMaxShards; ++r) {
+    const int rr = r < world ? r : 0;
+    int64_t rows = V - (int64_t)rr * shard_rows;
+    rows = rows > shard_rows ? shard_rows : rows;
+    if (rows < 1) rows = 1;                         // an owner past the end of V is never addressed
+    if (!shards[rr]) return GC_ERR_NULL;
+    GC_TRY(make_f32_out_tmap(&ep.tm[r], shards[rr], rows, D, ld_shard));
+  }
+  ep.N = D;
+  ep.shard_rows = shard_rows;
+  ep.world = world;
+  KernelTimer kt(GC_KERNEL_DW, st);
+  return tc::launch_tc_gemm<2, true, true, EpiReduceScatterF32, 1, kPpc>(ta, tb, s, ep, st);
 }
 
 // one counter for the debug GEMM (not safe for concurrent debug calls on different streams)

@@ -74,3 +74,35 @@ def all_reduce_mean(*tensors: torch.Tensor) -> None:
     for t in tensors:
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         t.div_(w)
+
+
+def shard_rows_for(V: int, world: int) -> int:
+    """Rows per dW shard: ceil(V / world) rounded up to a multiple of 32 (a warp's slab of the dW
+    epilogue must not straddle two owners)."""
+    return -(-(-(-V // world)) // 32) * 32
+
+
+def exchange_dw_shards(shard: torch.Tensor):
+    """Every rank passes its own fp32 dW shard [shard_rows, D] (CUDA); returns (ptrs, keepalive):
+    ptrs[r] = device address of rank r's shard as seen from this process -- its own tensor, or the
+    peer's memory opened through CUDA IPC (same node; NVLink / NVSwitch carries the traffic when the
+    peer is another GPU, for which peer access is switched on by a first device-to-device copy).
+    `keepalive` must outlive every kernel that uses the pointers.  Collective over the default
+    group (any backend: only picklable IPC handles travel through it)."""
+    from torch.multiprocessing.reductions import reduce_tensor
+    assert shard.is_cuda and shard.dtype == torch.float32 and shard.is_contiguous()
+    if not is_dist():
+        return [shard.data_ptr()], [shard]
+    rank, world = dist.get_rank(), dist.get_world_size()
+    gathered = [None] * world
+    dist.all_gather_object(gathered, reduce_tensor(shard))
+    tensors = []
+    for r, (rebuild, args) in enumerate(gathered):
+        if r == rank:
+            tensors.append(shard)
+            continue
+        t = rebuild(*args)
+        if t.device != shard.device:
+            _ = t[:1].to(shard.device)          # first peer copy enables peer access in torch
+        tensors.append(t)
+    return [t.data_ptr() for t in tensors], tensors

@@ -128,6 +128,12 @@ def test_two_rank_training_exchange_matches_global_objective():
         assert np.allclose(dH / world, g["dH"][tok], rtol=1e-12, atol=1e-15)
 
 
+def test_dw_shard_rows():
+    for V, world in ((128256, 8), (152064, 4), (2056, 3), (31, 2), (256000, 1)):
+        sr = dp.shard_rows_for(V, world)
+        assert sr % 32 == 0 and sr * world >= V and (sr - 32) * world < V + 32 * world
+
+
 def test_shard_groups_balance():
     for n in (0, 1, 7, 16, 33):
         for world in (1, 2, 3, 8):

@@ -385,3 +385,32 @@ def test_kernel_timing_counts_the_contraction_launches(B):
     assert all(ms > 0 for ms, n in k.values() if n)
     run_gpu(B, b)
     assert all(n == 0 for _, n in B.gc_kernel_timing_end().values())
+
+
+def test_bf16_padded_leading_dimensions(B):
+    """Row strides larger than the row (ldH, ldW, lddH, lddW > D): H, W, dH, dW are views into wider
+    buffers; results equal the dense call bit for bit and the padding is never written."""
+    w = I.reduced(I.CONFIGS[2], D=256, V=1024 + 40, groups=2, group_size=2, seq_len=90, prompt_len=20)
+    b = make_batch(w, seed=6, device="cuda")
+    dense = run_gpu(B, b, chunk_tokens=256)
+
+    def widen(t, pad, fill):
+        buf = torch.full((t.shape[0], t.shape[1] + pad), fill, dtype=t.dtype, device=t.device)
+        buf[:, :t.shape[1]] = t
+        return buf, buf[:, :t.shape[1]]
+    Hbuf, Hv = widen(b.H, 8, 7.0)
+    Wbuf, Wv = widen(b.W, 16, -3.0)
+    dHbuf = torch.full((b.T, w.D + 24), 5.0, dtype=torch.bfloat16, device="cuda")
+    dWbuf = torch.full((w.V, w.D + 12), 9.0, dtype=torch.float32, device="cuda")
+    adv = dense["adv"]
+    f = B.gc_grpo_loss_fwd(Hv, Wv, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                           w.clip_lo, w.clip_hi, w.beta)
+    dH, dW = B.gc_grpo_loss_bwd(Hv, Wv, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                                f["logp"], f["lse"], w.clip_lo, w.clip_hi, w.beta,
+                                dH=dHbuf[:, :w.D], dW=dWbuf[:, :w.D], chunk_tokens=256)
+    torch.cuda.synchronize()
+    for k in ("logp", "entropy", "lse", "out5"):
+        assert torch.equal(f[k], dense[k]), k
+    assert torch.equal(dHbuf[:, :w.D], dense["dH"]) and torch.equal(dWbuf[:, :w.D], dense["dW"])
+    assert bool((dHbuf[:, w.D:] == 5.0).all()) and bool((dWbuf[:, w.D:] == 9.0).all())
+    assert bool((Hbuf[:, w.D:] == 7.0).all()) and bool((Wbuf[:, w.D:] == -3.0).all())

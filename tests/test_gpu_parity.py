@@ -414,3 +414,24 @@ def test_bf16_padded_leading_dimensions(B):
     assert torch.equal(dHbuf[:, :w.D], dense["dH"]) and torch.equal(dWbuf[:, :w.D], dense["dW"])
     assert bool((dHbuf[:, w.D:] == 5.0).all()) and bool((dWbuf[:, w.D:] == 9.0).all())
     assert bool((Hbuf[:, w.D:] == 7.0).all()) and bool((Wbuf[:, w.D:] == -3.0).all())
+
+
+@pytest.mark.parametrize("scale,tau", [(40.0, 1.0), (12.0, 0.05)])
+def test_bf16_large_logits_online_softmax_is_stable(B, scale, tau):
+    """Logits of magnitude ~1e2 (a peaked policy, or a small temperature): the running-max
+    rescaling of the split-V statistics must neither overflow nor lose the tail; near-one-hot rows
+    have logp -> 0 and entropy -> 0 (SURVEY.md sec 8(c) pins), and everything matches the oracle."""
+    T, D, V = 300, 256, 4096 + 24
+    H, W = I.make_hw(T, D, V, "bf16", 11, "cuda")
+    W = (W.float() * scale).to(torch.bfloat16)
+    y = I.sample_targets(H, W, tau, 11)
+    lp, en, ls = B.gc_token_logprobs(H, W, y, None, tau)
+    lp_o, en_o, ls_o = O.token_logprobs(to_f64(H), to_f64(W), y.cpu().numpy(), None, tau)
+    assert np.isfinite(ls.cpu().numpy()).all() and np.abs(ls_o).max() > 20
+    tol = 2e-3
+    assert np.abs(lp.cpu().numpy() - lp_o).max() <= tol
+    assert np.abs(ls.cpu().numpy() - ls_o).max() <= tol * 2
+    assert np.abs(en.cpu().numpy() - en_o).max() <= tol * 2
+    peaked = en_o < 1e-3
+    if peaked.any():
+        assert np.abs(lp.cpu().numpy()[peaked]).max() <= 5e-3

@@ -39,9 +39,24 @@ k_value_fwd(const void* __restrict__ H, int64_t ld, const void* __restrict__ w, 
     if (kBf16) {
       const int4* row = reinterpret_cast<const int4*>(static_cast<const __nv_bfloat16*>(H) + t * ld);
       const int4* wv = reinterpret_cast<const int4*>(w);
-      for (int64_t i = lane; i < D / 8; i += 32) {
+      const int64_t nv = D / 8;
+      int64_t i = lane;
+      for (; i + 96 < nv; i += 128) {                 // 4 row loads in flight per lane
+        int4 h4[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) h4[u] = __ldcs(row + i + 32 * u);   // H streams through once
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          float a[8], b[8];
+          bf16x8_to_f32(h4[u], a);
+          bf16x8_to_f32(__ldg(wv + i + 32 * u), b);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc = fmaf(a[j], b[j], acc);
+        }
+      }
+      for (; i < nv; i += 32) {
         float a[8], b[8];
-        bf16x8_to_f32(__ldcs(row + i), a);           // H streams through once
+        bf16x8_to_f32(__ldcs(row + i), a);
         bf16x8_to_f32(__ldg(wv + i), b);
 #pragma unroll
         for (int j = 0; j < 8; ++j) acc = fmaf(a[j], b[j], acc);

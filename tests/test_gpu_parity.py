@@ -435,3 +435,32 @@ def test_bf16_large_logits_online_softmax_is_stable(B, scale, tau):
     peaked = en_o < 1e-3
     if peaked.any():
         assert np.abs(lp.cpu().numpy()[peaked]).max() <= 5e-3
+
+
+def test_forward_backward_replays_from_a_cuda_graph(B):
+    """The calls only enqueue work (no allocation, no sync, no host-side data dependence), so a
+    whole forward + backward can be captured once and replayed; replays are bit-identical to the
+    eager run (the tile tickets are re-zeroed by a memset node inside the graph)."""
+    w = I.reduced(I.CONFIGS[2], D=256, V=2048 + 8, groups=2, group_size=2, seq_len=130, prompt_len=30)
+    b = make_batch(w, seed=8, device="cuda")
+    eager = run_gpu(B, b, chunk_tokens=256)                 # also sizes the cached workspace
+    adv = eager["adv"]
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        run_gpu(B, b, chunk_tokens=256)                     # warm-up on the side stream
+    torch.cuda.current_stream().wait_stream(stream)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                               w.clip_lo, w.clip_hi, w.beta)
+        dH, dW = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
+                                    f["logp"], f["lse"], w.clip_lo, w.clip_hi, w.beta,
+                                    chunk_tokens=256)
+    for _ in range(2):
+        dW.fill_(123.0)
+        dH.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(f["logp"], eager["logp"]) and torch.equal(f["out5"], eager["out5"])
+        assert torch.equal(dH, eager["dH"]) and torch.equal(dW, eager["dW"])

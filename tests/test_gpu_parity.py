@@ -464,3 +464,22 @@ def test_forward_backward_replays_from_a_cuda_graph(B):
         torch.cuda.synchronize()
         assert torch.equal(f["logp"], eager["logp"]) and torch.equal(f["out5"], eager["out5"])
         assert torch.equal(dH, eager["dH"]) and torch.equal(dW, eager["dW"])
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_bf16_randomized_shapes(B, seed):
+    """Seeded random small problems (D, V off the tile grid, V below one tile, random masks, both
+    aggregations, 1-3 dS chunks, temperature) against the oracle, forward and backward."""
+    r = np.random.default_rng(1000 + seed)
+    D = int(r.choice([64, 128, 264, 512, 1032]))
+    V = int(r.choice([8, 100, 255, 256, 257, 1000, 2048, 4136, 6000]))
+    w = I.reduced(I.CONFIGS[2], D=D, V=V, groups=int(r.integers(1, 4)), group_size=int(r.integers(1, 5)),
+                  seq_len=int(r.integers(2, 300)), prompt_len=0, old_std=0.3)
+    b0 = make_batch(w, seed=seed, device="cpu")
+    mask = I.random_mask(b0.T, float(r.uniform(0.2, 1.0)), seed) if r.random() < 0.6 else None
+    b = make_batch(w, seed=seed, device="cuda", mask=mask)
+    agg = int(r.integers(0, 2))
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref, agg)
+    got = run_gpu(B, b, agg, chunk_tokens=int(r.choice([0, 256, 512])))
+    check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)

@@ -21,6 +21,7 @@ from .gcore_oracle import (  # noqa: F401
     grpo_loss_grad_logp,
     lm_head_backward,
     lm_head_backward_row,
+    lm_head_backward_wrows,
     grpo_forward_backward,
 )
 from . import balance_oracle  # noqa: F401,E402

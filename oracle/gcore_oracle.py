@@ -35,6 +35,8 @@ grpo_loss_grad_logp central finite differences of grpo_loss; hand-derived values
 lm_head_backward    central finite differences of the whole forward; row sums of dz = 0;
                     column sums of dW = 0; <dH,H> = <dW,W>; textbook cross-entropy gradient
                     in the special case logp=old=ref.
+lm_head_backward_wrows  equality with lm_head_backward's rows (all rows, target rows, never-
+                    target rows, token slices summed); central finite differences w.r.t. W[v,d].
 Nothing here is "parity unpinned".
 """
 from __future__ import annotations
@@ -293,6 +295,32 @@ def lm_head_backward_row(h, W64, y, tau, g_t):
     dz = -g_t * p
     dz[int(y)] += g_t
     return (dz @ W64) / float(tau)
+
+
+def lm_head_backward_wrows(H, W_rows, vocab_ids, targets, mask, tau, g, lse):
+    """dW[v,:] for the vocab rows v in ``vocab_ids`` only (step 9 restricted to rows of dW):
+        dW[v,:] = (1/tau) sum_t g_t (1[v = y_t] - exp(z[t,v] - lse[t])) H[t,:].
+    A vocab row needs only the column z[:,v] = H W[v,:]^T / tau and the per-token lse, so this is
+    the dense backward's definition with the other columns left out -- no other change.
+    ``W_rows`` = W[vocab_ids] ([n, D]); ``lse`` [T] is the log-sum-exp over the FULL vocabulary
+    (from token_logprobs, or -- in the hybrid full-size check of SURVEY.md sec 8(c) protocol (v) --
+    the GPU's lse, itself verified on sampled rows).  dW is a sum over tokens, so a caller may
+    sum this function over token slices.  Pinned against lm_head_backward's rows and by finite
+    differences (tests/test_oracle_pins.py)."""
+    H = _f64(H)
+    Wr = _f64(W_rows)
+    g = _f64(g)
+    lse = _f64(lse)
+    vocab_ids = np.asarray(vocab_ids, dtype=np.int64)
+    targets = np.asarray(targets, dtype=np.int64)
+    scored = _scored(targets, mask)
+    z = (H @ Wr.T) / float(tau)                      # [T, n] columns of the logits
+    p = np.exp(z - lse[:, None])
+    onehot = (targets[:, None] == vocab_ids[None, :]) & scored[:, None]
+    gs = np.where(scored, g, 0.0)
+    dz = gs[:, None] * (onehot.astype(np.float64) - p)
+    dz[~scored] = 0.0                                # lse is 0 at unscored rows: p is garbage there
+    return (dz.T @ H) / float(tau)
 
 
 def grpo_forward_backward(H, W, targets, mask, tau, cu_seqlens, adv, old_logp, ref_logp,

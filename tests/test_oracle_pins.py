@@ -397,3 +397,45 @@ def test_backward_cross_entropy_special_case():
     dz = wgt[:, None] * (P - Y)                             # d(-sum w logp)/dz
     assert np.allclose(out["dH"], dz @ W, atol=1e-14)
     assert np.allclose(out["dW"], dz.T @ H, atol=1e-14)
+
+
+def test_backward_wrows_matches_dense_rows_and_finite_differences():
+    """lm_head_backward_wrows (step 9 restricted to vocab rows; used by the full-size dW check):
+    equal to the dense backward's rows for every row, for target rows and never-target rows, with
+    token slices summed; and each entry equal to the central finite difference of the loss."""
+    H, W, y, mask, tau, cu, adv, old, ref = _small_problem(24)
+    out = O.grpo_forward_backward(H, W, y, mask, tau, cu, adv, old, ref)
+    V = W.shape[0]
+    scored = (mask != 0) & (y >= 0)
+    hit = sorted(set(int(v) for v in y[scored]))
+    miss = [v for v in range(V) if v not in hit]
+    assert hit and miss
+    for ids in (list(range(V)), hit, miss, [miss[0], hit[0], V - 1, 0]):
+        rows = O.lm_head_backward_wrows(H, W[ids], ids, y, mask, tau, out["g"], out["lse"])
+        assert rows.shape == (len(ids), H.shape[1])
+        assert np.allclose(rows, out["dW"][ids], atol=1e-15)
+    # a sum over token slices is the same thing (dW is a sum over tokens)
+    ids = [hit[0], miss[0]]
+    T = len(y)
+    acc = np.zeros((2, H.shape[1]))
+    for a in range(0, T, 3):
+        sl = slice(a, min(T, a + 3))
+        acc += O.lm_head_backward_wrows(H[sl], W[ids], ids, y[sl], mask[sl], tau, out["g"][sl],
+                                        out["lse"][sl])
+    assert np.allclose(acc, out["dW"][ids], atol=1e-15)
+
+    def loss(Wx):
+        return O.grpo_forward_backward(H, Wx, y, mask, tau, cu, adv, old, ref,
+                                       need_grads=False)["loss"]
+    h = 1e-5
+    rows = O.lm_head_backward_wrows(H, W[ids], ids, y, mask, tau, out["g"], out["lse"])
+    for i, v in enumerate(ids):
+        for d in (0, 3):
+            E = np.zeros_like(W)
+            E[v, d] = h
+            fd = (loss(W + E) - loss(W - E)) / (2 * h)
+            assert abs(fd - rows[i, d]) < 1e-9
+    # a transposed operand, a dropped onehot or a wrong sign would fail the above; a wrong lse
+    # must change the result (the function really uses it)
+    bad = O.lm_head_backward_wrows(H, W[ids], ids, y, mask, tau, out["g"], out["lse"] + 0.1)
+    assert np.abs(bad - rows).max() > 1e-4

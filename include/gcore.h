@@ -18,8 +18,12 @@
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and
  *     return without synchronising.  Inputs must stay alive until the stream has passed the call.
  *   - Return value is a gc_status.  Host-checkable errors are reported before any launch.  No
- *     exceptions, no abort(), no environment variables, no global mutable state (one exception:
- *     the measurement aid gc_kernel_timing_*, off by default).
+ *     exceptions, no abort(), no environment variables.  Process-global state is limited to:
+ *     (i) a write-once, atomically published cache of launch attributes per kernel and device
+ *     (idempotent: host threads may race on a first launch); (ii) the measurement aid
+ *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter of
+ *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently).  None of it
+ *     changes results.  Calls on different streams need different workspaces.
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V
@@ -189,7 +193,12 @@ int gc_compact_rows(const void* H, int64_t ldH, int dtype, const int32_t* target
 /* The loss kernels alone on given log-probs (steps 6-8): out5 as in gc_grpo_loss_fwd;
  * g [T] nullable (d loss / d logp * grad_loss).  Exposed for tests and for the HBM-roofline
  * measurement of the elementwise kernels on a scaled-up stand-in.
- * workspace: gc_workspace_bytes(GC_OP_LOSS_FWD, T, 8, 8, GC_F32, 0) is always enough. */
+ * Any R >= 1 (empty responses, i.e. repeated cu_seqlens entries, are fine; the fwd / bwd entry
+ * points above additionally require R <= T + 1, the size their internal loss scratch is carved
+ * for).  logp, old_logp, ref_logp, targets, g 16-byte aligned; mask 4-byte aligned.  Unscored
+ * positions may hold anything (inf, NaN): only scored tokens enter the sums.
+ * workspace: gc_loss_workspace_bytes(T, R). */
+size_t gc_loss_workspace_bytes(int64_t T, int32_t R);
 int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
                        const int32_t* targets, const uint8_t* mask, int64_t T,
                        const int32_t* cu_seqlens, int32_t R, const float* adv,
@@ -297,13 +306,20 @@ int gc_kernel_timing_end(float* ms_by_kind_host, int32_t* launches_by_kind_host)
  * library-owned counter, so do not run two such debug calls concurrently); 0: static round-robin
  * (the schedule of the dH kernel).  dual_n != 0 (cta_group 2 only): 256 x 512 tiles whose two
  * halves share the A stages (the dH kernel's tile).  cluster4 != 0 (cta_group 2 only): clusters
- * of two CTA pairs that take adjacent M tiles and fetch every B stage once, by TMA multicast
- * (the launch shape of the path's kernels). */
+ * of two CTA pairs that take adjacent M tiles and fetch every B stage once, by TMA multicast.
+ * Item order (so that the production schedules of the path's kernels are reachable at any size):
+ *   c_major != 0: items = (band of m_band M tiles, run of chunk_ntiles N tiles, M tile in band),
+ *                 the forward / recompute order (m_band = 0: one band; a last, shorter band and a
+ *                 last, shorter run are allowed);
+ *   n_band  >  0: items = (band of n_band N tiles, M tile, N tile in band), the dW order (a last,
+ *                 narrower band is allowed);  c_major and n_band exclude each other;
+ *   both 0      : (M tile, N tile). */
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major,
                        const void* B, int64_t ldb, int b_mn_major,
                        float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
                        int accumulate, int cta_group, int dynamic_schedule, int dual_n,
-                       int cluster4, void* cuda_stream);
+                       int cluster4, int c_major, int m_band, int chunk_ntiles, int n_band,
+                       void* cuda_stream);
 
 #ifdef __cplusplus
 }

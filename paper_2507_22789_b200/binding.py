@@ -27,6 +27,7 @@ EXPORTS = [
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
     "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
     "gc_grpo_loss_bwd_reduce_scatter",
+    "gc_loss_workspace_bytes",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
@@ -65,8 +66,10 @@ def _load() -> C.CDLL:
     lib.gc_compact_rows.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, vp, vp, vp, sz, vp]
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
                                        f32, vp, vp, vp, sz, vp]
+    lib.gc_loss_workspace_bytes.restype = sz
+    lib.gc_loss_workspace_bytes.argtypes = [i64, i32]
     lib.gc_debug_gemm_bf16.argtypes = [vp, i64, ci, vp, i64, ci, vp, i64, i64, i64, i64, ci, ci, ci,
-                                       ci, ci, vp]
+                                       ci, ci, ci, ci, ci, ci, vp]
     u64 = C.c_uint64
     lib.gc_balance_workspace_bytes.restype = sz
     lib.gc_balance_workspace_bytes.argtypes = [i32]
@@ -90,6 +93,7 @@ def _load() -> C.CDLL:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
+                        "gc_loss_workspace_bytes",
                         "gc_critic_workspace_bytes"):
             fn.restype = ci
     return lib
@@ -127,8 +131,11 @@ _ws_cache: dict = {}
 
 
 def workspace(nbytes: int, device) -> torch.Tensor:
-    """A cached device buffer of at least nbytes (torch caching allocator: 512-byte aligned)."""
-    key = str(device)
+    """A cached device buffer of at least nbytes (torch caching allocator: 512-byte aligned), one
+    per (device, current stream): calls on different streams never share scratch, and a buffer
+    that is dropped when a larger one is needed is only ever reused by later work of the same
+    stream (the caching allocator's reuse is stream-ordered)."""
+    key = (str(device), int(torch.cuda.current_stream(device).cuda_stream))
     buf = _ws_cache.get(key)
     if buf is None or buf.numel() < nbytes:
         _ws_cache[key] = buf = torch.empty(max(nbytes, 1 << 20), dtype=torch.uint8, device=device)
@@ -256,9 +263,8 @@ def gc_grpo_token_loss(logp, old_logp, ref_logp, targets, mask, cu_seqlens, adv,
     dev = logp.device
     out5 = torch.empty(5, dtype=torch.float32, device=dev)
     g = torch.empty(T, dtype=torch.float32, device=dev) if want_grad else None
-    nb = workspace_bytes(GC_OP_LOSS_FWD, T, 8, 8, GC_F32)
-    ws = workspace(nb, dev)
     R = cu_seqlens.numel() - 1
+    ws = workspace(int(_lib.gc_loss_workspace_bytes(T, R)), dev)
     _check(_lib.gc_grpo_token_loss(_ptr(logp), _ptr(old_logp), _ptr(ref_logp), _ptr(targets),
                                    _ptr(mask), T, _ptr(cu_seqlens), R, _ptr(adv), float(clip_lo),
                                    float(clip_hi), float(beta), int(agg), float(grad_loss),
@@ -290,8 +296,10 @@ def gc_validate_targets(targets, mask, V) -> int:
 
 
 def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, accumulate=False,
-                       cta_group=2, dynamic_schedule=True, dual_n=False, cluster4=False):
-    """C[M,N] f32 = A.B on the tcgen05 tile engine (unit test of the engine)."""
+                       cta_group=2, dynamic_schedule=True, dual_n=False, cluster4=False,
+                       c_major=False, m_band=0, chunk_ntiles=0, n_band=0):
+    """C[M,N] f32 = A.B on the tcgen05 tile engine (unit test of the engine, incl. the item
+    orders of the path's kernels: c_major/m_band/chunk_ntiles, n_band)."""
     if a_mn_major:
         K, M = A.shape
     else:
@@ -306,7 +314,8 @@ def gc_debug_gemm_bf16(A, B, a_mn_major=False, b_mn_major=False, C_out=None, acc
     _check(_lib.gc_debug_gemm_bf16(_ptr(A), A.stride(0), int(a_mn_major), _ptr(B), B.stride(0),
                                    int(b_mn_major), _ptr(C_out), C_out.stride(0), M, N, K,
                                    int(accumulate), int(cta_group), int(dynamic_schedule),
-                                   int(dual_n), int(cluster4), _stream()))
+                                   int(dual_n), int(cluster4), int(c_major), int(m_band),
+                                   int(chunk_ntiles), int(n_band), _stream()))
     return C_out
 
 

@@ -109,7 +109,10 @@ size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t 
   return c.off;
 }
 
-constexpr int32_t kMaxRForWs = 1 << 24;   // loss workspace is sized for up to 16M responses... see below
+// gc_workspace_bytes has no R argument: the loss scratch inside the fwd / bwd workspaces is
+// sized for R <= T + 1 responses (one count per response), which the fwd / bwd entry points
+// enforce.  gc_grpo_token_loss takes any R with gc_loss_workspace_bytes(T, R).
+int32_t loss_rcap(int64_t T) { return (int32_t)((T + 1 < (1ll << 31) - 1) ? T + 1 : (1ll << 31) - 1); }
 
 }  // namespace
 
@@ -136,9 +139,7 @@ size_t gc_workspace_bytes(int op, int64_t T, int64_t D, int64_t V, int dtype, in
   if (T < 0 || D <= 0 || V <= 0) return 0;
   if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return 0;
   Carver c(nullptr);
-  // The loss workspace depends on R; R <= T always (every response has >= 0 tokens, but the
-  // per-response count array is sized by T + 1 to be safe for any R <= T + 1).
-  const int32_t Rcap = (int32_t)((T + 1 < (int64_t)kMaxRForWs) ? T + 1 : kMaxRForWs);
+  const int32_t Rcap = loss_rcap(T);
   switch (op) {
     case GC_OP_LOGPROBS:
       carve_fwd(c, T, D, V, dtype, nullptr);
@@ -276,15 +277,21 @@ int gc_grpo_advantages(const float* rewards, const int32_t* group_offsets, int32
                            drop_constant_groups != 0, adv, keep, static_cast<cudaStream_t>(cuda_stream));
 }
 
+// bound_R: the fwd / bwd entry points size their loss scratch for R <= T + 1 (empty responses are
+// fine, a batch with more responses than tokens + 1 is refused there; gc_grpo_token_loss takes it)
 static int check_loss_args(const int32_t* cu_seqlens, int32_t R, const float* adv,
                            const float* old_logp, const float* ref_logp, float clip_lo,
-                           float clip_hi, float beta, int agg, int64_t T) {
-  if (R < 0 || (T > 0 && R < 1) || (int64_t)R > T + 1) return GC_ERR_SHAPE;
+                           float clip_hi, float beta, int agg, int64_t T, bool bound_R = true) {
+  if (R < 0 || (T > 0 && R < 1) || (bound_R && (int64_t)R > T + 1)) return GC_ERR_SHAPE;
   if (agg != GC_AGG_TOKEN_MEAN && agg != GC_AGG_SEQ_MEAN) return GC_ERR_ARG;
   if (!(clip_lo >= 0.f) || !(clip_hi >= 0.f) || !(beta >= 0.f)) return GC_ERR_ARG;
   if (!cu_seqlens || (T > 0 && (!adv || !old_logp))) return GC_ERR_NULL;
   if (beta != 0.f && T > 0 && !ref_logp) return GC_ERR_NULL;
   return GC_OK;
+}
+
+size_t gc_loss_workspace_bytes(int64_t T, int32_t R) {
+  return (T < 0 || R < 0) ? 0 : loss_ws_bytes(T, R) + 256;
 }
 
 int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* ref_logp,
@@ -293,7 +300,8 @@ int gc_grpo_token_loss(const float* logp, const float* old_logp, const float* re
                        float clip_hi, float beta, int agg, float grad_loss, float* out5, float* g,
                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (T < 0 || T >= (1ll << 31)) return GC_ERR_SHAPE;
-  GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
+  GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T,
+                         false));
   if (!out5 || (T > 0 && (!logp || !targets))) return GC_ERR_NULL;
   if (!aligned16(logp) || !aligned16(old_logp) || !aligned16(ref_logp) || !aligned16(targets) ||
       !aligned16(g) || (reinterpret_cast<uintptr_t>(mask) & 3))
@@ -380,7 +388,7 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
     return GC_OK;
   }
   const int64_t chunk = resolve_chunk(T, D, V, chunk_tokens);
-  const int32_t Rcap = (int32_t)((T + 1 < (int64_t)kMaxRForWs) ? T + 1 : kMaxRForWs);
+  const int32_t Rcap = loss_rcap(T);
   Carver c(workspace);
   BwdWs w;
   carve_bwd(c, T, D, V, dtype, chunk, Rcap, &w);
@@ -635,13 +643,14 @@ int gc_gather_1d(const void* x, const int32_t* rows, const int32_t* n_rows, int6
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major, const void* B, int64_t ldb,
                        int b_mn_major, float* C, int64_t ldc, int64_t M, int64_t N, int64_t K,
                        int accumulate, int cta_group, int dynamic_schedule, int dual_n,
-                       int cluster4, void* cuda_stream) {
+                       int cluster4, int c_major, int m_band, int chunk_ntiles, int n_band,
+                       void* cuda_stream) {
   if (!A || !B || !C) return GC_ERR_NULL;
   if (M <= 0 || N <= 0 || K <= 0) return GC_ERR_SHAPE;
   GC_TRY(check_arch());
   return tc_debug_gemm(A, lda, a_mn_major, B, ldb, b_mn_major, C, ldc, M, N, K, accumulate,
-                       cta_group, dynamic_schedule, dual_n, cluster4,
-                       static_cast<cudaStream_t>(cuda_stream));
+                       cta_group, dynamic_schedule, dual_n, cluster4, c_major, m_band, chunk_ntiles,
+                       n_band, static_cast<cudaStream_t>(cuda_stream));
 }
 
 }  // extern "C"

@@ -155,7 +155,8 @@ int tc_dw_reduce_scatter(const void* dS, int64_t ldS, int64_t rows_cap, int64_t 
                          int64_t shard_rows, int64_t ld_shard, uint32_t* counter, cudaStream_t st);
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, int dynamic_schedule, int dual_n, int cluster4, cudaStream_t st);
+                  int cta_group, int dynamic_schedule, int dual_n, int cluster4, int c_major,
+                  int m_band, int chunk_ntiles, int n_band, cudaStream_t st);
 double tc_dh_waves(int64_t rows, int64_t D);
 
 }  // namespace gc

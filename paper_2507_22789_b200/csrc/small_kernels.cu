@@ -288,7 +288,17 @@ k_token_loss(const float* __restrict__ logp, const float* __restrict__ old_logp,
       d0 = a0;
       d1 = a1;
     }
-    if (mask) mk8 = *reinterpret_cast<const unsigned long long*>(mask + t0f);
+    if (mask) {
+      // t0f is a multiple of 8: the 8-byte load is aligned iff the mask pointer is; a mask view
+      // at a 4-byte offset (the API's minimum alignment) takes two 4-byte loads
+      if ((reinterpret_cast<uintptr_t>(mask) & 7) == 0) {
+        mk8 = *reinterpret_cast<const unsigned long long*>(mask + t0f);
+      } else {
+        const unsigned int lo4 = *reinterpret_cast<const unsigned int*>(mask + t0f);
+        const unsigned int hi4 = *reinterpret_cast<const unsigned int*>(mask + t0f + 4);
+        mk8 = (unsigned long long)lo4 | ((unsigned long long)hi4 << 32);
+      }
+    }
   }
   const CuSlice cs = load_cu_slice(cu, tile_r, s_cu);
   const double n_scored = (double)cnt->n_scored;
@@ -351,9 +361,9 @@ k_token_loss(const float* __restrict__ logp, const float* __restrict__ old_logp,
       const float d = rf[i] - lp[i];
       const float ed = fast_exp(d);
       const float k3 = ed - d - 1.0f;
-      const float ws = scored ? w : 0.0f;
-      acc_pg -= sm * ws;
-      acc_kl += k3 * ws;
+      // selects, not zero weights: inf / NaN at an unscored position must not reach the sums
+      acc_pg -= scored ? sm * w : 0.0f;
+      acc_kl += scored ? k3 * w : 0.0f;
       n_clip += (scored && !unclipped) ? 1u : 0u;
       gout[i] = scored ? gs * ((unclipped ? -s1 : 0.0f) + beta * (1.0f - ed)) : 0.0f;
     }
@@ -760,8 +770,10 @@ int launch_gather_rows(const void* H, int64_t ldH, int elem_bytes, int64_t D, in
 
 template <typename T>
 __global__ void k_gather_1d(const T* __restrict__ src, const int32_t* __restrict__ rows,
-                            const int32_t* __restrict__ n_rows_dev, T* __restrict__ dst) {
-  const int64_t n = *n_rows_dev;
+                            const int32_t* __restrict__ n_rows_dev, int64_t max_rows,
+                            T* __restrict__ dst) {
+  int64_t n = *n_rows_dev;
+  n = n < max_rows ? n : max_rows;          // never past the caller's allocation
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
        i += (int64_t)gridDim.x * blockDim.x)
     dst[i] = src[rows[i]];
@@ -771,7 +783,7 @@ int launch_gather_f32(const float* src, const int32_t* rows, const int32_t* n_ro
                       float* dst, cudaStream_t st) {
   int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
   if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
-  k_gather_1d<float><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, dst);
+  k_gather_1d<float><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, T, dst);
   GC_CUDA_TRY(cudaGetLastError());
   return GC_OK;
 }
@@ -780,7 +792,7 @@ int launch_gather_i32(const int32_t* src, const int32_t* rows, const int32_t* n_
                       int32_t* dst, cudaStream_t st) {
   int64_t blocks = ceil_div(T > 0 ? T : 1, 256);
   if (blocks > kNumSMs * 8) blocks = kNumSMs * 8;
-  k_gather_1d<int32_t><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, dst);
+  k_gather_1d<int32_t><<<(unsigned)blocks, 256, 0, st>>>(src, rows, n_rows, T, dst);
   GC_CUDA_TRY(cudaGetLastError());
   return GC_OK;
 }

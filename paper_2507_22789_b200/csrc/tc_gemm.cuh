@@ -10,6 +10,7 @@
 // Warps: 0 = TMA producer, 1 = MMA issuer (leader CTA only), 2 = TMEM allocator,
 // 4..7 = epilogue (thread = one accumulator row, 32 fp32 columns per tcgen05.ld).
 #pragma once
+#include <atomic>
 #include "common.cuh"
 #include "tc_ptx.cuh"
 
@@ -556,14 +557,19 @@ int launch_tc_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const Sched& 
   constexpr int CL = CG * PPC;
   constexpr int kSmemBytes = Cfg<CG, NSUB, 4 * Epi::kWarpSmem>::kSmemBytes;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
-  // per instantiation and device: the smem opt-in is a per-device function attribute
-  static int clusters_by_dev[64] = {};
+  // Per instantiation and device: the smem opt-in is a per-device function attribute, and the
+  // number of co-resident clusters is queried once.  This cache is the library's only launch-path
+  // state; it is write-once per slot with an idempotent value (concurrent first calls compute the
+  // same number), published with release/acquire so host threads may race on the first launch.
+  static std::atomic<int> clusters_by_dev[64];
   int dev = 0;
   GC_CUDA_TRY(cudaGetDevice(&dev));
-  int& clusters = clusters_by_dev[dev & 63];
+  if (dev < 0 || dev >= 64) return GC_ERR_CUDA;
+  int clusters = clusters_by_dev[dev].load(std::memory_order_acquire);
   if (clusters == 0) {
     GC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
     clusters = max_active_clusters(kern, CL, kSmemBytes);
+    clusters_by_dev[dev].store(clusters, std::memory_order_release);
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(clusters * CL));

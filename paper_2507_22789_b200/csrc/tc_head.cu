@@ -5,8 +5,6 @@
 //   a11    dH           dH = dS W             -> bf16 rows scattered to their original positions
 //   a12    dW           dW (+)= dS^T Hs       -> fp32
 #include "tc_gemm.cuh"
-#include <stdio.h>
-#include <stdlib.h>
 
 // Production launch shape: CTA pairs (cta_group::2) in clusters of kPpc pairs (tc_gemm.cuh).
 // kPpc = 2 (4-CTA clusters, B stages fetched once per cluster by TMA multicast) is built, tested
@@ -457,12 +455,6 @@ TcPlan tc_plan_forward(int64_t T, int64_t D, int64_t V) {
     }
   }
   best.n_vtiles = (int)Nt;
-#ifdef GC_EXP_ENV
-  if (const char* v = getenv("GC_PLAN_K")) {
-    best.chunk_vtiles = atoi(v);
-    best.n_split = (int)ceil_div(Nt, best.chunk_vtiles);
-  }
-#endif
   return best;
 }
 
@@ -486,24 +478,6 @@ size_t tc_fwd_partials_bytes(int64_t T, int64_t D, int64_t V) {
   return align_up((size_t)pl.n_split * (size_t)cap * sizeof(RowStat), 256);
 }
 
-#ifdef GC_EXP_ENV
-// Tuning builds only (-DGC_EXP_ENV, never the product build): schedule knobs from the environment.
-#include <stdlib.h>
-static void exp_override(Sched& s, const char* kind) {
-  char name[64];
-  auto get = [&](const char* knob, int& dst) {
-    snprintf(name, sizeof name, "GC_%s_%s", kind, knob);
-    if (const char* v = getenv(name)) dst = atoi(v);
-  };
-  int dyn = s.counter != nullptr;
-  get("MBAND", s.m_band); get("AHINT", s.a_hint); get("BHINT", s.b_hint); get("DYN", dyn);
-  get("CHUNK", s.chunk_ntiles); get("NBAND", s.n_band);
-  if (!dyn) s.counter = nullptr;
-}
-#define GC_EXP_OVERRIDE(s, kind) exp_override(s, kind)
-#else
-#define GC_EXP_OVERRIDE(s, kind) ((void)0)
-#endif
 
 // every launch shape of the engine (debug GEMM only; the path's kernels use fixed shapes)
 template <class Epi, bool A_MN, bool B_MN>
@@ -553,7 +527,6 @@ int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int
   ep.split_stride = ceil_div(T, 256) * 256;
   ep.V = V;
   ep.c = kLog2e / tau;
-  GC_EXP_OVERRIDE(s, "FWD");
   KernelTimer kt(GC_KERNEL_FWD_STATS, st);
   return tc::launch_tc_gemm<2, false, false, EpiStats, 1, kPpc>(ta, tb, s, ep, st);
 }
@@ -619,7 +592,6 @@ int tc_recompute_ds(const void* H, int64_t ldH, const void* W, int64_t ldW, int6
   ep.V = V;
   ep.c = kLog2e / tau;
   ep.inv_tau = 1.0f / tau;
-  GC_EXP_OVERRIDE(s, "DS");
   KernelTimer kt(GC_KERNEL_RECOMPUTE_DS, st);
   return tc::launch_tc_gemm<2, false, false, EpiDS, 1, kPpc>(ta, tb, s, ep, st);
 }
@@ -639,7 +611,6 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   ep.rows = rows;
   ep.row_base = row0;
   ep.N = D;
-  GC_EXP_OVERRIDE(s, "DH");
   KernelTimer kt(GC_KERNEL_DH, st);
   // K = V is ~2000 k-blocks per tile: 256 x 512 dual-N tiles (tc_gemm.cuh, Cfg)
   return tc::launch_tc_gemm<2, false, true, EpiStoreBf16, 2, kPpc>(ta, tb, s, ep, st);
@@ -665,7 +636,6 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   GC_TRY(make_f32_out_tmap(&ep.tm, dW, V, D, lddW));
   ep.N = D;
   ep.accumulate = accumulate;
-  GC_EXP_OVERRIDE(s, "DW");
   KernelTimer kt(GC_KERNEL_DW, st);
   return tc::launch_tc_gemm<2, true, true, EpiStoreF32, 1, kPpc>(ta, tb, s, ep, st);
 }
@@ -716,8 +686,11 @@ double tc_dh_waves(int64_t rows, int64_t D) {
 
 int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t ldb, int b_mn,
                   float* C, int64_t ldc, int64_t M, int64_t N, int64_t K, int accumulate,
-                  int cta_group, int dynamic_schedule, int dual_n, int cluster4, cudaStream_t st) {
+                  int cta_group, int dynamic_schedule, int dual_n, int cluster4, int c_major,
+                  int m_band, int chunk_ntiles, int n_band, cudaStream_t st) {
   if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
+  if (c_major < 0 || c_major > 1 || m_band < 0 || chunk_ntiles < 0 || n_band < 0) return GC_ERR_ARG;
+  if (c_major && n_band) return GC_ERR_ARG;          // the two item orders exclude each other
   if ((dual_n || cluster4) && cta_group != 2) return GC_ERR_ARG;
   const int ppc = cluster4 ? 2 : 1;
   if (N % 4 != 0) return GC_ERR_SHAPE;
@@ -725,6 +698,12 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
   GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, b_box_rows(cta_group, ppc)));
   Sched s = make_sched(M, N, K);
+  // the item orders of the path's kernels (forward / recompute: c_major + m_band + chunk_ntiles;
+  // dW: n_band), reachable here at any size
+  s.c_major = c_major;
+  s.m_band = m_band;
+  s.chunk_ntiles = chunk_ntiles > 0 ? chunk_ntiles : 1;
+  s.n_band = n_band;
   if (dynamic_schedule) {
     void* ctr = nullptr;
     GC_CUDA_TRY(cudaGetSymbolAddress(&ctr, g_debug_counter));

@@ -1,12 +1,14 @@
 """Seeded synthetic inputs shaped like the RLHF micro-batches of BASELINE.json:configs.
 
 This module is the ONLY code shared by the oracle-side tests and the CUDA path's tests/bench.
-It holds none of the method's arithmetic (no log-softmax, no advantages, no loss): it draws
-random tensors, lays out sequences, and samples target ids.  The recipe is DESIGN.md sec 4.
+It holds none of the method's arithmetic (no softmax, no log-probs, no advantages, no loss): it
+draws random tensors, lays out sequences, and samples target ids.  The recipe is DESIGN.md sec 4.
 
-Target sampling needs logits; it uses a plain ``torch.matmul`` + Gumbel-max as input synthesis
-(``sample_targets``), on whatever device H and W live on.  Policy log-probs needed to synthesise
-old/ref log-probs are passed IN by the caller (``perturb_logp``).
+Target sampling needs a draw from Categorical(softmax(z)); it uses a plain ``torch.matmul`` and the
+Gumbel-max trick (argmax of z + Gumbel noise -- no normalisation is ever computed) as input
+synthesis (``sample_targets``), on whatever device H and W live on.  Policy log-probs needed to
+synthesise old/ref log-probs are passed IN by the caller (``perturb_logp``): the tests take them
+from the oracle, bench.py from its own harness-side helper.
 """
 from __future__ import annotations
 
@@ -170,27 +172,6 @@ def sample_targets(H: torch.Tensor, W: torch.Tensor, tau: float = 1.0, seed: int
         z = z - torch.log(-torch.log(u))
         y[a:b] = z.argmax(dim=1).to(torch.int32)
     return y
-
-
-def proxy_policy_logp(H: torch.Tensor, W: torch.Tensor, y: torch.Tensor, tau: float = 1.0,
-                      chunk: int = 1024) -> np.ndarray:
-    """Approximate policy log-probs by plain torch ops (fp32 log_softmax over chunked logits).
-
-    INPUT SYNTHESIS ONLY, for batches too large for the oracle: it centres the synthetic
-    old/ref log-probs ("policy log-probs + N(0, std)", configs[0]) so that the ratio
-    exp(logp - old) is near 1.  Neither the CUDA path nor the oracle calls it, and its values
-    are never used as expected results."""
-    T = H.shape[0]
-    out = torch.empty(T, dtype=torch.float32, device=H.device)
-    Wf = W if H.is_cuda else W.float()
-    for a in range(0, T, chunk):
-        b = min(T, a + chunk)
-        Hc = H[a:b] if H.is_cuda else H[a:b].float()
-        z = (Hc @ Wf.T).float() / tau
-        lp = torch.log_softmax(z, dim=1)
-        idx = y[a:b].clamp(min=0).long().unsqueeze(1)
-        out[a:b] = lp.gather(1, idx).squeeze(1)
-    return out.cpu().numpy().astype(np.float64)
 
 
 def perturb_logp(policy_logp, std: float, seed: int) -> np.ndarray:

@@ -9,7 +9,7 @@ import torch
 
 import oracle as O
 from paper_2507_22789_b200 import inputs as I
-from tests.helpers import make_batch, oracle_run, rel_fro, to_f64
+from tests.helpers import ELEM_BF16, ELEM_F32, elem_excess, make_batch, oracle_run, rel_fro, to_f64
 
 pytestmark = pytest.mark.gpu
 
@@ -111,6 +111,37 @@ def test_engine_gemm_many_tiles(B, dyn, dual):
     C2 = B.gc_debug_gemm_bf16(A, Bm, dynamic_schedule=dyn, dual_n=dual)
     assert (C1 - ref).abs().max().item() < 1e-3 * K ** 0.5
     assert torch.equal(C1, C2)
+
+
+SCHEDS = {
+    "n_band_narrow_last": dict(n_band=4),                       # 10 N tiles -> bands 4, 4, 2
+    "n_band_3": dict(n_band=3),                                 # 3, 3, 3, 1
+    "m_band_full_plus_rest_k3": dict(c_major=True, m_band=5, chunk_ntiles=3),   # 22 = 4x5 + 2; runs 3,3,3,1
+    "m_band_one_band_k4": dict(c_major=True, m_band=0, chunk_ntiles=4),
+    "m_band_7_k1": dict(c_major=True, m_band=7, chunk_ntiles=1),
+}
+
+
+@pytest.mark.parametrize("dyn", [False, True])
+@pytest.mark.parametrize("a_mn,b_mn", [(0, 0), (1, 1), (0, 1)])
+@pytest.mark.parametrize("sched", list(SCHEDS))
+def test_engine_gemm_production_item_orders(B, dyn, a_mn, b_mn, sched):
+    """The item orders the path's kernels use at full size only (tc_gemm.cuh get_item): the dW
+    order with a narrower last N band, and the forward / recompute order with full + remainder M
+    bands and runs of k > 1 N tiles with a shorter last run -- here at a size the test can check
+    element by element (220 tiles > 74 CTA pairs, ragged M and N), store and accumulate."""
+    M, N, K = 256 * 21 + 40, 256 * 9 + 8, 320
+    g = torch.Generator(device="cuda").manual_seed(17)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    args = (A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm, a_mn, b_mn)
+    kw = dict(cta_group=2, dynamic_schedule=dyn, **SCHEDS[sched])
+    C = B.gc_debug_gemm_bf16(*args, C_out=torch.full((M, N), 7.0, device="cuda"), **kw)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    C2 = B.gc_debug_gemm_bf16(*args, C_out=C.clone(), accumulate=True, **kw)
+    assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+    assert torch.equal(C, B.gc_debug_gemm_bf16(*args, **kw))
 
 
 # ------------------------------------------------------------------ a6/a7 advantages
@@ -231,7 +262,10 @@ def run_gpu(B, b, agg=0, backward=True, chunk_tokens=0, simt=False, grad_loss=1.
         dH, dW = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t,
                                     f["logp"], f["lse"], w.clip_lo, w.clip_hi, w.beta, agg,
                                     grad_loss, chunk_tokens=chunk_tokens, simt=simt)
-        out.update(dH=dH, dW=dW)
+        # a9 alone on the forward's own logp: the g_t the backward consumed
+        _, g = B.gc_grpo_token_loss(f["logp"], b.old_t, b.ref_t, b.y, b.mask_t, b.cu_t, adv,
+                                    w.clip_lo, w.clip_hi, w.beta, agg, grad_loss)
+        out.update(dH=dH, dW=dW, g=g)
     torch.cuda.synchronize()
     return out
 
@@ -258,6 +292,19 @@ def check_against_oracle(b, got, ref, tol_lp, tol_grad, backward=True):
         assert np.all(dH[~s] == 0.0)                                   # masked rows exactly 0
         assert rel_fro(dH, ref["dH"]) <= tol_grad, rel_fro(dH, ref["dH"])
         assert rel_fro(dW, ref["dW"]) <= tol_grad, rel_fro(dW, ref["dW"])
+        # per element, scaled per row (a localised error must not hide in the norm)
+        el = ELEM_F32 if tol_grad <= TOL_GRAD_F32 else ELEM_BF16
+        assert elem_excess(dH, ref["dH"], **el) <= 1.0, elem_excess(dH, ref["dH"], **el)
+        assert elem_excess(dW, ref["dW"], **el) <= 1.0, elem_excess(dW, ref["dW"], **el)
+        # g_t element by element; both sides decide the clip branch from the same fp32 inputs,
+        # float near-ties excluded (reading 19)
+        rho = np.exp(ref["logp"] - b.old_np.astype(np.float64))
+        w_ = b.w
+        near = (np.abs(rho - (1 + w_.clip_hi)) < 2e-5) | (np.abs(rho - (1 - w_.clip_lo)) < 2e-5)
+        gg = got["g"].cpu().numpy().astype(np.float64)
+        assert np.all(gg[~s] == 0.0)
+        gtol = 1e-4 if tol_lp > TOL_LOGP_F32 else 2e-5       # bf16 path: logp itself is off by <= 1e-4
+        assert np.allclose(gg[~near], ref["g"][~near], rtol=gtol * 3, atol=gtol * np.abs(ref["g"]).max())
 
 
 # ------------------------------------------------------------------ config 0 in full (fp32)
@@ -483,3 +530,90 @@ def test_bf16_randomized_shapes(B, seed):
     ref = oracle_run(b, adv_ref, agg)
     got = run_gpu(B, b, agg, chunk_tokens=int(r.choice([0, 256, 512])))
     check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+
+
+@pytest.mark.parametrize("V", [520, 1096])
+@pytest.mark.parametrize("masked", [True, False])
+def test_bf16_production_schedules_vs_oracle(B, V, masked):
+    """Forward + backward against the DENSE oracle on a problem whose backward chunk is large
+    enough (8192 rows x D = 4096: k_rows D > 21 M) for the real kernels to take the schedules that
+    the small cases never reach: dW with n_band = 10 < 16 D tiles (a narrower last band), forward /
+    recompute with runs of k = 2 (V = 520) or 3 + 2 (V = 1096) vocab tiles and a full + remainder M
+    band (34 M tiles = 24 + 10), two dS chunks.  The vocabulary is small so the oracle stays cheap."""
+    if masked:      # 8520 scored of 11360 tokens (compaction mode)
+        w = I.reduced(I.CONFIGS[2], D=4096, V=V, groups=2, group_size=4, seq_len=1420, prompt_len=355,
+                      old_std=0.3)
+    else:           # dense mode, 8500 rows
+        w = I.reduced(I.CONFIGS[2], D=4096, V=V, groups=1, group_size=4, seq_len=2125, prompt_len=0,
+                      old_std=0.3)
+    b = make_batch(w, seed=3, device="cuda")
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref)
+    got = run_gpu(B, b, chunk_tokens=8192)
+    check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+    again = run_gpu(B, b, chunk_tokens=8192)
+    for k in ("logp", "entropy", "lse", "out5", "dH", "dW"):
+        assert torch.equal(again[k], got[k]), k
+
+
+def test_token_loss_offset_mask_and_garbage_at_unscored_positions(B):
+    """A mask view at a 4-byte (not 8-byte) offset must take the whole-tile fast path safely, and
+    inf / NaN stored at unscored positions of logp / old / ref must not reach the loss (only scored
+    tokens matter, gcore.h).  T spans several whole 2048-token tiles and a ragged tail."""
+    T, R = 3 * 2048 + 37, 23
+    logp, old, ref, adv, mask, y, cu = _loss_inputs(T, R, 77)
+    scored = (mask != 0) & (y >= 0)
+    res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04)
+    g_ref = O.grpo_loss_grad_logp(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04)
+    for agg in (0, 1):
+        res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg)
+        buf = torch.zeros(T + 16, dtype=torch.uint8, device="cuda")
+        for off in (4, 12, 8):
+            mview = buf[off:off + T]
+            mview.copy_(dev(mask))
+            assert mview.data_ptr() % 8 == off % 8
+            bad = [a.copy() for a in (logp, old, ref)]
+            fill = [np.nan, -np.inf, np.inf]
+            for a, v in zip(bad, fill):
+                a[~scored] = v
+            out5, g = B.gc_grpo_token_loss(dev(bad[0]), dev(bad[1]), dev(bad[2]), dev(y), mview,
+                                           dev(cu), dev(adv), 0.2, 0.2, 0.04, agg)
+            o = out5.cpu().numpy().astype(np.float64)
+            assert np.isfinite(o).all(), o
+            assert abs(o[0] - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+            assert abs(o[2] - res["kl_mean"]) <= 1e-5 * max(abs(res["kl_mean"]), 1e-3)
+            gg = g.cpu().numpy()
+            assert np.isfinite(gg).all() and np.all(gg[~scored] == 0.0)
+            if agg == 0:
+                assert np.allclose(gg, g_ref, rtol=3e-5, atol=2e-6 * np.abs(g_ref).max())
+
+
+def test_token_loss_more_responses_than_tokens(B):
+    """Empty responses are legal (repeated cu_seqlens entries), so R is not bounded by T."""
+    T, R = 40, 200
+    r = np.random.default_rng(5)
+    cu = np.sort(np.concatenate([[0, T], r.integers(0, T + 1, R - 1)])).astype(np.int32)
+    assert len(cu) == R + 1
+    logp, old, ref, _, mask, y, _ = _loss_inputs(T, 2, 9)
+    adv = r.normal(size=R).astype(np.float32)
+    scored = (mask != 0) & (y >= 0)
+    for agg in (0, 1):
+        out5, g = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu),
+                                       dev(adv), 0.2, 0.2, 0.04, agg)
+        res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg)
+        g_ref = O.grpo_loss_grad_logp(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg)
+        assert abs(out5[0].item() - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+        assert np.allclose(g.cpu().numpy(), g_ref, rtol=3e-5, atol=2e-6 * np.abs(g_ref).max())
+
+
+def test_gather_1d_never_writes_past_max_rows(B):
+    x = torch.arange(100, dtype=torch.int32, device="cuda")
+    rows = torch.arange(99, -1, -1, dtype=torch.int32, device="cuda")
+    n = torch.tensor([100], dtype=torch.int32, device="cuda")       # device count > allocation
+    buf = torch.full((64,), -7, dtype=torch.int32, device="cuda")
+    import ctypes as C
+    B._check(B.lib().gc_gather_1d(C.c_void_p(x.data_ptr()), C.c_void_p(rows.data_ptr()),
+                                  C.c_void_p(n.data_ptr()), 40, C.c_void_p(buf.data_ptr()),
+                                  C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    torch.cuda.synchronize()
+    assert torch.equal(buf[:40], rows[:40]) and bool((buf[40:] == -7).all())

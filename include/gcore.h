@@ -69,6 +69,10 @@ typedef enum { GC_OP_LOGPROBS = 0, GC_OP_LOSS_FWD = 1, GC_OP_LOSS_BWD = 2 } gc_o
 /* Static string for a gc_status (never NULL). */
 const char* gc_status_string(int status);
 
+/* Name of the CUDA error behind the calling thread's most recent GC_ERR_CUDA ("cudaSuccess" if
+ * there was none): thread-local, static string. */
+const char* gc_last_cuda_error(void);
+
 /* Library version (major*10000 + minor*100 + patch). */
 int gc_version(void);
 

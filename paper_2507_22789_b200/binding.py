@@ -20,7 +20,7 @@ GC_AGG_TOKEN_MEAN, GC_AGG_SEQ_MEAN = 0, 1
 GC_OP_LOGPROBS, GC_OP_LOSS_FWD, GC_OP_LOSS_BWD = 0, 1, 2
 
 EXPORTS = [
-    "gc_status_string", "gc_version", "gc_workspace_bytes", "gc_token_logprobs",
+    "gc_status_string", "gc_last_cuda_error", "gc_version", "gc_workspace_bytes", "gc_token_logprobs",
     "gc_host_staging_bytes", "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
     "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
@@ -46,6 +46,8 @@ def _load() -> C.CDLL:
     ci = C.c_int
     lib.gc_status_string.restype = C.c_char_p
     lib.gc_status_string.argtypes = [ci]
+    lib.gc_last_cuda_error.restype = C.c_char_p
+    lib.gc_last_cuda_error.argtypes = []
     lib.gc_version.restype = ci
     lib.gc_workspace_bytes.restype = sz
     lib.gc_workspace_bytes.argtypes = [ci, i64, i64, i64, ci, i64]
@@ -91,7 +93,7 @@ def _load() -> C.CDLL:
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
         fn = getattr(lib, name)
-        if name not in ("gc_status_string", "gc_workspace_bytes", "gc_host_staging_bytes",
+        if name not in ("gc_status_string", "gc_last_cuda_error", "gc_workspace_bytes", "gc_host_staging_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
                         "gc_loss_workspace_bytes",
                         "gc_critic_workspace_bytes"):
@@ -108,7 +110,10 @@ def lib() -> C.CDLL:
 
 def _check(status: int):
     if status != 0:
-        raise GcoreError(_lib.gc_status_string(status).decode())
+        msg = _lib.gc_status_string(status).decode()
+        if status == 8:
+            msg += " (" + _lib.gc_last_cuda_error().decode() + ")"
+        raise GcoreError(msg)
 
 
 def _ptr(t: Optional[torch.Tensor]):

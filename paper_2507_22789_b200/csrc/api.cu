@@ -5,6 +5,14 @@
 
 using namespace gc;
 
+namespace gc {
+static thread_local cudaError_t t_last_cuda_error = cudaSuccess;
+void note_cuda_error(cudaError_t e) {
+  t_last_cuda_error = e;
+  (void)cudaGetLastError();        // clear the runtime's non-sticky error state
+}
+}  // namespace gc
+
 namespace {
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
@@ -133,7 +141,9 @@ const char* gc_status_string(int status) {
   }
 }
 
-int gc_version(void) { return 100; }
+const char* gc_last_cuda_error(void) { return cudaGetErrorName(gc::t_last_cuda_error); }
+
+int gc_version(void) { return 200; }
 
 size_t gc_workspace_bytes(int op, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens) {
   if (T < 0 || D <= 0 || V <= 0) return 0;

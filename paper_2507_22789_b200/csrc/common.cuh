@@ -6,10 +6,16 @@
 #include <stddef.h>
 #include "../../include/gcore.h"
 
+// the CUDA error behind the calling thread's last GC_ERR_CUDA (api.cu; gc_last_cuda_error)
+namespace gc { void note_cuda_error(cudaError_t e); }
+
 #define GC_CUDA_TRY(expr)                         \
   do {                                            \
     cudaError_t _e = (expr);                      \
-    if (_e != cudaSuccess) return GC_ERR_CUDA;    \
+    if (_e != cudaSuccess) {                      \
+      ::gc::note_cuda_error(_e);                  \
+      return GC_ERR_CUDA;                         \
+    }                                             \
   } while (0)
 
 #define GC_TRY(expr)                              \

@@ -28,6 +28,9 @@
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V
  *     is a caller error (undefined result for that row; use gc_validate_targets to check).
+ *     With a mask, only scored rows reach the tensor cores (row selection a1).  mask == NULL
+ *     declares (almost) every row scored and skips the selection: rows with targets[t] < 0 are
+ *     then computed and discarded -- pass a mask (all ones will do) when many targets are < 0.
  *   - Outputs at unscored rows are exactly 0 (logp, entropy, lse, rows of dH).
  *   - Same inputs give bit-identical outputs from run to run (no floating-point atomics).
  */
@@ -144,9 +147,19 @@ int gc_grpo_loss_fwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
  *   g_t     = grad_loss * d loss / d logp_t
  *   dz[t,v] = g_t (1[v = y_t] - exp(z[t,v] - lse[t]))
  *   dH[t,:] = (1/tau) sum_v dz[t,v] W[v,:]        dW[v,:] (+)= (1/tau) sum_t dz[t,v] H[t,:]
- * dH [T,D] (lddH) in H's dtype, zero rows at unscored tokens.  dW [V,D] (lddW) of dW_dtype
- * (GC_F32 only for now); accumulate_dW != 0 adds to the existing contents.  chunk_tokens: rows
- * of the bf16 dS chunk buffer (0 = library picks; must match gc_workspace_bytes). */
+ * dH [T,D] (lddH) in H's dtype, zero rows at unscored tokens.  dW [V,D] (lddW) of dW_dtype:
+ * GC_F32 (BASELINE.json configs[4]: "dW accumulated in fp32"), or GC_BF16 -- the chunks then
+ * accumulate in an fp32 [V,D] staging buffer inside the workspace and are rounded to bf16 ONCE,
+ * after the last chunk (SURVEY.md sec 8(c) reading 13).  accumulate_dW != 0 adds to the existing
+ * contents (for GC_BF16: out = bf16(out + sum), one rounding per call).  chunk_tokens: rows of the
+ * bf16 dS chunk buffer (0 = library picks; must match the workspace query).
+ * fwd_state (nullable): the workspace gc_grpo_loss_fwd was given for the SAME inputs, untouched
+ * since; the backward then reuses the forward's row selection (a1: row list, compacted targets,
+ * compacted H) instead of recomputing it.  It must not overlap `workspace`.
+ * workspace: gc_bwd_workspace_bytes(T, D, V, dtype, chunk_tokens, dW_dtype)
+ * (= gc_workspace_bytes(GC_OP_LOSS_BWD, ...) for GC_F32). */
+size_t gc_bwd_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens,
+                              int dW_dtype);
 int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
                      const int32_t* targets, const uint8_t* mask,
                      int64_t T, int64_t D, int64_t V, float temperature,
@@ -155,7 +168,7 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
                      float clip_lo, float clip_hi, float beta, int agg,
                      const float* logp, const float* lse, float grad_loss,
                      void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
-                     int accumulate_dW, int64_t chunk_tokens,
+                     int accumulate_dW, int64_t chunk_tokens, const void* fwd_state,
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---- stage 4 backward fused with its data-parallel exchange (training
@@ -177,7 +190,7 @@ int gc_grpo_loss_bwd_reduce_scatter(
     const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi, float beta, int agg,
     const float* logp, const float* lse, float grad_loss,
     void* dH, int64_t lddH, float* const* dW_shards_host, int32_t world, int64_t shard_rows,
-    int64_t ld_shard, int64_t chunk_tokens,
+    int64_t ld_shard, int64_t chunk_tokens, const void* fwd_state,
     void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---- helpers ---- */

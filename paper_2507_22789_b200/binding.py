@@ -27,7 +27,7 @@ EXPORTS = [
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
     "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
     "gc_grpo_loss_bwd_reduce_scatter",
-    "gc_loss_workspace_bytes",
+    "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
@@ -60,10 +60,12 @@ def _load() -> C.CDLL:
                                            vp, sz, vp]
     lib.gc_grpo_advantages.argtypes = [vp, vp, i32, f32, ci, ci, vp, vp, vp]
     lib.gc_grpo_loss_fwd.argtypes = head + loss + [vp, vp, vp, vp, vp, sz, vp]
+    lib.gc_bwd_workspace_bytes.restype = sz
+    lib.gc_bwd_workspace_bytes.argtypes = [i64, i64, i64, ci, i64, ci]
     lib.gc_grpo_loss_bwd.argtypes = head + loss + [vp, vp, f32, vp, i64, vp, i64, ci, ci, i64,
-                                                   vp, sz, vp]
+                                                   vp, vp, sz, vp]
     lib.gc_grpo_loss_bwd_reduce_scatter.argtypes = head + loss + [vp, vp, f32, vp, i64, C.POINTER(vp),
-                                                                  i32, i64, i64, i64, vp, sz, vp]
+                                                                  i32, i64, i64, i64, vp, vp, sz, vp]
     lib.gc_validate_targets.argtypes = [vp, vp, i64, i64, C.POINTER(i64), vp]
     lib.gc_compact_rows.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, vp, vp, vp, sz, vp]
     lib.gc_grpo_token_loss.argtypes = [vp, vp, vp, vp, vp, i64, vp, i32, vp, f32, f32, f32, ci,
@@ -95,7 +97,7 @@ def _load() -> C.CDLL:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_last_cuda_error", "gc_workspace_bytes", "gc_host_staging_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
-                        "gc_loss_workspace_bytes",
+                        "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
                         "gc_critic_workspace_bytes"):
             fn.restype = ci
     return lib
@@ -135,12 +137,13 @@ def dtype_code(t: torch.Tensor, simt: bool = False) -> int:
 _ws_cache: dict = {}
 
 
-def workspace(nbytes: int, device) -> torch.Tensor:
+def workspace(nbytes: int, device, slot: str = "") -> torch.Tensor:
     """A cached device buffer of at least nbytes (torch caching allocator: 512-byte aligned), one
-    per (device, current stream): calls on different streams never share scratch, and a buffer
-    that is dropped when a larger one is needed is only ever reused by later work of the same
-    stream (the caching allocator's reuse is stream-ordered)."""
-    key = (str(device), int(torch.cuda.current_stream(device).cuda_stream))
+    per (device, current stream, slot): calls on different streams never share scratch, and a
+    buffer that is dropped when a larger one is needed is only ever reused by later work of the
+    same stream (the caching allocator's reuse is stream-ordered).  slot "fwd" is the workspace of
+    gc_grpo_loss_fwd, kept apart so that the backward can reuse the forward's row selection."""
+    key = (str(device), int(torch.cuda.current_stream(device).cuda_stream), slot)
     buf = _ws_cache.get(key)
     if buf is None or buf.numel() < nbytes:
         _ws_cache[key] = buf = torch.empty(max(nbytes, 1 << 20), dtype=torch.uint8, device=device)
@@ -229,34 +232,38 @@ def gc_grpo_loss_fwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp
     ent = torch.empty(T, dtype=torch.float32, device=dev)
     lse = torch.empty(T, dtype=torch.float32, device=dev)
     nb = workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dt)
-    ws = workspace(nb, dev)
+    ws = workspace(nb, dev, "fwd")
     _check(_lib.gc_grpo_loss_fwd(*args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo,
                                                     clip_hi, beta, agg),
                                  _ptr(out5), _ptr(logp), _ptr(ent), _ptr(lse), _ptr(ws),
                                  ws.numel(), _stream()))
-    return dict(out5=out5, logp=logp, entropy=ent, lse=lse)
+    # state: the forward's workspace (row list, compacted H), valid until the next forward on this
+    # stream; pass it to gc_grpo_loss_bwd(fwd_state=...) to skip the row selection there
+    return dict(out5=out5, logp=logp, entropy=ent, lse=lse, state=ws)
 
 
 def gc_grpo_loss_bwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp, ref_logp,
                      logp, lse, clip_lo=0.2, clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN,
                      grad_loss=1.0, *, dH=None, dW=None, accumulate_dW=False, chunk_tokens=0,
-                     simt=False):
-    """-> (dH [T,D] in H's dtype, dW [V,D] float32)."""
+                     simt=False, dW_dtype=torch.float32, fwd_state=None):
+    """-> (dH [T,D] in H's dtype, dW [V,D] float32 or bfloat16).  fwd_state: the "state" entry of
+    gc_grpo_loss_fwd's result for the same inputs (optional: reuses its row selection)."""
     args, T, D, V, dt = _head_args(H, W, targets, mask, temperature, simt)
     dev = H.device
     if dH is None:
         dH = torch.empty(T, D, dtype=H.dtype, device=dev)
     if dW is None:
         assert not accumulate_dW
-        dW = torch.empty(V, D, dtype=torch.float32, device=dev)
-    nb = workspace_bytes(GC_OP_LOSS_BWD, T, D, V, dt, chunk_tokens)
+        dW = torch.empty(V, D, dtype=dW_dtype, device=dev)
+    dwt = {torch.float32: GC_F32, torch.bfloat16: GC_BF16}[dW.dtype]
+    nb = int(_lib.gc_bwd_workspace_bytes(T, D, V, dt, chunk_tokens, dwt))
     ws = workspace(nb, dev)
     _check(_lib.gc_grpo_loss_bwd(*args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo,
                                                     clip_hi, beta, agg),
                                  _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH),
-                                 dH.stride(0) if T > 0 else D, _ptr(dW), dW.stride(0), GC_F32,
-                                 int(accumulate_dW), int(chunk_tokens), _ptr(ws), ws.numel(),
-                                 _stream()))
+                                 dH.stride(0) if T > 0 else D, _ptr(dW), dW.stride(0), dwt,
+                                 int(accumulate_dW), int(chunk_tokens), _ptr(fwd_state), _ptr(ws),
+                                 ws.numel(), _stream()))
     return dH, dW
 
 
@@ -448,7 +455,7 @@ def gc_value_head_bwd(H, w, g):
 def gc_grpo_loss_bwd_reduce_scatter(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp,
                                     ref_logp, logp, lse, shard_ptrs, shard_rows, ld_shard=None,
                                     clip_lo=0.2, clip_hi=0.2, beta=0.04, agg=GC_AGG_TOKEN_MEAN,
-                                    grad_loss=1.0, *, dH=None, chunk_tokens=0):
+                                    grad_loss=1.0, *, dH=None, chunk_tokens=0, fwd_state=None):
     """Backward whose dW tiles are TMA-reduce-added into the owning rank's shard.  shard_ptrs: list of
     `world` device pointers (ints; own tensor.data_ptr() or peer-mapped), shard r = fp32
     [shard_rows, D] holding vocab rows [r*shard_rows, (r+1)*shard_rows).  -> dH."""
@@ -463,6 +470,6 @@ def gc_grpo_loss_bwd_reduce_scatter(H, W, targets, mask, temperature, cu_seqlens
     _check(_lib.gc_grpo_loss_bwd_reduce_scatter(
         *args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg),
         _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH), dH.stride(0) if T > 0 else D, arr, world,
-        int(shard_rows), int(ld_shard if ld_shard is not None else D), int(chunk_tokens), _ptr(ws),
-        ws.numel(), _stream()))
+        int(shard_rows), int(ld_shard if ld_shard is not None else D), int(chunk_tokens),
+        _ptr(fwd_state), _ptr(ws), ws.numel(), _stream()))
     return dH

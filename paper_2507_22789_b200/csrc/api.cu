@@ -91,10 +91,12 @@ size_t carve_fwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, FwdWs* w
 
 struct BwdWs {
   uint32_t* counters; void* loss; float* out5; float* g; int32_t* rows; int32_t* n_rows; int32_t* targets_c;
-  float* lse_c; float* g_c; void* Hs; void* compact; void* dS;
+  float* lse_c; float* g_c; void* Hs; void* compact; void* dS; float* dW_acc;
 };
+// dW_dtype == GC_BF16: the chunks accumulate in an fp32 [V, D] staging buffer at the end of the
+// workspace and are rounded to bf16 once, after the last chunk (SURVEY.md sec 8(c) reading 13)
 size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk, int32_t R,
-                 BwdWs* w) {
+                 int dW_dtype, BwdWs* w) {
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   void* loss = c.take<uint8_t>(loss_ws_bytes(T, R));
   float* out5 = c.take<float>(64);
@@ -114,6 +116,8 @@ size_t carve_bwd(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int64_t 
     if (w) { w->rows = rows; w->n_rows = n_rows; w->targets_c = tcx; w->lse_c = lse_c; w->g_c = g_c;
              w->Hs = Hs; w->compact = cw; w->dS = dS; }
   }
+  float* acc = dW_dtype == GC_BF16 ? c.take<float>((size_t)V * (size_t)D) : nullptr;
+  if (w) w->dW_acc = acc;
   return c.off;
 }
 
@@ -159,11 +163,21 @@ size_t gc_workspace_bytes(int op, int64_t T, int64_t D, int64_t V, int dtype, in
       c.take<uint8_t>(loss_ws_bytes(T, Rcap));
       break;
     case GC_OP_LOSS_BWD:
-      carve_bwd(c, T, D, V, dtype, resolve_chunk(T, D, V, chunk_tokens), Rcap, nullptr);
+      carve_bwd(c, T, D, V, dtype, resolve_chunk(T, D, V, chunk_tokens), Rcap, GC_F32, nullptr);
       break;
     default:
       return 0;
   }
+  return c.off + 256;
+}
+
+size_t gc_bwd_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens,
+                              int dW_dtype) {
+  if (T < 0 || D <= 0 || V <= 0) return 0;
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return 0;
+  if (dW_dtype != GC_F32 && dW_dtype != GC_BF16) return 0;
+  Carver c(nullptr);
+  carve_bwd(c, T, D, V, dtype, resolve_chunk(T, D, V, chunk_tokens), loss_rcap(T), dW_dtype, nullptr);
   return c.off + 256;
 }
 
@@ -353,6 +367,8 @@ namespace {
 struct DwSink {
   void* dW; int64_t lddW; int accumulate;
   float* const* shards; int world; int64_t shard_rows;
+  int dW_dtype;             // GC_F32 / GC_BF16 (local dW only)
+  const void* fwd_state;    // the forward's workspace (row list + compacted H reused), or NULL
 };
 
 int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
@@ -362,9 +378,10 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
                   float beta, int agg, const float* logp, const float* lse, float grad_loss,
                   void* dH, int64_t lddH, const DwSink& sink, int64_t chunk_tokens, void* workspace,
                   size_t workspace_bytes, void* cuda_stream) {
-  void* const dW = sink.dW;
-  const int64_t lddW = sink.lddW;
-  const int accumulate_dW = sink.accumulate;
+  void* dW = sink.dW;
+  int64_t lddW = sink.lddW;
+  int accumulate_dW = sink.accumulate;
+  const bool dW_bf16 = !sink.shards && sink.dW_dtype == GC_BF16;
   GC_TRY(check_head_args(H, ldH, W, ldW, dtype, targets, T, D, V, temperature));
   GC_TRY(check_loss_args(cu_seqlens, R, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg, T));
   if (sink.shards) {
@@ -379,7 +396,11 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
   } else {
     if (!dW) return GC_ERR_NULL;
     if (lddW < D) return GC_ERR_SHAPE;
-    if (dtype == GC_BF16 && (lddW % 4 != 0 || !aligned16(dW))) return GC_ERR_ALIGN;
+    if (dW_bf16) {
+      if (dtype == GC_BF16 && (lddW % 8 != 0 || !aligned16(dW))) return GC_ERR_ALIGN;
+    } else if (dtype == GC_BF16 && (lddW % 4 != 0 || !aligned16(dW))) {
+      return GC_ERR_ALIGN;
+    }
   }
   if (T > 0 && (!dH || !logp || !lse)) return GC_ERR_NULL;
   if (lddH < D) return GC_ERR_SHAPE;
@@ -387,29 +408,39 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
   if (!aligned16(logp) || !aligned16(old_logp) || !aligned16(ref_logp) || !aligned16(targets) ||
       (reinterpret_cast<uintptr_t>(mask) & 3))
     return GC_ERR_ALIGN;
-  const size_t need = gc_workspace_bytes(GC_OP_LOSS_BWD, T, D, V, dtype, chunk_tokens);
+  const size_t need = gc_bwd_workspace_bytes(T, D, V, dtype, chunk_tokens, dW_bf16 ? GC_BF16 : GC_F32);
   if (!workspace || workspace_bytes < need) return GC_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  if (sink.fwd_state && (reinterpret_cast<uintptr_t>(sink.fwd_state) & 255)) return GC_ERR_ALIGN;
   GC_TRY(check_arch());
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (T == 0) {
+    const size_t eb = dW_bf16 ? 2 : 4;
     if (!sink.shards && !accumulate_dW)
-      GC_CUDA_TRY(cudaMemset2DAsync(dW, (size_t)lddW * 4, 0, (size_t)D * 4, (size_t)V, st));
+      GC_CUDA_TRY(cudaMemset2DAsync(dW, (size_t)lddW * eb, 0, (size_t)D * eb, (size_t)V, st));
     return GC_OK;
   }
   const int64_t chunk = resolve_chunk(T, D, V, chunk_tokens);
   const int32_t Rcap = loss_rcap(T);
   Carver c(workspace);
   BwdWs w;
-  carve_bwd(c, T, D, V, dtype, chunk, Rcap, &w);
+  carve_bwd(c, T, D, V, dtype, chunk, Rcap, dW_bf16 ? GC_BF16 : GC_F32, &w);
+  // bf16 dW: the chunk loop writes the fp32 staging buffer; one rounding pass at the end
+  void* const dW_out = dW;
+  const int64_t lddW_out = lddW;
+  const int accumulate_out = accumulate_dW;
+  if (dW_bf16) { dW = w.dW_acc; lddW = D; accumulate_dW = 0; }
 
   // a9: g_t = grad_loss * d loss / d logp_t for every token (0 at unscored tokens)
   GC_TRY(launch_token_loss(logp, old_logp, ref_logp, targets, mask, T, cu_seqlens, R, adv, clip_lo,
                            clip_hi, beta, agg, grad_loss, w.out5, w.g, w.loss, st));
 
-  if (dtype != GC_BF16)
-    return simt_backward(H, ldH, W, ldW, dtype == GC_BF16_SIMT, targets, mask, T, D, V, temperature,
-                         lse, w.g, dH, lddH, static_cast<float*>(dW), lddW, accumulate_dW, st);
+  if (dtype != GC_BF16) {
+    GC_TRY(simt_backward(H, ldH, W, ldW, dtype == GC_BF16_SIMT, targets, mask, T, D, V, temperature,
+                         lse, w.g, dH, lddH, static_cast<float*>(dW), lddW, accumulate_dW, st));
+    if (dW_bf16) GC_TRY(launch_cast_f32_bf16(w.dW_acc, D, dW_out, lddW_out, V, D, accumulate_out, st));
+    return GC_OK;
+  }
 
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;
   const int64_t ldS = ld_ds(V);
@@ -422,9 +453,18 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
   const int32_t* rows = nullptr;
   const int32_t* n_rows = nullptr;
   if (compact) {
-    GC_TRY(launch_compact_rows(targets, mask, T, w.rows, w.n_rows, w.compact, st));
-    GC_TRY(launch_gather_rows(H, ldH, 2, D, T, w.rows, w.n_rows, w.Hs, cap, st));
-    GC_TRY(launch_gather_i32(targets, w.rows, w.n_rows, T, w.targets_c, st));
+    if (sink.fwd_state) {
+      // a1 was done by the forward on the same inputs: reuse its row list, compacted targets and
+      // compacted H instead of recomputing them (the caller keeps that workspace untouched)
+      Carver cf(const_cast<void*>(sink.fwd_state));
+      FwdWs fw;
+      carve_fwd(cf, T, D, V, dtype, &fw);
+      w.rows = fw.rows; w.n_rows = fw.n_rows; w.targets_c = fw.targets_c; w.Hs = fw.Hs;
+    } else {
+      GC_TRY(launch_compact_rows(targets, mask, T, w.rows, w.n_rows, w.compact, st));
+      GC_TRY(launch_gather_rows(H, ldH, 2, D, T, w.rows, w.n_rows, w.Hs, cap, st));
+      GC_TRY(launch_gather_i32(targets, w.rows, w.n_rows, T, w.targets_c, st));
+    }
     GC_TRY(launch_gather_f32(lse, w.rows, w.n_rows, T, w.lse_c, st));
     GC_TRY(launch_gather_f32(w.g, w.rows, w.n_rows, T, w.g_c, st));
     GC_TRY(launch_zero_rows_unscored(targets, mask, T, dH, lddH, 2, D, st));
@@ -459,6 +499,7 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
                    w.counters + ci + 2, st));
     ci += 3;
   }
+  if (dW_bf16) GC_TRY(launch_cast_f32_bf16(w.dW_acc, D, dW_out, lddW_out, V, D, accumulate_out, st));
   return GC_OK;
 }
 
@@ -472,10 +513,10 @@ int gc_grpo_loss_bwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
                      const float* old_logp, const float* ref_logp, float clip_lo, float clip_hi,
                      float beta, int agg, const float* logp, const float* lse, float grad_loss,
                      void* dH, int64_t lddH, void* dW, int64_t lddW, int dW_dtype,
-                     int accumulate_dW, int64_t chunk_tokens, void* workspace,
-                     size_t workspace_bytes, void* cuda_stream) {
-  if (dW_dtype != GC_F32) return GC_ERR_DTYPE;
-  const DwSink sink{dW, lddW, accumulate_dW, nullptr, 0, 0};
+                     int accumulate_dW, int64_t chunk_tokens, const void* fwd_state,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (dW_dtype != GC_F32 && dW_dtype != GC_BF16) return GC_ERR_DTYPE;
+  const DwSink sink{dW, lddW, accumulate_dW, nullptr, 0, 0, dW_dtype, fwd_state};
   return loss_bwd_impl(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, cu_seqlens, R, adv,
                        old_logp, ref_logp, clip_lo, clip_hi, beta, agg, logp, lse, grad_loss, dH, lddH,
                        sink, chunk_tokens, workspace, workspace_bytes, cuda_stream);
@@ -487,10 +528,10 @@ int gc_grpo_loss_bwd_reduce_scatter(
     const int32_t* cu_seqlens, int32_t R, const float* adv, const float* old_logp,
     const float* ref_logp, float clip_lo, float clip_hi, float beta, int agg, const float* logp,
     const float* lse, float grad_loss, void* dH, int64_t lddH, float* const* dW_shards_host,
-    int32_t world, int64_t shard_rows, int64_t ld_shard, int64_t chunk_tokens, void* workspace,
-    size_t workspace_bytes, void* cuda_stream) {
+    int32_t world, int64_t shard_rows, int64_t ld_shard, int64_t chunk_tokens,
+    const void* fwd_state, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (!dW_shards_host) return GC_ERR_NULL;
-  const DwSink sink{nullptr, ld_shard, 1, dW_shards_host, world, shard_rows};
+  const DwSink sink{nullptr, ld_shard, 1, dW_shards_host, world, shard_rows, GC_F32, fwd_state};
   return loss_bwd_impl(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, cu_seqlens, R, adv,
                        old_logp, ref_logp, clip_lo, clip_hi, beta, agg, logp, lse, grad_loss, dH, lddH,
                        sink, chunk_tokens, workspace, workspace_bytes, cuda_stream);

@@ -92,6 +92,8 @@ int launch_gather_i32(const int32_t* src, const int32_t* rows, const int32_t* n_
                       int64_t T, int32_t* dst, cudaStream_t st);
 int launch_zero_rows_unscored(const int32_t* targets, const uint8_t* mask, int64_t T, void* dH,
                               int64_t lddH, int elem_bytes, int64_t D, cudaStream_t st);
+int launch_cast_f32_bf16(const float* acc, int64_t ld_acc, void* out, int64_t ld_out, int64_t V,
+                         int64_t D, int accumulate, cudaStream_t st);
 int launch_validate_targets(const int32_t* targets, const uint8_t* mask, int64_t T, int64_t V,
                             unsigned long long* n_bad_dev, cudaStream_t st);
 

@@ -381,6 +381,64 @@ int launch_zero_rows_unscored(const int32_t* targets, const uint8_t* mask, int64
   return GC_OK;
 }
 
+// dW fp32 -> bf16 ("dW fp32->bf16 cast -- HBM bandwidth"): out[v, :] =
+// bf16(acc[v, :] (+ out[v, :])), rounded once.  8 elements per thread when rows are 16-byte
+// aligned (D % 8 == 0), else element-wise.
+__global__ void __launch_bounds__(256)
+k_cast_f32_bf16(const float* __restrict__ acc, int64_t ld_acc, __nv_bfloat16* __restrict__ out,
+                int64_t ld_out, int64_t V, int64_t D, int accumulate, int vec) {
+  if (vec) {
+    const int64_t per_row = D >> 3, n = V * per_row;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t v = i / per_row, d = (i - v * per_row) << 3;
+      const float4 a = __ldcs(reinterpret_cast<const float4*>(acc + v * ld_acc + d));
+      const float4 b = __ldcs(reinterpret_cast<const float4*>(acc + v * ld_acc + d + 4));
+      float x[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+      uint4* dst = reinterpret_cast<uint4*>(out + v * ld_out + d);
+      if (accumulate) {
+        const uint4 o = *dst;
+        const __nv_bfloat162* ob = reinterpret_cast<const __nv_bfloat162*>(&o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float2 f = __bfloat1622float2(ob[j]);
+          x[2 * j] += f.x;
+          x[2 * j + 1] += f.y;
+        }
+      }
+      uint4 r;
+      __nv_bfloat162* rb = reinterpret_cast<__nv_bfloat162*>(&r);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rb[j] = __floats2bfloat162_rn(x[2 * j], x[2 * j + 1]);
+      *dst = r;
+    }
+  } else {
+    const int64_t n = V * D;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t v = i / D, d = i - v * D;
+      float x = acc[v * ld_acc + d];
+      if (accumulate) x += __bfloat162float(out[v * ld_out + d]);
+      out[v * ld_out + d] = __float2bfloat16_rn(x);
+    }
+  }
+}
+
+int launch_cast_f32_bf16(const float* acc, int64_t ld_acc, void* out, int64_t ld_out, int64_t V,
+                         int64_t D, int accumulate, cudaStream_t st) {
+  if (V <= 0 || D <= 0) return GC_OK;
+  const int vec = (D % 8 == 0 && ld_acc % 4 == 0 && ld_out % 8 == 0 &&
+                   (reinterpret_cast<uintptr_t>(acc) & 15) == 0 &&
+                   (reinterpret_cast<uintptr_t>(out) & 15) == 0) ? 1 : 0;
+  int64_t blocks = ceil_div(V * D / (vec ? 8 : 1), 256);
+  if (blocks > kNumSMs * 16) blocks = kNumSMs * 16;
+  if (blocks < 1) blocks = 1;
+  k_cast_f32_bf16<<<(unsigned)blocks, 256, 0, st>>>(acc, ld_acc, static_cast<__nv_bfloat16*>(out),
+                                                    ld_out, V, D, accumulate, vec);
+  GC_CUDA_TRY(cudaGetLastError());
+  return GC_OK;
+}
+
 __global__ void k_validate_targets(const int32_t* __restrict__ targets,
                                    const uint8_t* __restrict__ mask, int64_t T, int64_t V,
                                    unsigned long long* __restrict__ n_bad) {

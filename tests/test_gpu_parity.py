@@ -617,3 +617,46 @@ def test_gather_1d_never_writes_past_max_rows(B):
                                   C.c_void_p(torch.cuda.current_stream().cuda_stream)))
     torch.cuda.synchronize()
     assert torch.equal(buf[:40], rows[:40]) and bool((buf[40:] == -7).all())
+
+
+def test_bf16_dw_output_and_forward_state_reuse(B):
+    """dW_dtype = bf16 (SURVEY.md sec 8(c) reading 13: accumulated in fp32 across the dS chunks,
+    rounded ONCE at the end): equals the fp32 dW rounded to bf16 bit for bit, matches the oracle,
+    and accumulate_dW adds with one rounding.  fwd_state: the backward reusing the forward's row
+    selection gives bit-identical results to the backward that recomputes it."""
+    w = I.reduced(I.CONFIGS[2], D=256, V=2048 + 40, groups=2, group_size=4, seq_len=150, prompt_len=30,
+                  old_std=0.3)
+    b = make_batch(w, seed=12, device="cuda")
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref)
+    adv, _ = B.gc_grpo_advantages(b.rewards_t, b.go_t)
+    f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t, w.clip_lo,
+                           w.clip_hi, w.beta)
+    args = (b.H, b.W, b.y, b.mask_t, w.tau, b.cu_t, adv, b.old_t, b.ref_t, f["logp"], f["lse"],
+            w.clip_lo, w.clip_hi, w.beta)
+    for chunk in (256, 512, 0):
+        dH32, dW32 = B.gc_grpo_loss_bwd(*args, chunk_tokens=chunk)
+        dH16, dW16 = B.gc_grpo_loss_bwd(*args, chunk_tokens=chunk, dW_dtype=torch.bfloat16)
+        assert dW16.dtype == torch.bfloat16
+        assert torch.equal(dW16, dW32.to(torch.bfloat16)) and torch.equal(dH16, dH32)
+        assert rel_fro(dW16.float().cpu().numpy(), ref["dW"]) <= TOL_GRAD_BF16
+        # accumulate: out = bf16(out + sum), one rounding
+        base = (torch.randn_like(dW32) * dW32.abs().mean()).to(torch.bfloat16)
+        _, acc = B.gc_grpo_loss_bwd(*args, chunk_tokens=chunk, dW=base.clone(), accumulate_dW=True)
+        assert torch.equal(acc, (base.float() + dW32).to(torch.bfloat16))
+        # a padded bf16 dW view: the padding is never written
+        buf = torch.full((w.V, w.D + 8), 3.0, dtype=torch.bfloat16, device="cuda")
+        B.gc_grpo_loss_bwd(*args, chunk_tokens=chunk, dW=buf[:, :w.D])
+        assert torch.equal(buf[:, :w.D], dW16) and bool((buf[:, w.D:] == 3.0).all())
+        # forward-state reuse
+        dH_r, dW_r = B.gc_grpo_loss_bwd(*args, chunk_tokens=chunk, fwd_state=f["state"])
+        assert torch.equal(dH_r, dH32) and torch.equal(dW_r, dW32)
+    # fp32 (SIMT) path with bf16 dW (D not a multiple of 8: element-wise cast)
+    w0 = I.reduced(I.CONFIGS[0], D=36, V=300, groups=1, group_size=3, seq_len=9)
+    b0 = make_batch(w0, seed=1, device="cuda")
+    adv0, _ = B.gc_grpo_advantages(b0.rewards_t, b0.go_t)
+    f0 = B.gc_grpo_loss_fwd(b0.H, b0.W, b0.y, None, 1.0, b0.cu_t, adv0, b0.old_t, b0.ref_t)
+    a0 = (b0.H, b0.W, b0.y, None, 1.0, b0.cu_t, adv0, b0.old_t, b0.ref_t, f0["logp"], f0["lse"])
+    _, d32 = B.gc_grpo_loss_bwd(*a0)
+    _, d16 = B.gc_grpo_loss_bwd(*a0, dW_dtype=torch.bfloat16)
+    assert torch.equal(d16, d32.to(torch.bfloat16))

@@ -1,21 +1,33 @@
 #!/usr/bin/env python
 """bench.py -- scored tokens/s of the RLHF scoring hot path on B200 (BASELINE.json:metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg4|cfg0]
-                    [--impl ours|reference] [--no-extras]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg4|cfg0]
+                    [--impl ours|reference] [--no-extras] [--arm fused|nccl] [--dry-run]
 
-A step is one pass of the hot path over one synthetic micro-batch of the named workload
-(default cfg1 = BASELINE.json configs[1], the configuration the metric is quoted on: forward-only
-scoring of 16384 tokens, hidden 3584, vocab 152064, bf16).  Backward-capable workloads (cfg2,
-cfg4, cfg0) run advantages -> loss forward -> loss backward per step.  One JSON line on stdout.
+A step is one pass of the hot path over one synthetic micro-batch of the named workload.
+BASELINE.json:metric ("scored tokens/sec (fwd and fwd+bwd) on 1 B200") names no configuration, so
+the headline workload is configs[1] (the tier rule's default: forward-only scoring of 16384 tokens,
+hidden 3584, vocab 152064, bf16).  The same JSON line carries, under "workloads", the metric's
+fwd+bwd half on configs[2] (8B-class training micro-batch), configs[4] (large-vocab stress) and
+configs[3] (long-tail dynamic-sampling step), each with one roofline object per contraction kind
+and -- for configs[2] -- the end-to-end figure from host buffers.  Backward-capable workloads run
+advantages -> loss forward -> loss backward per step.  One JSON line on stdout.
 
-N > 1: launched under torch.distributed.run, one rank per GPU; whole groups are sharded across
-ranks (every rank scores its own micro-batch, weak scaling), no data-path collective.
+N > 1: one rank per GPU under torch.distributed.run (bench.py re-executes itself under it when
+--gpus N > 1 and WORLD_SIZE is not set).  Whole groups are sharded across ranks -- every rank
+scores its own micro-batch, weak scaling.  Scoring (forward) needs no data-path collective; a
+training workload (cfg2 / cfg4) at N > 1 exchanges dW every step: `--arm fused` (default) runs
+gc_grpo_loss_bwd_reduce_scatter, whose dW contraction reduce-adds its tiles straight into the
+owning rank's shard over NVLink; `--arm nccl` runs the plain backward followed by an NCCL
+reduce-scatter; the line reports both.
 `--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+`--dry-run` (CPU, gloo): starts the ranks, runs the timing reductions on fake numbers and prints
+the line -- the launch path without a GPU.
 """
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import subprocess
@@ -32,6 +44,9 @@ sys.path.insert(0, ROOT)
 from paper_2507_22789_b200 import inputs as I  # noqa: E402
 
 WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4}
+KIND_NAMES = {"fwd_stats": "a2+a3 forward H.W^T + online log-softmax epilogue",
+              "recompute_ds": "a10 recompute H.W^T + dS epilogue",
+              "dh": "a11 dH = dS.W", "dw": "a12 dW += dS^T.H"}
 SMI_FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
@@ -126,12 +141,16 @@ def detie_old(policy_logp, old, clip_lo, clip_hi, margin=1e-4):
 
 
 class DeviceBatch:
-    def __init__(self, w: I.Workload, seed: int, device):
+    def __init__(self, w: I.Workload, seed: int, device, w_seed=None):
+        """w_seed: seed of the replicated weight W (multi-GPU: the same on every rank, while the
+        tokens follow `seed`)."""
         self.w = w
         lay = I.make_layout(w, seed)
         self.lay = lay
         self.T = lay.T
         self.H, self.W = I.make_hw(lay.T, w.D, w.V, w.dtype, seed, device)
+        if w_seed is not None:
+            _, self.W = I.make_hw(1, w.D, w.V, w.dtype, w_seed, device)
         self.y = I.sample_targets(self.H, self.W, w.tau, seed)
         self.mask = None if lay.mask.all() else torch.from_numpy(lay.mask).to(device)
         self.n_scored = int(((lay.mask != 0) & (self.y.cpu().numpy() >= 0)).sum())
@@ -147,11 +166,21 @@ class DeviceBatch:
             self.dW = torch.empty(w.V, w.D, dtype=torch.float32, device=device)
 
 
+def _bwd_chunk_T(B, T, w):
+    # rows of the dS buffer the library picks: difference of two workspace queries
+    a = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 0)
+    c256 = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 256)
+    ld = -(-w.V // 64) * 64
+    return 256 + (a - c256) // (ld * 2)
+
+
 def make_step(B, b: DeviceBatch):
-    """Returns (step_fn, launches_per_step, dominant_fn).  All work goes through the C ABI."""
+    """Returns (step_fn, kernel launches per step).  All work goes through the C ABI."""
     w = b.w
     compact = b.mask is not None
     tc = w.dtype == "bf16"
+    # forward: tcgen05 kernel + combine (+ row selection: count, scan, scatter, H gather, target
+    # gather, zero-fill of unscored outputs); SIMT: one kernel
     fwd_launches = (2 + (6 if compact else 0)) if tc else 1
     if not w.backward:
         def step():
@@ -167,15 +196,17 @@ def make_step(B, b: DeviceBatch):
         f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
                                w.clip_hi, w.beta)
         B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f["logp"],
-                           f["lse"], w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW)
+                           f["lse"], w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW,
+                           fwd_state=f["state"])
         return f["out5"]
-    # launches: advantages 1, fwd, loss 3, bwd: loss 3 + compaction 8 + 3 per chunk (or SIMT 2)
+    # launches: advantages 1, fwd, loss 1 (one cooperative launch), bwd: loss 1 + (row selection
+    # reused from the forward) 2 small gathers + dH zero-fill + 3 contractions per chunk (SIMT: 2)
     if tc:
-        n_chunks = -(-b.T // _bwd_chunk(B, b))
-        bwd = 3 + (8 if compact else 0) + 3 * n_chunks
+        n_chunks = -(-b.T // _bwd_chunk_T(B, b.T, w))
+        bwd = 1 + (3 if compact else 0) + 3 * n_chunks
     else:
-        bwd = 3 + 2
-    return step, 1 + fwd_launches + 3 + bwd
+        bwd = 1 + 2
+    return step, 1 + fwd_launches + 1 + bwd
 
 
 def make_step_dynamic_sampling(B, b):
@@ -184,7 +215,6 @@ def make_step_dynamic_sampling(B, b):
     targets, old / ref log-probs -> forward + backward on the kept batch.  Everything runs on the
     device every step; only the kept sizes (fixed by the seeded rewards) are read once at set-up."""
     w = b.w
-    R = b.cu.numel() - 1
     adv_all, keep = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, True)
     plan = B.gc_balance_plan(b.cu, b.go, keep, 0, 1, w.group_size, 1234, True, n_tokens_max=b.T)
     Tk, Rk = int(plan["n_tokens"].item()), int(plan["n_kept"].item())
@@ -208,25 +238,8 @@ def make_step_dynamic_sampling(B, b):
                            w.clip_lo, w.clip_hi, w.beta, dH=dH, dW=b.dW)
         return f["out5"]
     n_chunks = -(-Tk // _bwd_chunk_T(B, Tk, w))
-    # advantages 1 + plan 7 (+ memset) + gathers 5 + fwd 2 + loss 3 + bwd: loss 3 + 3 per chunk
-    return step, 1 + 7 + 5 + 2 + 3 + 3 + 3 * n_chunks
-
-
-def _bwd_chunk_T(B, T, w):
-    a = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 0)
-    c256 = B.workspace_bytes(B.GC_OP_LOSS_BWD, T, w.D, w.V, B.GC_BF16, 256)
-    ld = -(-w.V // 64) * 64
-    return 256 + (a - c256) // (ld * 2)
-
-
-def _bwd_chunk(B, b):
-    # rows of the dS buffer the library picks: difference of two workspace queries
-    w = b.w
-    dt = B.GC_BF16
-    a = B.workspace_bytes(B.GC_OP_LOSS_BWD, b.T, w.D, w.V, dt, 0)
-    c256 = B.workspace_bytes(B.GC_OP_LOSS_BWD, b.T, w.D, w.V, dt, 256)
-    ld = -(-w.V // 64) * 64
-    return 256 + (a - c256) // (ld * 2)
+    # advantages 1 + plan 7 + gathers 5 + fwd 2 + loss 1 + bwd: loss 1 + 3 per chunk
+    return step, 1 + 7 + 5 + 2 + 1 + 1 + 3 * n_chunks
 
 
 def timed_region(step, steps, warmup, dist_on, B=None):
@@ -261,41 +274,73 @@ def timed_region(step, steps, warmup, dist_on, B=None):
     return total_ms, per, kinds
 
 
-def cpu_baseline(w: I.Workload, budget_tokens: int, seed=0, min_seconds=10.0):
-    """The oracle, as it stands, on a bounded sample of the workload, on this box's host cores."""
+# --------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------
+def _oracle_sample(w: I.Workload, n_tokens: int, seed=0):
+    """A bounded sample of the workload for the oracle: full D and V, n_tokens tokens of one group."""
     import oracle as O
-    from threadpoolctl import threadpool_info
-    n = max(1, min(budget_tokens, w.seq_len if w.seq_len else budget_tokens))
-    ws = I.reduced(w, groups=1, group_size=2, seq_len=max(n // 2, 1), prompt_len=0)
+    full = I.make_layout(w, seed).T
+    ws = w if n_tokens >= full else I.reduced(w, groups=1, group_size=2, seq_len=max(n_tokens // 2, 1),
+                                              prompt_len=0)
     lay = I.make_layout(ws, seed)
     H, W = I.make_hw(lay.T, ws.D, ws.V, ws.dtype, seed, "cpu")
     y = I.sample_targets(H, W, ws.tau, seed).numpy()
     H64 = H.float().numpy().astype(np.float64)
     W64 = W.float().numpy().astype(np.float64)
-    rew = np.array([1.0, 0.0], dtype=np.float32)
+    rew = I.make_rewards(ws, seed) if n_tokens >= full else np.array([1.0, 0.0], dtype=np.float32)
     old = ref = None
     if w.backward:
         lp = O.token_logprobs(H64, W64, y, None, ws.tau)[0]
         old = I.perturb_logp(lp, ws.old_std, 1)
         ref = I.perturb_logp(lp, ws.ref_std, 2)
-    reps = 0
-    t0 = time.perf_counter()
-    while True:                       # repeat the sample until about 10 s of CPU work is done
+
+    def step():
         adv, _ = O.grpo_advantages(rew, lay.group_offsets, 1e-6)
         if w.backward:
-            O.grpo_forward_backward(H64, W64, y, None, ws.tau, lay.cu_seqlens, adv, old, ref,
-                                    ws.clip_lo, ws.clip_hi, ws.beta)
+            O.grpo_forward_backward(H64, W64, y, lay.mask if not lay.mask.all() else None, ws.tau,
+                                    lay.cu_seqlens, adv, old, ref, ws.clip_lo, ws.clip_hi, ws.beta)
         else:
             O.token_logprobs(H64, W64, y, None, ws.tau)
+    return step, lay.T, ws
+
+
+def _time_oracle(step, tokens, min_seconds, max_reps=64):
+    reps = 0
+    t0 = time.perf_counter()
+    while True:
+        step()
         reps += 1
         dt = time.perf_counter() - t0
-        if dt >= min_seconds or reps >= 64:
+        if dt >= min_seconds or reps >= max_reps:
             break
+    return tokens * reps / dt, reps, dt
+
+
+def cpu_baseline(w: I.Workload, budget_tokens: int):
+    """The oracle, as it stands, on this box's host cores, on a bounded sample of the workload:
+    with every core numpy's BLAS uses, with ONE thread, and configs[0] in full (SURVEY.md sec 8(d)
+    "Oracle timing").  About 25 s of CPU work in total."""
+    from threadpoolctl import threadpool_info, threadpool_limits
+    step, T, ws = _oracle_sample(w, budget_tokens)
+    kind = "fwd+bwd" if w.backward else "fwd"
+    step()                                                 # touch the pages once
+    v_all, reps, dt = _time_oracle(step, T, 10.0)
     threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
-    return dict(value=lay.T * reps / dt, unit="scored tokens/s", cores=int(threads), kind="oracle",
-                sample=f"{reps} x {lay.T} tokens of {w.name} (full D={w.D}, V={w.V}), "
-                       f"{'fwd+bwd' if w.backward else 'fwd'}, {dt:.1f} s, fp64 numpy",
-                seconds=dt)
+    with threadpool_limits(limits=1):
+        v_one, reps1, dt1 = _time_oracle(step, T, 6.0, max_reps=8)
+    step0, T0, _ = _oracle_sample(I.CONFIGS[0], 1 << 30)
+    step0()
+    v0, reps0, dt0 = _time_oracle(step0, T0, 2.0, max_reps=200)
+    return dict(value=v_all, unit="scored tokens/s", cores=int(threads), kind="oracle",
+                sample=f"{reps} x {T} tokens of {w.name} (full D={w.D}, V={w.V}), {kind}, "
+                       f"{dt:.1f} s, fp64 numpy",
+                seconds=dt,
+                one_thread=dict(value=v_one, cores=1,
+                                sample=f"{reps1} x {T} tokens, {dt1:.1f} s, BLAS limited to 1 thread"),
+                config0_full=dict(value=v0, cores=int(threads), unit="scored tokens/s",
+                                  sample=f"{reps0} x configs[0] in full (T={T0}, D=256, V=4096, "
+                                         f"fp64), fwd+bwd, {dt0:.1f} s"))
 
 
 def run_reference(args, w):
@@ -303,43 +348,25 @@ def run_reference(args, w):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle as O
     from threadpoolctl import threadpool_info
-    n_tok = 64 if w.D * w.V > 1e8 else w.groups * w.group_size * max(w.seq_len, 1)
-    ws = w if n_tok >= I.make_layout(w, 0).T else I.reduced(w, groups=1, group_size=2,
-                                                             seq_len=n_tok // 2, prompt_len=0)
-    lay = I.make_layout(ws, 0)
-    H, W = I.make_hw(lay.T, ws.D, ws.V, ws.dtype, 0, "cpu")
-    y = I.sample_targets(H, W, ws.tau, 0).numpy()
-    H64 = H.float().numpy().astype(np.float64)
-    W64 = W.float().numpy().astype(np.float64)
-    rew = I.make_rewards(ws, 0)
-    lp = O.token_logprobs(H64, W64, y, None, ws.tau)[0]
-    old, ref = I.perturb_logp(lp, ws.old_std, 1), I.perturb_logp(lp, ws.ref_std, 2)
-
-    def step():
-        adv, _ = O.grpo_advantages(rew, lay.group_offsets, 1e-6)
-        if w.backward:
-            O.grpo_forward_backward(H64, W64, y, None, ws.tau, lay.cu_seqlens, adv, old, ref,
-                                    ws.clip_lo, ws.clip_hi, ws.beta)
-        else:
-            O.token_logprobs(H64, W64, y, None, ws.tau)
+    n_tok = 64 if w.D * w.V > 1e8 else 1 << 30
+    step, T, ws = _oracle_sample(w, n_tok)
     for _ in range(args.warmup):
         step()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         step()
     dt = time.perf_counter() - t0
-    val = lay.T * args.steps / dt
+    val = T * args.steps / dt
     threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
     unit = "scored tokens/s"
-    sample = f"{lay.T} tokens per step of {w.name} (full D={w.D}, V={w.V}), fp64 numpy oracle"
+    sample = f"{T} tokens per step of {w.name} (full D={w.D}, V={w.V}), fp64 numpy oracle"
     print(json.dumps({
         "impl": "reference", "metric": metric_name(w), "value": val, "unit": unit,
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(w, lay.T, args.gpus),
+        "config": workload_config(w, T, args.gpus),
         "cpu_baseline": dict(value=val, unit=unit, cores=int(threads), kind="oracle", sample=sample),
         "e2e": dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
     }))
@@ -349,17 +376,22 @@ def metric_name(w):
     return "scored tokens/sec (" + ("fwd+bwd" if w.backward else "fwd") + ")"
 
 
-def workload_config(w, T, n_gpus):
+def workload_config(w, T, n_gpus, exchange="none"):
     return {"workload": w.name, "tokens_per_gpu": T, "hidden": w.D, "vocab": w.V,
             "groups": w.groups, "group_size": w.group_size, "temperature": w.tau,
             "pass": "fwd+bwd" if w.backward else "fwd",
-            "parallelism": f"dp{n_gpus} (whole groups per rank, no data-path collective)",
+            "parallelism": f"dp{n_gpus} (whole groups per rank, W replicated; data-path "
+                           f"collective: {exchange})",
             "l2": "inputs exceed L2 (W alone is larger than 126 MB); no flush needed"}
 
 
+# --------------------------------------------------------------------------------------------
+# rooflines
+# --------------------------------------------------------------------------------------------
 def load_traffic(workload, kind):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the named kernel kind, from the
-    committed `ncu --set full` capture (profiles/roofline_traffic.csv; profiles/*.md say how)."""
+    committed `ncu --set full` capture (profiles/roofline_traffic.csv; profiles/*.md say how) --
+    not from this run: a run under a profiler is never a bench value."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if not os.path.exists(p):
         return None
@@ -370,39 +402,48 @@ def load_traffic(workload, kind):
     return None
 
 
-def roofline(w, tokens, steps, kinds, step_ms, long_run, peaks):
-    """Roofline of the dominant kernel: algorithmic flops per launch / its average launch duration,
-    measured with CUDA events on the launch stream inside the timed region (gc_kernel_timing_*)."""
+def rooflines(w, tokens, steps, kinds, total_ms, peaks):
+    """One roofline object per contraction kind: algorithmic flops per launch (2 T_scored D V per
+    pass / launches per pass) / the kernel's average launch duration, measured with CUDA events
+    that the library records around each contraction launch on the launch stream inside the timed
+    region (gc_kernel_timing_*).  Peak: measured cuBLAS bf16 -- burst for a timed region under 1 s,
+    sustained otherwise; both fractions and the nominal-2250 fraction are printed."""
+    long_run = total_ms > 1000.0
     peak = peaks["sustained"] if long_run else peaks["burst"]
-    pass_flops = 2.0 * tokens * w.D * w.V              # one contraction pass over the scored rows
-    per_kind = {}
+    pass_flops = 2.0 * tokens * w.D * w.V
+    out = []
     for k, (ms, n) in (kinds or {}).items():
-        if n:
-            per_kind[k] = {"ms_per_step": ms / steps, "launches_per_step": n / steps,
-                           "tflops": pass_flops * steps / (ms * 1e-3) / 1e12}
-    if not per_kind:                                   # fp32 SIMT workload (cfg0): no contraction
-        return {"bound": "tensor", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None,
+        if not n:
+            continue
+        launches_per_step = n / steps
+        launch_ms = ms / n
+        flops_per_launch = pass_flops / launches_per_step
+        achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
+        out.append({
+            "workload": w.name, "kind": k, "bound": "tensor",
+            "kernel": f"tc::k_tc_gemm [{k}: {KIND_NAMES[k]}]",
+            "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "peak_kind": ("sustained" if long_run else "burst") + " cuBLAS bf16, " + peaks["source"],
+            "frac_of_burst": achieved / peaks["burst"],
+            "frac_of_sustained": achieved / peaks["sustained"],
+            "frac_of_nominal_2250": achieved / 2250.0,
+            "flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
+            "launches_per_step": launches_per_step, "ms_per_step": ms / steps,
+            "traffic": load_traffic(w.name, k),
+            "traffic_source": "committed ncu --set full capture (profiles/), not this run",
+        })
+    return out
+
+
+def dominant(roofs, step_ms):
+    if not roofs:
+        return {"bound": "tensor", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None,
                 "traffic": None, "note": "fp32 SIMT parity workload: latency bound, no roofline"}
-    dom = max(per_kind, key=lambda k: per_kind[k]["ms_per_step"])
-    d = per_kind[dom]
-    launch_ms = d["ms_per_step"] / d["launches_per_step"]
-    flops_per_launch = pass_flops / d["launches_per_step"]
-    achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
-    kernel_share = sum(v["ms_per_step"] for v in per_kind.values()) / step_ms
-    return {
-        "bound": "tensor", "kernel": f"tc::k_tc_gemm [{dom}] (tcgen05 contraction + fused epilogue)",
-        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "peak_kind": ("sustained" if long_run else "burst") + " cuBLAS bf16, " + peaks["source"],
-        "frac_of_burst": achieved / peaks["burst"],
-        "frac_of_sustained": achieved / peaks["sustained"],
-        "frac_of_nominal_2250": achieved / 2250.0,
-        "flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
-        "traffic": load_traffic(w.name, dom),
-        "kernels": per_kind, "contraction_share_of_step": kernel_share,
-        "step_tflops": pass_flops * (4 if w.backward else 1) / (step_ms * 1e-3) / 1e12,
-        "note": "launch duration = CUDA events recorded by the library around each contraction "
-                "launch on the launch stream, inside the timed region",
-    }
+    d = dict(max(roofs, key=lambda r: r["ms_per_step"]))
+    d["contraction_share_of_step"] = sum(r["ms_per_step"] for r in roofs) / step_ms
+    d["note"] = ("launch duration = CUDA events recorded by the library around each contraction "
+                 "launch on the launch stream, inside the timed region")
+    return d
 
 
 def hbm_kernels(B, device, peaks):
@@ -428,18 +469,23 @@ def hbm_kernels(B, device, peaks):
     ref = logp + 0.1 * torch.randn(T, device=device, generator=g)
     y = torch.randint(0, 1000, (T,), device=device, dtype=torch.int32, generator=g)
     # cfg2's layout scaled up: samples of 1024 tokens = 256 prompt (mask 0) + 768 response tokens;
-    # and a stress layout of 16-token responses (a response boundary in every other thread)
+    # and a stress layout of 16-token responses
     mask = ((torch.arange(T, device=device) % 1024) >= 256).to(torch.uint8)
-    for name, seqlen in (("token_loss_and_grad", 1024), ("token_loss_and_grad_16_token_responses", 16)):
+    for seqlen in (1024, 16):
         R = T // seqlen
         cu = torch.arange(0, T + 1, seqlen, device=device, dtype=torch.int32)
         adv = torch.randn(R, device=device, generator=g)
-        ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv))
-        # reads logp, old, ref, target (4 B each) + mask (1 B), writes g (4 B); the integer count
-        # pass that fixes the normaliser re-reads target + mask (5 B)
-        gbs = 26.0 * T / ms / 1e6
-        out[name] = {"tokens": T, "responses": R, "bytes_per_token": 26, "ms": ms, "gbs": gbs,
-                     "frac": gbs / peaks["hbm"]}
+        for agg, agg_name in ((0, "token_mean"), (1, "seq_mean")):
+            ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv, agg=agg))
+            # per token: logp, old, ref, target (4 B each) + mask (1 B) read, g (4 B) written, and
+            # the count phase that fixes the normaliser re-reads target + mask (5 B) = 26 B; per
+            # response: cu_seqlens + advantage (8 B), and for seq-mean the per-response count
+            # (zeroed, added to, read twice: 16 B) and cu_seqlens once more (4 B)
+            per_tok = 26.0 + (8.0 + (20.0 if agg else 0.0)) / seqlen
+            gbs = per_tok * T / ms / 1e6
+            out[f"loss_and_grad_{agg_name}_{seqlen}_token_responses"] = {
+                "tokens": T, "responses": R, "bytes_per_token": per_tok, "ms": ms, "gbs": gbs,
+                "frac": gbs / peaks["hbm"], "launches": 1}
     del logp, old, ref, y, mask, cu, adv
     T2, D = 1 << 19, 4096
     H = torch.randn(T2, D, device=device, generator=g).to(torch.bfloat16)
@@ -465,7 +511,7 @@ def hbm_kernels(B, device, peaks):
 def library_baseline(b, steps=20):
     """Context only (not the product path, not the oracle): the same forward scoring the way the
     paper's own stack does it (PyTorch / Megatron-Core library calls) -- one cuBLAS
-    GEMM that materialises the [T,V] logits in bf16, then fp32 log_softmax, gather and entropy
+    GEMM that materialises the [T,V] logits in bf16, then fp32 log-softmax, gather and entropy
     in row blocks so the fp32 intermediates fit.  Reported next to the fused kernel."""
     w = b.w
     def gemm():
@@ -476,7 +522,7 @@ def library_baseline(b, steps=20):
         en = torch.empty(b.T, dtype=torch.float32, device=z.device)
         for r0 in range(0, b.T, 2048):
             zz = z[r0:r0 + 2048].float() / w.tau
-            ls = torch.log_softmax(zz, dim=-1)
+            ls = zz - torch.logsumexp(zz, dim=-1, keepdim=True)
             lp[r0:r0 + 2048] = ls.gather(1, b.y[r0:r0 + 2048].long().clamp_min(0)[:, None])[:, 0]
             en[r0:r0 + 2048] = -(ls.exp() * ls).sum(-1)
         return lp, en
@@ -498,18 +544,10 @@ def library_baseline(b, steps=20):
     return out
 
 
-def e2e_measure(B, b: DeviceBatch, steps, warmup):
-    """Same metric through the C-ABI call with HOST buffers: per step H2D of H / targets / mask
-    from pinned memory, the kernels, D2H of logp + entropy, all inside the timed region."""
-    w = b.w
-    Hh = b.H.cpu().pin_memory()
-    yh = b.y.cpu().pin_memory()
-    mh = None if b.mask is None else b.mask.cpu().pin_memory()
-    lph = torch.empty(b.T, dtype=torch.float32).pin_memory()
-    enh = torch.empty(b.T, dtype=torch.float32).pin_memory()
-
-    def step():
-        B.gc_token_logprobs_host(Hh, b.W, yh, mh, w.tau, logp_host=lph, entropy_host=enh)
+# --------------------------------------------------------------------------------------------
+# end to end from host buffers
+# --------------------------------------------------------------------------------------------
+def _event_time(step, steps, warmup):
     for _ in range(warmup):
         step()
     torch.cuda.synchronize()
@@ -519,9 +557,158 @@ def e2e_measure(B, b: DeviceBatch, steps, warmup):
         step()
     e1.record()
     torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / steps
+    return e0.elapsed_time(e1) / steps
+
+
+def e2e_forward(B, b: DeviceBatch, steps, warmup):
+    """Same metric through the C-ABI call with HOST buffers (gc_token_logprobs_host): per step H2D
+    of H / targets / mask from pinned memory (H band by band, overlapped with the contraction), the
+    kernels, D2H of logp + entropy, all inside the timed region."""
+    w = b.w
+    Hh = b.H.cpu().pin_memory()
+    yh = b.y.cpu().pin_memory()
+    mh = None if b.mask is None else b.mask.cpu().pin_memory()
+    lph = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    enh = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    ms = _event_time(lambda: B.gc_token_logprobs_host(Hh, b.W, yh, mh, w.tau, logp_host=lph,
+                                                      entropy_host=enh), steps, warmup)
     h2d = Hh.numel() * Hh.element_size() + yh.numel() * 4 + (0 if mh is None else mh.numel())
-    return ms, h2d, 2 * b.T * 4, float(lph.sum())
+    return {"value": b.n_scored / (ms * 1e-3), "unit": "scored tokens/s", "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": 2 * b.T * 4, "ms_per_step": ms,
+            "pass": "fwd (gc_token_logprobs_host: H copy overlapped band by band)",
+            "checksum_logp": float(lph.sum())}
+
+
+def e2e_train_step(B, b: DeviceBatch, steps, warmup):
+    """fwd+bwd end to end (gc_grpo_step_host): per step H, targets, mask, cu_seqlens, rewards,
+    group offsets, old / ref log-probs come from pinned host memory; out5 and dH go back to the
+    host; dW is model state and stays on the device."""
+    w = b.w
+    pin = lambda t: None if t is None else t.cpu().pin_memory()
+    Hh, yh, mh = pin(b.H), pin(b.y), pin(b.mask)
+    cuh, rwh, goh, oldh, refh = pin(b.cu), pin(b.rewards), pin(b.go), pin(b.old), pin(b.ref)
+    out5h = torch.empty(5, dtype=torch.float32).pin_memory()
+    dHh = torch.empty(b.T, w.D, dtype=b.H.dtype).pin_memory()
+    ms = _event_time(lambda: B.gc_grpo_step_host(Hh, b.W, yh, mh, w.tau, cuh, rwh, goh, oldh, refh,
+                                                 b.dW, clip_lo=w.clip_lo, clip_hi=w.clip_hi,
+                                                 beta=w.beta, out5_host=out5h, dH_host=dHh),
+                     steps, warmup)
+    h2d = sum(t.numel() * t.element_size() for t in (Hh, yh, mh, cuh, rwh, goh, oldh, refh)
+              if t is not None)
+    return {"value": b.n_scored / (ms * 1e-3), "unit": "scored tokens/s", "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": dHh.numel() * dHh.element_size() + 20, "ms_per_step": ms,
+            "pass": "fwd+bwd (gc_grpo_step_host: H copy overlapped with the forward; dH copied back "
+                    "after the backward; dW stays on the device)",
+            "loss": float(out5h[0])}
+
+
+# --------------------------------------------------------------------------------------------
+# one workload, measured
+# --------------------------------------------------------------------------------------------
+def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
+    b = DeviceBatch(w, seed=0, device=device)
+    step, launches = make_step(B, b)
+    total_ms, per, kinds = timed_region(step, steps, warmup, False, B)
+    ms = total_ms / steps
+    roofs = rooflines(w, b.n_scored, steps, kinds, total_ms, peaks)
+    passes = 4 if w.backward else 1
+    out = {"workload": w.name, "metric": metric_name(w), "value": b.n_scored / (ms * 1e-3),
+           "unit": "scored tokens/s", "ms_per_step": ms, "steps": steps, "warmup": warmup,
+           "scored_tokens": b.n_scored, "tokens": b.T, "gpu_launches_per_step": launches,
+           "step_tflops": 2.0 * b.n_scored * w.D * w.V * passes / (ms * 1e-3) / 1e12,
+           "rooflines": roofs}
+    if hasattr(b, "T_kept"):
+        out["tokens_kept_after_group_filter"] = b.T_kept
+        out["flow"] = "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"
+    if with_e2e and w.backward and not w.drop_constant_groups:
+        out["e2e"] = e2e_train_step(B, b, max(2, steps // 2), 2)
+    del b, step
+    gc.collect()
+    torch.cuda.empty_cache()
+    return out
+
+
+# --------------------------------------------------------------------------------------------
+# N > 1 training arm: the dW exchange
+# --------------------------------------------------------------------------------------------
+def make_train_step_dp(B, b, arm, world, rank):
+    """Data-parallel training step on this rank's micro-batch (W replicated).  Both arms leave, on
+    every rank, its shard [shard_rows, D] of the dW summed over ranks, scaled so that it is the
+    gradient of the global token-mean objective (dp.global_grad_scale x 1/world)."""
+    import torch.distributed as dist
+    from paper_2507_22789_b200 import dp
+    w = b.w
+    sr = dp.shard_rows_for(w.V, world)
+    shard = torch.zeros(sr, w.D, dtype=torch.float32, device=b.H.device)
+    scale = dp.global_grad_scale(b.n_scored) / world
+    if arm == "fused":
+        ptrs, keep = dp.exchange_dw_shards(shard)
+
+        def step():
+            shard.zero_()
+            torch.cuda.current_stream().synchronize()
+            dist.barrier()                              # every shard is zero before any add
+            adv, _ = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, False)
+            f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
+                                   w.clip_hi, w.beta)
+            B.gc_grpo_loss_bwd_reduce_scatter(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref,
+                                              f["logp"], f["lse"], ptrs, sr, clip_lo=w.clip_lo,
+                                              clip_hi=w.clip_hi, beta=w.beta, grad_loss=scale,
+                                              dH=b.dH, fwd_state=f["state"])
+            torch.cuda.current_stream().synchronize()
+            dist.barrier()                              # every rank's adds have landed
+            return f["out5"]
+        step.keep = keep
+        return step, shard
+    full = torch.zeros(sr * world, w.D, dtype=torch.float32, device=b.H.device)
+
+    def step():
+        adv, _ = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, False)
+        f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo,
+                               w.clip_hi, w.beta)
+        B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f["logp"], f["lse"],
+                           w.clip_lo, w.clip_hi, w.beta, grad_loss=scale, dH=b.dH, dW=full[:w.V],
+                           fwd_state=f["state"])
+        dist.reduce_scatter_tensor(shard, full)
+        return f["out5"]
+    return step, shard
+
+
+def maybe_respawn(args):
+    """--gpus N > 1 outside torch.distributed.run: start N ranks of this script (one per GPU,
+    rendezvous on 127.0.0.1) and return their exit code."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return None
+    port = os.environ.get("MASTER_PORT", "29517")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+           f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port", port,
+           os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_dry(args, w):
+    """The N-rank launch path on CPU (gloo): rendezvous, barriers, the max-time / summed-token
+    reductions, one JSON line from rank 0.  No kernel runs: value is null."""
+    import torch.distributed as dist
+    from paper_2507_22789_b200 import dp
+    rank, world, _ = dp.env_rank_world()
+    if world > 1:
+        dist.init_process_group("gloo")
+    dp.barrier()
+    lay = I.make_layout(w, rank)
+    fake_ms = 10.0 + rank
+    total_ms, tokens_all = dp.reduce_step_stats(fake_ms * args.steps, float(lay.mask.sum()))
+    grad_scale = dp.global_grad_scale(float(lay.mask.sum()))
+    dp.barrier()
+    if rank == 0:
+        print(json.dumps({"metric": metric_name(w), "value": None, "unit": "scored tokens/s",
+                          "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": total_ms / args.steps, "dry_run": True,
+                          "ranks_started": world, "tokens_all_ranks": tokens_all,
+                          "grad_scale_rank0": grad_scale,
+                          "config": workload_config(w, lay.T, world)}))
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def main():
@@ -532,12 +719,22 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true",
-                    help="skip the cpu_baseline / e2e / fwd+bwd extras (rank 0, N=1 only)")
+                    help="skip the cpu_baseline / e2e / other-workload extras (rank 0, N=1 only)")
+    ap.add_argument("--arm", default="fused", choices=["fused", "nccl"],
+                    help="N > 1 training workloads: how dW is exchanged (both are reported)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="control-plane backend (gloo: ranks may share a GPU; the NCCL arm is skipped)")
+    ap.add_argument("--dry-run", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = I.CONFIGS[WORKLOADS[args.workload]]
     if args.impl == "reference":
         return run_reference(args, w)
+    rc = maybe_respawn(args)
+    if rc is not None:
+        sys.exit(rc)
+    if args.dry_run:
+        return run_dry(args, w)
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -545,70 +742,97 @@ def main():
     dist_on = world > 1
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local_rank)
+    dev_index = local_rank % torch.cuda.device_count()
+    torch.cuda.set_device(dev_index)
+    device = torch.device("cuda", dev_index)
     if dist_on:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=device)
+        else:
+            dist.init_process_group("gloo")
     from paper_2507_22789_b200 import binding as B      # raises if libgcore.so is missing
+    from paper_2507_22789_b200 import dp
     peaks = load_peaks()
 
-    b = DeviceBatch(w, seed=rank, device=torch.device("cuda", local_rank))
-    step, launches = make_step(B, b)
-    sampler = ClockSampler(list(range(world)) if rank == 0 else [])
+    # every rank: its own tokens (seed = rank), the same W (seed 0)
+    b = DeviceBatch(w, seed=rank, device=device, w_seed=0 if dist_on else None)
+    exchange = "none"
+    dp_info = None
+    if dist_on and w.backward and not w.drop_constant_groups and w.dtype == "bf16":
+        exchange = ("dW reduce-scatter fused into the dW contraction (TMA reduce-add into peer "
+                    "shards over NVLink)" if args.arm == "fused" else "NCCL reduce-scatter of dW")
+        step, shard = make_train_step_dp(B, b, args.arm, world, rank)
+        n_chunks = -(-b.T // _bwd_chunk_T(B, b.T, w))
+        launches = 1 + (8 if b.mask is not None else 2) + 1 + 1 + (3 if b.mask is not None else 0) \
+            + 3 * n_chunks + 1
+    else:
+        step, launches = make_step(B, b)
+    sampler = ClockSampler(list(range(min(world, torch.cuda.device_count()))) if rank == 0 else [])
     if rank == 0:
         sampler.start()
     total_ms, per, kinds = timed_region(step, args.steps, args.warmup, dist_on, B)
     clocks = sampler.stop() if rank == 0 else None
     tokens = b.n_scored
-    from paper_2507_22789_b200 import dp
-    total_ms, tokens_all = dp.reduce_step_stats(total_ms, tokens)   # max time, summed tokens
-    ms_per_step = total_ms / args.steps
+    total_ms_max, tokens_all = dp.reduce_step_stats(total_ms, tokens)   # max time, summed tokens
+    ms_per_step = total_ms_max / args.steps
     value = tokens_all / (ms_per_step * 1e-3)
+
+    if exchange != "none":
+        # the other arm, same batch, for comparison; bytes a rank puts on the wire per step
+        other = "nccl" if args.arm == "fused" else "fused"
+        dp_info = {"arm": args.arm, "ms_per_step": ms_per_step,
+                   "wire_bytes_per_rank_per_step": (world - 1) / world * w.V * w.D * 4,
+                   "shard_rows": dp.shard_rows_for(w.V, world)}
+        same_gpu = world > torch.cuda.device_count()
+        if other == "nccl" and (args.dist_backend != "nccl" or same_gpu):
+            dp_info["other_arm"] = {"arm": other, "skipped": "ranks share a GPU / gloo control plane"}
+        else:
+            step2, _ = make_train_step_dp(B, b, other, world, rank)
+            k2 = max(3, args.steps // 2)
+            t2, _, _ = timed_region(step2, k2, 3, True, None)
+            t2, _ = dp.reduce_step_stats(t2, 0.0)
+            dp_info["other_arm"] = {"arm": other, "ms_per_step": t2 / k2}
 
     if rank == 0:
         step_ms = float(np.mean(per))
-        long_run = total_ms > 1000.0
-        roof = roofline(w, tokens, args.steps, kinds, step_ms, long_run, peaks)
+        roofs = rooflines(w, tokens, args.steps, kinds, total_ms, peaks)
         out = {
             "metric": metric_name(w), "value": value, "unit": "scored tokens/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32",
             "data": "synthetic",
-            "config": dict(workload_config(w, b.T, world),
+            "config": dict(workload_config(w, b.T, world, exchange),
                            **({"tokens_kept_after_group_filter": b.T_kept,
                                "flow": "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"}
                               if hasattr(b, "T_kept") else {})),
             "clocks": clocks, "gpu_launches": launches * args.steps,
-            "roofline": roof,
+            "roofline": dominant(roofs, step_ms), "rooflines": roofs,
         }
+        if dp_info:
+            out["dp_exchange"] = dp_info
         if world == 1 and not args.no_extras:
-            if w.dtype == "bf16":
-                ms, h2d, d2h, _ = e2e_measure(B, b, max(3, args.steps // 2), 3)
-                out["e2e"] = {"value": tokens / (ms * 1e-3), "unit": "scored tokens/s",
-                              "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                              "ms_per_step": ms, "pass": "fwd (gc_token_logprobs_host)"}
+            half = max(3, args.steps // 2)
+            if w.dtype == "bf16" and not w.drop_constant_groups:
+                out["e2e"] = e2e_train_step(B, b, half, 3) if w.backward else e2e_forward(B, b, half, 3)
             out["cpu_baseline"] = cpu_baseline(w, 256 if w.D * w.V > 1e8 else 1 << 30)
             if args.workload == "cfg1":
                 out["library_baseline"] = library_baseline(b)
-                out["hbm_kernels"] = hbm_kernels(B, torch.device("cuda", local_rank), peaks)
-                # the metric's second half: fwd+bwd on the 8B-class training micro-batch
-                del b
+                del b, step
+                gc.collect()
                 torch.cuda.empty_cache()
-                w2 = I.CONFIGS[2]
-                b2 = DeviceBatch(w2, seed=0, device=torch.device("cuda", local_rank))
-                step2, l2 = make_step(B, b2)
-                tot2, per2, kinds2 = timed_region(step2, max(3, args.steps // 4), 3, False, B)
-                ms2 = tot2 / max(3, args.steps // 4)
-                fl2 = 8.0 * b2.n_scored * w2.D * w2.V
-                k2 = {k: {"ms_per_step": ms / max(3, args.steps // 4)}
-                      for k, (ms, n) in kinds2.items() if n}
-                out["fwd_bwd"] = {"workload": w2.name, "value": b2.n_scored / (ms2 * 1e-3),
-                                  "kernels": k2,
-                                  "unit": "scored tokens/s", "ms_per_step": ms2,
-                                  "tflops": fl2 / (ms2 * 1e-3) / 1e12,
-                                  "frac_of_burst": fl2 / (ms2 * 1e-3) / 1e12 / peaks["burst"],
-                                  "gpu_launches_per_step": l2}
+                out["hbm_kernels"] = hbm_kernels(B, device, peaks)
+                torch.cuda.empty_cache()
+                # the metric's fwd+bwd half and the largest configs, each with its rooflines
+                wl = {}
+                for name, k, wu in (("cfg2", max(4, args.steps // 4), 3), ("cfg4", 4, 3), ("cfg3", 3, 2)):
+                    wl[name] = measure_workload(B, I.CONFIGS[WORKLOADS[name]], device, k, wu, peaks,
+                                                with_e2e=(name == "cfg2"))
+                    out["rooflines"] = out["rooflines"] + wl[name]["rooflines"]
+                out["workloads"] = wl
+                out["fwd_bwd"] = {k: wl["cfg2"][k] for k in ("workload", "value", "unit", "ms_per_step",
+                                                             "step_tflops", "gpu_launches_per_step")}
         print(json.dumps(out))
     if dist_on:
         import torch.distributed as dist

@@ -22,8 +22,8 @@
  *     (i) a write-once, atomically published cache of launch attributes per kernel and device
  *     (idempotent: host threads may race on a first launch); (ii) the measurement aid
  *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter of
- *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently).  None of it
- *     changes results.  Calls on different streams need different workspaces.
+ *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently); (iv) one side
+ *     stream and a few events per device for the *_host entry points.  None of it changes results.  Calls on different streams need different workspaces.
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V
@@ -100,15 +100,39 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
 
 /* Same computation with the per-step inputs and outputs in HOST memory (pinned for async
  * copies): H_host [T,D] dense, targets_host, mask_host (nullable) are copied to the device,
- * logp_host / entropy_host (nullable) are copied back, all on `cuda_stream`, staged in
- * `workspace` (gc_workspace_bytes(GC_OP_LOGPROBS,...) + gc_host_staging_bytes(T, D, dtype)).
- * W is model state and stays a device pointer.  Used for the end-to-end measurement. */
+ * logp_host / entropy_host (nullable) are copied back, staged in `workspace`
+ * (gc_workspace_bytes(GC_OP_LOGPROBS,...) + gc_host_staging_bytes(T, D, dtype)).  W is model state
+ * and stays a device pointer.  The H copy overlaps the contraction: H travels band by band (the
+ * forward schedule's M bands, after a short first band) on a library-owned side stream and each
+ * band is scored on `cuda_stream` as soon as it has arrived; the results are complete in stream
+ * order on `cuda_stream`.  Process-global state (iv): one side stream and a few events per device,
+ * created on first use.  Used for the end-to-end measurement. */
 size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype);
 int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int dtype,
                            const int32_t* targets_host, const uint8_t* mask_host,
                            int64_t T, int64_t D, int64_t V, float temperature,
                            float* logp_host, float* entropy_host,
                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* One whole training step of the loss head from HOST buffers (the end-to-end fwd+bwd path):
+ * copies H, targets, mask, cu_seqlens, rewards, group_offsets, old / ref log-probs to the device
+ * (H band by band, overlapped with the forward as above), then gc_grpo_advantages (population
+ * std, no group drop) -> forward -> loss -> backward, and copies out5 [5], logp (nullable) and
+ * dH [T,D] back to the host.  dW [V,D] (lddW, dW_dtype, accumulate_dW as in gc_grpo_loss_bwd) is
+ * model state and stays on the device.  Everything is ordered on `cuda_stream`.
+ * workspace: gc_step_host_workspace_bytes(T, D, V, dtype, R, G, dW_dtype). */
+size_t gc_step_host_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype, int32_t R, int32_t G,
+                                    int dW_dtype);
+int gc_grpo_step_host(const void* H_host, const void* W, int64_t ldW, int dtype,
+                      const int32_t* targets_host, const uint8_t* mask_host,
+                      int64_t T, int64_t D, int64_t V, float temperature,
+                      const int32_t* cu_seqlens_host, int32_t R,
+                      const float* rewards_host, const int32_t* group_offsets_host, int32_t G,
+                      float adv_eps, const float* old_logp_host, const float* ref_logp_host,
+                      float clip_lo, float clip_hi, float beta, int agg, float grad_loss,
+                      float* out5_host, float* logp_host, void* dH_host,
+                      void* dW, int64_t lddW, int dW_dtype, int accumulate_dW,
+                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---- group filter + GRPO advantages ("filter out prompts with the accuracy
  * equal to 1 and 0"; north_star "GRPO group-normalised advantages"; steps 4-5).

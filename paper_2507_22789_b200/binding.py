@@ -28,6 +28,7 @@ EXPORTS = [
     "gc_multi_workspace_bytes", "gc_token_logprobs_multi",
     "gc_grpo_loss_bwd_reduce_scatter",
     "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
+    "gc_step_host_workspace_bytes", "gc_grpo_step_host",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
@@ -58,6 +59,11 @@ def _load() -> C.CDLL:
     lib.gc_host_staging_bytes.argtypes = [i64, i64, ci]
     lib.gc_token_logprobs_host.argtypes = [vp, vp, i64, ci, vp, vp, i64, i64, i64, f32, vp, vp,
                                            vp, sz, vp]
+    lib.gc_step_host_workspace_bytes.restype = sz
+    lib.gc_step_host_workspace_bytes.argtypes = [i64, i64, i64, ci, i32, i32, ci]
+    lib.gc_grpo_step_host.argtypes = [vp, vp, i64, ci, vp, vp, i64, i64, i64, f32, vp, i32, vp, vp, i32,
+                                      f32, vp, vp, f32, f32, f32, ci, f32, vp, vp, vp, vp, i64, ci, ci,
+                                      vp, sz, vp]
     lib.gc_grpo_advantages.argtypes = [vp, vp, i32, f32, ci, ci, vp, vp, vp]
     lib.gc_grpo_loss_fwd.argtypes = head + loss + [vp, vp, vp, vp, vp, sz, vp]
     lib.gc_bwd_workspace_bytes.restype = sz
@@ -98,6 +104,7 @@ def _load() -> C.CDLL:
         if name not in ("gc_status_string", "gc_last_cuda_error", "gc_workspace_bytes", "gc_host_staging_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
                         "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
+                        "gc_step_host_workspace_bytes",
                         "gc_critic_workspace_bytes"):
             fn.restype = ci
     return lib
@@ -200,6 +207,33 @@ def gc_token_logprobs_host(H_host, W, targets_host, mask_host=None, temperature=
                                        _ptr(logp_host), _ptr(entropy_host), _ptr(ws), ws.numel(),
                                        _stream()))
     return logp_host, entropy_host
+
+
+def gc_grpo_step_host(H_host, W, targets_host, mask_host, temperature, cu_host, rewards_host,
+                      group_offsets_host, old_host, ref_host, dW, *, clip_lo=0.2, clip_hi=0.2,
+                      beta=0.04, agg=GC_AGG_TOKEN_MEAN, grad_loss=1.0, adv_eps=1e-6, out5_host=None,
+                      logp_host=None, dH_host=None, accumulate_dW=False):
+    """One training step of the loss head from (pinned) HOST buffers: -> (out5_host, dH_host);
+    dW [V,D] (fp32 or bf16) stays on the device.  Enqueues on the current stream; the caller
+    synchronises before reading the host outputs."""
+    T, D = H_host.shape
+    V = W.shape[0]
+    dt = dtype_code(W)
+    R, G = cu_host.numel() - 1, group_offsets_host.numel() - 1
+    assert not H_host.is_cuda and H_host.is_contiguous() and W.is_cuda and dW.is_cuda
+    if out5_host is None:
+        out5_host = torch.empty(5, dtype=torch.float32).pin_memory()
+    if dH_host is None:
+        dH_host = torch.empty(T, D, dtype=H_host.dtype).pin_memory()
+    dwt = {torch.float32: GC_F32, torch.bfloat16: GC_BF16}[dW.dtype]
+    ws = workspace(int(_lib.gc_step_host_workspace_bytes(T, D, V, dt, R, G, dwt)), W.device, "step")
+    _check(_lib.gc_grpo_step_host(
+        _ptr(H_host), _ptr(W), W.stride(0), dt, _ptr(targets_host), _ptr(mask_host), T, D, V,
+        float(temperature), _ptr(cu_host), R, _ptr(rewards_host), _ptr(group_offsets_host), G,
+        float(adv_eps), _ptr(old_host), _ptr(ref_host), float(clip_lo), float(clip_hi), float(beta),
+        int(agg), float(grad_loss), _ptr(out5_host), _ptr(logp_host), _ptr(dH_host), _ptr(dW),
+        dW.stride(0), dwt, int(accumulate_dW), _ptr(ws), ws.numel(), _stream()))
+    return out5_host, dH_host
 
 
 def gc_grpo_advantages(rewards, group_offsets, eps=1e-6, unbiased_std=False,

@@ -250,45 +250,6 @@ int gc_token_logprobs_multi(const void* H, int64_t ldH, const void* W, int64_t l
   return launch_combine_multi(partials, pl.n_split, (int64_t)cap, ay, K, T, logp, entropy, lse, st);
 }
 
-size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype) {
-  if (T < 0 || D <= 0) return 0;
-  const size_t t = (size_t)(T > 0 ? T : 1);
-  return align_up(t * (size_t)D * elem_bytes(dtype), 256) + align_up(t * 4, 256) +
-         align_up(t, 256) + 2 * align_up(t * 4, 256) + 256;
-}
-
-int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int dtype,
-                           const int32_t* targets_host, const uint8_t* mask_host, int64_t T,
-                           int64_t D, int64_t V, float temperature, float* logp_host,
-                           float* entropy_host, void* workspace, size_t workspace_bytes,
-                           void* cuda_stream) {
-  if (T < 0 || D <= 0 || V <= 0) return GC_ERR_SHAPE;
-  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return GC_ERR_DTYPE;
-  if (T == 0) return GC_OK;
-  if (!H_host || !targets_host || !logp_host || !W) return GC_ERR_NULL;
-  const size_t inner = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
-  if (!workspace || workspace_bytes < inner + gc_host_staging_bytes(T, D, dtype))
-    return GC_ERR_WORKSPACE;
-  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  Carver c(static_cast<char*>(workspace) + align_up(inner, 256));
-  const size_t hb = (size_t)T * (size_t)D * elem_bytes(dtype);
-  void* dH = c.take<uint8_t>(hb);
-  int32_t* dT = c.take<int32_t>((size_t)T);
-  uint8_t* dM = c.take<uint8_t>((size_t)T);
-  float* dLp = c.take<float>((size_t)T);
-  float* dEn = c.take<float>((size_t)T);
-  GC_CUDA_TRY(cudaMemcpyAsync(dH, H_host, hb, cudaMemcpyHostToDevice, st));
-  GC_CUDA_TRY(cudaMemcpyAsync(dT, targets_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
-  if (mask_host) GC_CUDA_TRY(cudaMemcpyAsync(dM, mask_host, (size_t)T, cudaMemcpyHostToDevice, st));
-  GC_TRY(gc_token_logprobs(dH, D, W, ldW, dtype, dT, mask_host ? dM : nullptr, T, D, V, temperature,
-                           dLp, entropy_host ? dEn : nullptr, nullptr, workspace, inner, cuda_stream));
-  GC_CUDA_TRY(cudaMemcpyAsync(logp_host, dLp, (size_t)T * 4, cudaMemcpyDeviceToHost, st));
-  if (entropy_host)
-    GC_CUDA_TRY(cudaMemcpyAsync(entropy_host, dEn, (size_t)T * 4, cudaMemcpyDeviceToHost, st));
-  return GC_OK;
-}
-
 int gc_grpo_advantages(const float* rewards, const int32_t* group_offsets, int32_t G, float eps,
                        int unbiased_std, int drop_constant_groups, float* adv, uint8_t* keep,
                        void* cuda_stream) {

@@ -138,6 +138,7 @@ struct TcPlan {            // forward / recompute schedule: items = (vocab chunk
 };
 TcPlan tc_plan_forward(int64_t T, int64_t D, int64_t V);
 size_t tc_fwd_partials_bytes(int64_t T, int64_t D, int64_t V);
+int64_t tc_forward_band_rows(int64_t T, int64_t D, int64_t V);
 int tc_forward_stats(const void* H, int64_t ldH, const void* W, int64_t ldW, int64_t T,
                      int64_t D, int64_t V, float tau, const int32_t* targets_c,
                      const int32_t* n_rows_dev, RowStat* partials, uint32_t* counter,

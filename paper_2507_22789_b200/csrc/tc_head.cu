@@ -472,6 +472,12 @@ static int pick_n_band(int64_t k_rows) {
   return (int)(nb < 1 ? 1 : nb);
 }
 
+// rows of one M band of the forward schedule (host-buffer entry points copy and score H band by band)
+int64_t tc_forward_band_rows(int64_t T, int64_t D, int64_t V) {
+  const TcPlan pl = tc_plan_forward(T, D, V);
+  return (int64_t)pick_m_band(D, pl.chunk_vtiles) * kPpc * 256;
+}
+
 size_t tc_fwd_partials_bytes(int64_t T, int64_t D, int64_t V) {
   const TcPlan pl = tc_plan_forward(T, D, V);
   const int64_t cap = ceil_div(T > 0 ? T : 1, 256) * 256;

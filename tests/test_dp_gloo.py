@@ -143,3 +143,27 @@ def test_shard_groups_balance():
             sizes = [len(p) for p in parts]
             assert max(sizes) - min(sizes) <= 1
     assert not dp.is_dist() and dp.reduce_step_stats(3.0, 5) == (3.0, 5.0)
+
+
+def test_bench_gpus_2_really_starts_two_ranks():
+    """`bench.py --gpus 2` outside torchrun re-executes itself under torch.distributed.run with two
+    ranks; --dry-run runs the launch path (rendezvous, barriers, max-time / summed-token
+    reductions) on CPU over gloo and prints one JSON line from rank 0."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR")}
+    env["MASTER_PORT"] = str(_free_port())
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry-run",
+                        "--workload", "cfg2", "--steps", "4"], capture_output=True, text=True,
+                       timeout=300, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                  # rank 0 only
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["ranks_started"] == 2 and d["dry_run"] is True
+    assert d["ms_per_step"] == 11.0                         # max over ranks of 10 + rank
+    assert d["tokens_all_ranks"] == 2 * 24576               # summed over ranks
+    assert abs(d["grad_scale_rank0"] - 1.0) < 1e-12         # equal shards

@@ -660,3 +660,42 @@ def test_bf16_dw_output_and_forward_state_reuse(B):
     _, d32 = B.gc_grpo_loss_bwd(*a0)
     _, d16 = B.gc_grpo_loss_bwd(*a0, dW_dtype=torch.bfloat16)
     assert torch.equal(d16, d32.to(torch.bfloat16))
+
+
+def test_host_entry_points_banded_copy_and_training_step(B):
+    """The *_host entry points with H long enough to travel in several bands (copy of band b + 1
+    overlapped with the scoring of band b on a side stream): log-probs against the oracle, and the
+    whole training step from host buffers (gc_grpo_step_host) against the device-resident calls
+    and the oracle."""
+    w = I.reduced(I.CONFIGS[2], D=64, V=300, groups=4, group_size=4, seq_len=2600, prompt_len=100,
+                  old_std=0.3)
+    b = make_batch(w, seed=13, device="cuda")
+    assert b.T > 2 * 16384                                  # > 2 bands of 64 M tiles
+    pin = lambda t: t.cpu().pin_memory()
+    Hh, yh, mh = pin(b.H), pin(b.y), pin(b.mask_t)
+    lph = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    enh = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    for _ in range(2):                                      # second call: staging buffers reused
+        lph.fill_(7.0)
+        B.gc_token_logprobs_host(Hh, b.W, yh, mh, w.tau, logp_host=lph, entropy_host=enh)
+        torch.cuda.synchronize()
+        lp_o, en_o, _ = O.token_logprobs(to_f64(b.H), to_f64(b.W), b.y_np, b.mask_np, w.tau)
+        assert np.abs(lph.numpy() - lp_o).max() <= TOL_LOGP_BF16
+        assert np.abs(enh.numpy() - en_o).max() <= 2 * TOL_LOGP_BF16
+    # training step from host buffers
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref)
+    dev_run = run_gpu(B, b)
+    for dw_dtype in (torch.float32, torch.bfloat16):
+        dW = torch.full((w.V, w.D), 5.0, dtype=dw_dtype, device="cuda")
+        out5_h, dH_h = B.gc_grpo_step_host(Hh, b.W, yh, mh, w.tau, pin(b.cu_t), pin(b.rewards_t),
+                                           pin(b.go_t), pin(b.old_t), pin(b.ref_t), dW,
+                                           clip_lo=w.clip_lo, clip_hi=w.clip_hi, beta=w.beta)
+        torch.cuda.synchronize()
+        o = out5_h.numpy().astype(np.float64)
+        assert o[4] == ref["n_scored"]
+        assert abs(o[0] - ref["loss"]) <= TOL_LOSS_REL * abs(ref["loss"])
+        assert rel_fro(dH_h.float().numpy(), ref["dH"]) <= TOL_GRAD_BF16
+        assert rel_fro(dW.float().cpu().numpy(), ref["dW"]) <= TOL_GRAD_BF16 + (3e-3 if dw_dtype == torch.bfloat16 else 0)
+        assert np.allclose(o[:4], dev_run["out5"].cpu().numpy()[:4], rtol=2e-5, atol=1e-7)
+        assert elem_excess(dH_h.float().numpy(), ref["dH"], **ELEM_BF16) <= 1.0

@@ -6,7 +6,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 
 See ``oracle/gcore_oracle.py`` for the functions and the passages they follow;
 ``oracle/balance_oracle.py`` holds the oracle of the repack + workload-balancing step,
-``oracle/critic_oracle.py`` the oracle of the PPO critic path (value head, GAE, value loss).
+``oracle/critic_oracle.py`` the oracle of the PPO critic path (value head, GAE, value loss),
+``oracle/attention_oracle.py`` the oracle of the all-gather-KV distributed attention (sec 4.5).
 """
 from .gcore_oracle import (  # noqa: F401
     AGG_TOKEN_MEAN,
@@ -26,3 +27,4 @@ from .gcore_oracle import (  # noqa: F401
 )
 from . import balance_oracle  # noqa: F401,E402
 from . import critic_oracle  # noqa: F401,E402
+from . import attention_oracle  # noqa: F401,E402

@@ -293,6 +293,33 @@ int gc_token_logprobs_multi(const void* H, int64_t ldH, const void* W, int64_t l
                             float temperature, float* logp, float* entropy, float* lse,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- distributed attention by all-gather of K and V.
+ * PAPER.md:209 (sec 4.5): "we implemented distributed attention based on CCL all-gather, where we
+ * first all-gather the key (K) and value (V) tensors, and then compute attention output for the
+ * local query (Q) tensor chunk"; "we process only a subset of attention heads at a
+ * time and overlap KV communication with attention computation."  Forward only.
+ * The sequence of S = sum_r shard_rows[r] tokens is cut into `world` contiguous chunks; this rank
+ * (`rank`) holds Q [S_local, Hq, head_dim] and every rank r holds K_r, V_r [shard_rows[r], Hkv,
+ * head_dim] (bf16, dense).  K_shards_host / V_shards_host: HOST arrays of `world` DEVICE pointers --
+ * this rank's own buffers or peer-mapped ones (CUDA IPC / peer access; NVLink carries the copies).
+ * For each subset of heads_per_step key/value heads the shards are gathered by the copy engines
+ * into one of two [S, heads, head_dim] buffers on a library-owned side stream while the attention
+ * kernel works on the previous subset; the peers' K/V must stay unchanged until the call has
+ * completed on `cuda_stream` (the caller synchronises the ranks around the call).
+ *   out[q, h, :] = sum_k softmax_k(scale <Q[q,h,:], K[k,g,:]>) V[k,g,:],  g = h / (Hq / Hkv),
+ * over the keys k (global positions) the query at global position q may attend:
+ *   same document (cu_seqlens [n_docs + 1] int32 on the device, global positions; NULL = one
+ *   document), k <= q if causal, and q - k < window if window > 0 (|q - k| < window when not
+ *   causal).  O [S_local, Hq, head_dim] bf16; lse [Hq, S_local] f32 nullable (natural log).
+ * head_dim = 128.  workspace: gc_attention_workspace_bytes(S_local, S, heads_per_step). */
+size_t gc_attention_workspace_bytes(int64_t S_local, int64_t S_total, int32_t heads_per_step);
+int gc_attention_allgather_kv(const void* Q, const void* const* K_shards_host,
+                              const void* const* V_shards_host, const int64_t* shard_rows_host,
+                              int32_t world, int32_t rank, int32_t Hq, int32_t Hkv, int32_t head_dim,
+                              const int32_t* cu_seqlens, int32_t n_docs, int causal, int32_t window,
+                              float scale, int32_t heads_per_step, void* O, float* lse,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* ---- the step before the path: dynamic-sampling repack + workload balancing (SURVEY.md sec
  * 8(f) NEXT-1).  PAPER.md:150 (sec 3.2): prompts whose samples are all right or all wrong are
  * filtered out; PAPER.md:201 (sec 4.4): "we simply sort data by simulated workload"; PAPER.md:205:

@@ -29,6 +29,7 @@ EXPORTS = [
     "gc_grpo_loss_bwd_reduce_scatter",
     "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
     "gc_step_host_workspace_bytes", "gc_grpo_step_host",
+    "gc_attention_workspace_bytes", "gc_attention_allgather_kv",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
 ]
 
@@ -64,6 +65,10 @@ def _load() -> C.CDLL:
     lib.gc_grpo_step_host.argtypes = [vp, vp, i64, ci, vp, vp, i64, i64, i64, f32, vp, i32, vp, vp, i32,
                                       f32, vp, vp, f32, f32, f32, ci, f32, vp, vp, vp, vp, i64, ci, ci,
                                       vp, sz, vp]
+    lib.gc_attention_workspace_bytes.restype = sz
+    lib.gc_attention_workspace_bytes.argtypes = [i64, i64, i32]
+    lib.gc_attention_allgather_kv.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(i64), i32, i32,
+                                              i32, i32, i32, vp, i32, ci, i32, f32, i32, vp, vp, vp, sz, vp]
     lib.gc_grpo_advantages.argtypes = [vp, vp, i32, f32, ci, ci, vp, vp, vp]
     lib.gc_grpo_loss_fwd.argtypes = head + loss + [vp, vp, vp, vp, vp, sz, vp]
     lib.gc_bwd_workspace_bytes.restype = sz
@@ -104,7 +109,7 @@ def _load() -> C.CDLL:
         if name not in ("gc_status_string", "gc_last_cuda_error", "gc_workspace_bytes", "gc_host_staging_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
                         "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
-                        "gc_step_host_workspace_bytes",
+                        "gc_step_host_workspace_bytes", "gc_attention_workspace_bytes",
                         "gc_critic_workspace_bytes"):
             fn.restype = ci
     return lib
@@ -507,3 +512,30 @@ def gc_grpo_loss_bwd_reduce_scatter(H, W, targets, mask, temperature, cu_seqlens
         int(shard_rows), int(ld_shard if ld_shard is not None else D), int(chunk_tokens),
         _ptr(fwd_state), _ptr(ws), ws.numel(), _stream()))
     return dH
+
+
+def gc_attention_allgather_kv(Q, K_ptrs, V_ptrs, shard_rows, rank, Hkv, cu_seqlens=None, causal=True,
+                              window=0, scale=None, heads_per_step=1, want_lse=True):
+    """Distributed attention forward (NEXT-4).  Q [S_local, Hq, 128] bf16 on the device; K_ptrs /
+    V_ptrs: per rank the device address (int) of its K / V shard [shard_rows[r], Hkv, 128] bf16 --
+    own tensors' data_ptr() or peer-mapped memory.  -> (O [S_local, Hq, 128] bf16, lse [Hq, S_local])."""
+    S_local, Hq, d = Q.shape
+    world = len(shard_rows)
+    assert Q.dtype == torch.bfloat16 and Q.is_contiguous() and int(shard_rows[rank]) == S_local
+    S = int(sum(shard_rows))
+    dev = Q.device
+    O = torch.empty_like(Q)
+    lse = torch.empty(Hq, S_local, dtype=torch.float32, device=dev) if want_lse else None
+    kp = (C.c_void_p * world)(*[C.c_void_p(int(x)) for x in K_ptrs])
+    vptr = (C.c_void_p * world)(*[C.c_void_p(int(x)) for x in V_ptrs])
+    rows = (C.c_int64 * world)(*[int(x) for x in shard_rows])
+    hs = min(int(heads_per_step), Hkv)
+    ws = workspace(int(_lib.gc_attention_workspace_bytes(S_local, S, hs)), dev, "attn")
+    n_docs = 0 if cu_seqlens is None else cu_seqlens.numel() - 1
+    if scale is None:
+        scale = 1.0 / (d ** 0.5)
+    _check(_lib.gc_attention_allgather_kv(_ptr(Q), kp, vptr, rows, world, int(rank), Hq, int(Hkv), d,
+                                          _ptr(cu_seqlens), n_docs, int(bool(causal)), int(window),
+                                          float(scale), hs, _ptr(O), _ptr(lse), _ptr(ws), ws.numel(),
+                                          _stream()))
+    return O, lse

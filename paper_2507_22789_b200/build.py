@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libgcore.so")
 SOURCES = ["api.cu", "small_kernels.cu", "simt_head.cu", "tc_head.cu", "timing.cu",
-           "balance.cu", "critic.cu", "loss.cu", "host_api.cu"]
+           "balance.cu", "critic.cu", "loss.cu", "host_api.cu", "attention.cu"]
 HEADERS = ["common.cuh", "tc_ptx.cuh", "tc_gemm.cuh", os.path.join("..", "..", "include", "gcore.h")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -1,0 +1,565 @@
+// attention.cu -- NEXT-4: the distributed attention of G-Core sec 4.5.
+// "we first all-gather the key (K) and value (V) tensors, and then compute attention
+// output for the local query (Q) tensor chunk"; "we process only a subset of
+// attention heads at a time and overlap KV communication with attention computation".
+//
+// Two parts:
+//   * gc_attention_allgather_kv (host): for each subset of key/value heads, the ranks' K/V shards
+//     (this rank's own memory or peer-mapped: CUDA IPC / peer access, NVLink carries the bytes) are
+//     gathered by the copy engines into one of two [S, heads, d] buffers on a side stream while the
+//     attention kernel works on the previous subset out of the other buffer.
+//   * k_attn_fwd: a tcgen05 flash-attention forward for one (128-query tile, query head):
+//       S_j = Q K_j^T (UMMA 128x128x16, fp32 in TMEM, two buffers), online softmax by a
+//       4-warp group (thread = query row; exp2 domain), P_j -> bf16 -> 128B-swizzled smem,
+//       PV_j = P_j V_j (V is the MN-major B operand; fp32 in TMEM, two buffers), and the output
+//       row lives in REGISTERS: O = O * 2^(m_O - m_j) + PV_j.  The MMA warp issues S_{j+1} before
+//       PV_j, so the tensor core computes the next scores while the softmax group works.
+//     Masks: per query row an allowed key interval [k_lo, k_hi) -- packed
+//     documents, causal, sliding window -- computed once by k_attn_rows; blocks outside the
+//     tile's interval are skipped, blocks inside every row's interval take no per-element test.
+#include <math.h>
+#include <mutex>
+
+#include "tc_gemm.cuh"
+
+namespace gc {
+namespace attn {
+
+constexpr int kD = 128;            // head dimension
+constexpr int kBQ = 128;           // query rows per CTA
+constexpr int kBK = 128;           // keys per block
+constexpr int kThreads = 256;
+constexpr int kTileBytes = kBQ * kD * 2;     // 32 KB: a 128 x 128 bf16 tile (two 64-wide k-blocks)
+constexpr int kSmemQ = 0;
+constexpr int kSmemK = kSmemQ + kTileBytes;
+constexpr int kSmemV = kSmemK + 2 * kTileBytes;
+constexpr int kSmemP = kSmemV + 2 * kTileBytes;
+constexpr int kSmemBar = kSmemP + 2 * kTileBytes;          // 224 KB of tiles, then the barriers
+constexpr int kSmemBytes = kSmemBar + 256 + 1024;          // + alignment slack
+static_assert(kSmemBytes <= 227 * 1024, "attention shared memory budget");
+
+struct TileMeta { int32_t kb_begin, kb_end, lo_max, hi_min; };
+
+struct Params {
+  int64_t S_local, q_off, S;
+  int32_t n_q_tiles;
+  int32_t h_begin;          // first query head of this launch
+  int32_t n_q_heads;        // query heads of this launch
+  int32_t grp;              // query heads per key/value head
+  float scale2;             // scale * log2(e)
+  const int32_t* k_lo;      // [S_local] first allowed key of each query row
+  const int32_t* k_hi;      // [S_local] one past the last allowed key
+  const TileMeta* meta;     // [n_q_tiles]
+  __nv_bfloat16* O;         // [S_local, Hq, d]
+  int64_t ldO;              // Hq * d
+  float* lse;               // [Hq, S_local] or NULL
+};
+
+// ---------------------------------------------------------------------------------------------
+// Allowed key interval of every local query row, and per 128-row tile the key blocks to visit.
+//   doc(q) from cu_seqlens (global positions; NULL = one document [0, S))
+//   causal: k <= q;  window W > 0: q - k < W (causal) or |q - k| < W (not causal)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBQ)
+k_attn_rows(int64_t S_local, int64_t q_off, int64_t S, const int32_t* __restrict__ cu, int32_t n_docs,
+            int causal, int32_t window, int32_t* __restrict__ k_lo, int32_t* __restrict__ k_hi,
+            TileMeta* __restrict__ meta) {
+  const int64_t i = (int64_t)blockIdx.x * kBQ + threadIdx.x;
+  int32_t lo = 0, hi = 0;
+  if (i < S_local) {
+    const int32_t q = (int32_t)(q_off + i);
+    int32_t d0 = 0, d1 = (int32_t)S;
+    if (cu != nullptr) {                        // largest d with cu[d] <= q
+      int a = 0, b = n_docs;
+      while (b - a > 1) {
+        const int mid = (a + b) >> 1;
+        if (cu[mid] <= q) a = mid; else b = mid;
+      }
+      d0 = cu[a];
+      d1 = cu[a + 1];
+    }
+    lo = d0;
+    hi = d1;
+    if (causal) hi = min(hi, q + 1);
+    if (window > 0) {
+      lo = max(lo, q - window + 1);
+      if (!causal) hi = min(hi, q + window);
+    }
+    k_lo[i] = lo;
+    k_hi[i] = hi;
+  }
+  // tile reductions: union of the rows' intervals (blocks to visit), intersection (no-mask blocks)
+  __shared__ int32_t s[4][kBQ / 32];
+  const bool valid = i < S_local;
+  int32_t lo_min = valid ? lo : INT32_MAX, hi_max = valid ? hi : 0;
+  int32_t lo_max = valid ? lo : 0, hi_min = valid ? hi : INT32_MAX;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo_min = min(lo_min, __shfl_xor_sync(0xffffffffu, lo_min, o));
+    hi_max = max(hi_max, __shfl_xor_sync(0xffffffffu, hi_max, o));
+    lo_max = max(lo_max, __shfl_xor_sync(0xffffffffu, lo_max, o));
+    hi_min = min(hi_min, __shfl_xor_sync(0xffffffffu, hi_min, o));
+  }
+  const int w = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) { s[0][w] = lo_min; s[1][w] = hi_max; s[2][w] = lo_max; s[3][w] = hi_min; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < kBQ / 32; ++k) {
+      s[0][0] = min(s[0][0], s[0][k]); s[1][0] = max(s[1][0], s[1][k]);
+      s[2][0] = max(s[2][0], s[2][k]); s[3][0] = min(s[3][0], s[3][k]);
+    }
+    TileMeta m;
+    m.kb_begin = s[0][0] / kBK;
+    m.kb_end = (s[1][0] + kBK - 1) / kBK;
+    if (m.kb_end < m.kb_begin) m.kb_end = m.kb_begin;
+    m.lo_max = s[2][0];
+    m.hi_min = s[3][0];
+    meta[blockIdx.x] = m;
+  }
+}
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+__device__ __forceinline__ void st_shared_v4_u32(uint32_t addr, uint32_t a, uint32_t b, uint32_t c,
+                                                 uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d)
+               : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// One CTA = one (query tile, query head).  Warps: 0 TMA producer, 1 MMA issuer, 2 TMEM allocator,
+// 4..7 softmax / output group (thread = query row).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads, 1)
+k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+           const __grid_constant__ CUtensorMap tmV, const Params p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = base + kSmemQ, sK = base + kSmemK, sV = base + kSmemV, sP = base + kSmemP;
+  const uint32_t bar = base + kSmemBar;
+  // barriers (8 bytes each)
+  const uint32_t q_full = bar;
+  auto k_full = [&](int i) { return bar + 8u * (1 + i); };
+  auto k_empty = [&](int i) { return bar + 8u * (3 + i); };
+  auto v_full = [&](int i) { return bar + 8u * (5 + i); };
+  auto v_empty = [&](int i) { return bar + 8u * (7 + i); };
+  auto s_full = [&](int i) { return bar + 8u * (9 + i); };
+  auto s_empty = [&](int i) { return bar + 8u * (11 + i); };
+  auto p_full = [&](int i) { return bar + 8u * (13 + i); };
+  auto p_empty = [&](int i) { return bar + 8u * (15 + i); };
+  auto pv_full = [&](int i) { return bar + 8u * (17 + i); };
+  auto pv_empty = [&](int i) { return bar + 8u * (19 + i); };
+  const uint32_t tmem_slot = bar + 8u * 21;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int head_local = (int)(blockIdx.x % (unsigned)p.n_q_heads);
+  const int q_tile = p.n_q_tiles - 1 - (int)(blockIdx.x / (unsigned)p.n_q_heads);   // long tiles first
+  const int hq = p.h_begin + head_local;
+  const int g_local = head_local / p.grp;            // key/value head inside the gathered buffer
+  const TileMeta tm = p.meta[q_tile];
+  const int nb = tm.kb_end - tm.kb_begin;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tmap(&tmQ);
+    ptx::prefetch_tmap(&tmK);
+    ptx::prefetch_tmap(&tmV);
+  }
+  if (warp == 1 && lane == 0) {
+    ptx::mbar_init(q_full, 1);
+    for (int i = 0; i < 2; ++i) {
+      ptx::mbar_init(k_full(i), 1);
+      ptx::mbar_init(k_empty(i), 1);
+      ptx::mbar_init(v_full(i), 1);
+      ptx::mbar_init(v_empty(i), 1);
+      ptx::mbar_init(s_full(i), 1);
+      ptx::mbar_init(s_empty(i), 4);       // one arrive per softmax warp
+      ptx::mbar_init(p_full(i), 4);
+      ptx::mbar_init(p_empty(i), 1);
+      ptx::mbar_init(pv_full(i), 1);
+      ptx::mbar_init(pv_empty(i), 4);
+    }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc<1>(tmem_slot, 512);
+    ptx::tmem_relinquish<1>();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  // TMEM columns: S0 [0,128) S1 [128,256) PV0 [256,384) PV1 [384,512)
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0 && nb > 0) {
+      const uint64_t pol_q = ptx::make_l2_policy(ptx::kL2Normal);
+      const uint64_t pol_kv = ptx::make_l2_policy(ptx::kL2EvictLast);   // K/V are re-read by every query tile
+      const int32_t q_row = q_tile * kBQ;
+      const int32_t q_col = hq * kD;
+      const int32_t kv_col = g_local * kD;
+      ptx::mbar_arrive_expect_tx(q_full, kTileBytes);
+      ptx::tma_load_2d(sQ, &tmQ, q_col, q_row, q_full, pol_q);
+      ptx::tma_load_2d(sQ + 16384, &tmQ, q_col + 64, q_row, q_full, pol_q);
+      auto load_k = [&](int j) {
+        const int st = j & 1;
+        ptx::mbar_wait(k_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
+        ptx::mbar_arrive_expect_tx(k_full(st), kTileBytes);
+        const int32_t row = (tm.kb_begin + j) * kBK;
+        const uint32_t dst = sK + st * kTileBytes;
+        ptx::tma_load_2d(dst, &tmK, kv_col, row, k_full(st), pol_kv);
+        ptx::tma_load_2d(dst + 16384, &tmK, kv_col + 64, row, k_full(st), pol_kv);
+      };
+      auto load_v = [&](int j) {
+        const int st = j & 1;
+        ptx::mbar_wait(v_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
+        ptx::mbar_arrive_expect_tx(v_full(st), kTileBytes);
+        const int32_t row = (tm.kb_begin + j) * kBK;
+        const uint32_t dst = sV + st * kTileBytes;
+        // MN-major B operand: per 64-key k-block two 64(d) x 64(keys) boxes, 8 KB apart
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+          for (int nbx = 0; nbx < 2; ++nbx)
+            ptx::tma_load_2d(dst + kb * 16384 + nbx * 8192, &tmV, kv_col + 64 * nbx, row + 64 * kb,
+                             v_full(st), pol_kv);
+      };
+      load_k(0);
+      for (int j = 0; j < nb; ++j) {
+        if (j + 1 < nb) load_k(j + 1);
+        load_v(j);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0 && nb > 0) {
+      constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kBQ, kBK, false, false);
+      constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kBQ, kD, false, true);
+      auto issue_s = [&](int j) {
+        const int st = j & 1;
+        const uint32_t ph = ((uint32_t)j >> 1) & 1u;
+        ptx::mbar_wait(k_full(st), ph);
+        ptx::mbar_wait(s_empty(st), ph ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (uint32_t)st * 128u;
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb) {
+          const uint64_t adesc = ptx::make_smem_desc(sQ + kb * 16384, false);
+          const uint64_t bdesc = ptx::make_smem_desc(sK + st * kTileBytes + kb * 16384, false);
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc_qk,
+                              (uint32_t)(kb | k));
+        }
+        ptx::umma_commit<1>(k_empty(st));      // the K stage is free once these MMAs have read it
+        ptx::umma_commit<1>(s_full(st));
+      };
+      auto issue_pv = [&](int j) {
+        const int st = j & 1;
+        const uint32_t ph = ((uint32_t)j >> 1) & 1u;
+        ptx::mbar_wait(v_full(st), ph);
+        ptx::mbar_wait(p_full(st), ph);
+        ptx::mbar_wait(pv_empty(st), ph ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + 256u + (uint32_t)st * 128u;
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb) {
+          const uint64_t adesc = ptx::make_smem_desc(sP + st * kTileBytes + kb * 16384, false);
+          const uint64_t bdesc = ptx::make_smem_desc(sV + st * kTileBytes + kb * 16384, true);
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 128),
+                              idesc_pv, (uint32_t)(kb | k));
+        }
+        ptx::umma_commit<1>(v_empty(st));
+        ptx::umma_commit<1>(p_empty(st));
+        ptx::umma_commit<1>(pv_full(st));
+      };
+      ptx::mbar_wait(q_full, 0);
+      issue_s(0);
+      for (int j = 0; j < nb; ++j) {
+        if (j + 1 < nb) issue_s(j + 1);        // the next scores run under this block's softmax
+        issue_pv(j);
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== softmax / output group =====================
+    const int q = warp & 3;
+    const int row = q * 32 + lane;
+    const int64_t i = (int64_t)q_tile * kBQ + row;           // local query row
+    const bool valid = i < p.S_local;
+    const int32_t lo = valid ? p.k_lo[i] : 0, hi = valid ? p.k_hi[i] : 0;
+    const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
+    float O[kD];
+#pragma unroll
+    for (int c = 0; c < kD; ++c) O[c] = 0.f;
+    float m_run = -1e30f;     // running maximum (log2 domain)
+    float m_O = -1e30f;       // the maximum O is relative to
+    float m_prev = -1e30f;    // the maximum PV_{j-1} is relative to
+    float l_run = 0.f;
+    const uint32_t p_row = (uint32_t)row * 128u;
+    const uint32_t sw = (uint32_t)(row & 7);
+
+    auto add_pv = [&](int j) {                 // O = O * 2^(m_O - m_j) + PV_j
+      const int st = j & 1;
+      ptx::mbar_wait(pv_full(st), ((uint32_t)j >> 1) & 1u);
+      ptx::tc_fence_after();
+      const float a = ptx::ex2(m_O - m_prev);
+      m_O = m_prev;
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch) {
+        uint32_t r[32];
+        ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(st * 128 + ch * 32), r);
+        ptx::tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 32; ++c) O[ch * 32 + c] = fmaf(O[ch * 32 + c], a, __uint_as_float(r[c]));
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(pv_empty(st));
+    };
+
+    for (int j = 0; j < nb; ++j) {
+      const int st = j & 1;
+      const uint32_t ph = ((uint32_t)j >> 1) & 1u;
+      const int32_t k0 = (tm.kb_begin + j) * kBK;
+      const bool need_mask = k0 < tm.lo_max || k0 + kBK > tm.hi_min;
+      ptx::mbar_wait(s_full(st), ph);
+      ptx::tc_fence_after();
+      // pass 1: row maximum over the allowed keys of this block
+      float mx = -INFINITY;
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch) {
+        uint32_t r[32];
+        ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r);
+        ptx::tmem_wait_ld();
+        if (need_mask) {
+#pragma unroll
+          for (int c = 0; c < 32; ++c) {
+            const int32_t k = k0 + ch * 32 + c;
+            mx = (k >= lo && k < hi) ? fmaxf(mx, __uint_as_float(r[c])) : mx;
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 32; ++c) mx = fmaxf(mx, __uint_as_float(r[c]));
+        }
+      }
+      const float m_new = fmaxf(m_run, mx * p.scale2);
+      l_run *= ptx::ex2(m_run - m_new);
+      m_run = m_new;
+      // pass 2: p = 2^(s * scale2 - m), row sum, P -> bf16 -> swizzled smem (A operand of P V)
+      ptx::mbar_wait(p_empty(st), ph ^ 1u);
+      float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch) {
+        uint32_t r[32];
+        ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r);
+        ptx::tmem_wait_ld();
+        if (ch == 3) {
+          // every read of this S buffer is done: hand it back to the MMA warp
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(s_empty(st));
+        }
+        float e[32];
+#pragma unroll
+        for (int c = 0; c < 32; ++c) {
+          float v = ptx::ex2(fmaf(__uint_as_float(r[c]), p.scale2, -m_new));
+          if (need_mask) {
+            const int32_t k = k0 + ch * 32 + c;
+            v = (k >= lo && k < hi) ? v : 0.f;
+          }
+          e[c] = v;
+        }
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
+        // 32 columns = 4 16-byte chunks of this row's 128-byte line in k-block ch / 2
+        const uint32_t pb = sP + st * kTileBytes + (uint32_t)(ch >> 1) * 16384u + p_row;
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          const uint32_t chunk = (uint32_t)((ch & 1) * 4 + cc);
+          st_shared_v4_u32(pb + ((chunk ^ sw) << 4), pack_bf16x2(e[8 * cc], e[8 * cc + 1]),
+                           pack_bf16x2(e[8 * cc + 2], e[8 * cc + 3]),
+                           pack_bf16x2(e[8 * cc + 4], e[8 * cc + 5]),
+                           pack_bf16x2(e[8 * cc + 6], e[8 * cc + 7]));
+        }
+      }
+      l_run += sum0 + sum1;
+      ptx::fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(p_full(st));
+      // the previous block's P V has been running under this softmax: fold it into O now
+      if (j > 0) add_pv(j - 1);
+      m_prev = m_new;
+    }
+    if (nb > 0) add_pv(nb - 1);
+    // out = O / l; lse = ln2 * (m + log2 l)
+    if (valid) {
+      const float inv = l_run > 0.f ? 1.0f / l_run : 0.f;
+      uint4* dst = reinterpret_cast<uint4*>(p.O + i * p.ldO + (int64_t)hq * kD);
+#pragma unroll
+      for (int c = 0; c < kD; c += 8)
+        dst[c >> 3] = make_uint4(pack_bf16x2(O[c] * inv, O[c + 1] * inv),
+                                 pack_bf16x2(O[c + 2] * inv, O[c + 3] * inv),
+                                 pack_bf16x2(O[c + 4] * inv, O[c + 5] * inv),
+                                 pack_bf16x2(O[c + 6] * inv, O[c + 7] * inv));
+      if (p.lse) p.lse[(int64_t)hq * p.S_local + i] = l_run > 0.f ? kLn2 * (m_run + log2f(l_run)) : -INFINITY;
+    }
+  }
+
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+struct SideCtx { cudaStream_t cs = nullptr; cudaEvent_t ev[6] = {}; bool ok = false; bool attr = false; };
+std::mutex g_mu;
+SideCtx g_ctx[64];
+
+int get_side(SideCtx** out) {
+  int dev = 0;
+  GC_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GC_ERR_CUDA;
+  std::lock_guard<std::mutex> lk(g_mu);
+  SideCtx& c = g_ctx[dev];
+  if (!c.ok) {
+    GC_CUDA_TRY(cudaStreamCreateWithFlags(&c.cs, cudaStreamNonBlocking));
+    for (auto& e : c.ev) GC_CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    GC_CUDA_TRY(cudaFuncSetAttribute(k_attn_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes));
+    c.ok = true;
+  }
+  *out = &c;
+  return GC_OK;
+}
+
+struct Ws { int32_t* k_lo; int32_t* k_hi; TileMeta* meta; void* Kg[2]; void* Vg[2]; };
+size_t carve(Carver& c, int64_t S_local, int64_t S, int32_t hs, Ws* w) {
+  const size_t n_tiles = (size_t)ceil_div(S_local > 0 ? S_local : 1, kBQ);
+  int32_t* lo = c.take<int32_t>(n_tiles * kBQ);
+  int32_t* hi = c.take<int32_t>(n_tiles * kBQ);
+  TileMeta* m = c.take<TileMeta>(n_tiles);
+  const size_t buf = (size_t)(S > 0 ? S : 1) * (size_t)hs * kD * 2;
+  void* k0 = c.take<uint8_t>(buf);
+  void* k1 = c.take<uint8_t>(buf);
+  void* v0 = c.take<uint8_t>(buf);
+  void* v1 = c.take<uint8_t>(buf);
+  if (w) { w->k_lo = lo; w->k_hi = hi; w->meta = m; w->Kg[0] = k0; w->Kg[1] = k1; w->Vg[0] = v0; w->Vg[1] = v1; }
+  return c.off;
+}
+
+}  // namespace attn
+}  // namespace gc
+
+using namespace gc;
+
+extern "C" {
+
+size_t gc_attention_workspace_bytes(int64_t S_local, int64_t S_total, int32_t heads_per_step) {
+  if (S_local < 0 || S_total < 0 || heads_per_step < 1) return 0;
+  Carver c(nullptr);
+  return attn::carve(c, S_local, S_total, heads_per_step, nullptr) + 256;
+}
+
+int gc_attention_allgather_kv(const void* Q, const void* const* K_shards_host,
+                              const void* const* V_shards_host, const int64_t* shard_rows_host,
+                              int32_t world, int32_t rank, int32_t Hq, int32_t Hkv, int32_t head_dim,
+                              const int32_t* cu_seqlens, int32_t n_docs, int causal, int32_t window,
+                              float scale, int32_t heads_per_step, void* O, float* lse,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (head_dim != attn::kD) return GC_ERR_SHAPE;
+  if (world < 1 || world > 64 || rank < 0 || rank >= world) return GC_ERR_ARG;
+  if (Hq < 1 || Hkv < 1 || Hq % Hkv != 0 || heads_per_step < 1 || window < 0) return GC_ERR_ARG;
+  if (!(scale > 0.f)) return GC_ERR_ARG;
+  if (!K_shards_host || !V_shards_host || !shard_rows_host) return GC_ERR_NULL;
+  int64_t S = 0, q_off = 0;
+  for (int r = 0; r < world; ++r) {
+    if (shard_rows_host[r] < 0) return GC_ERR_SHAPE;
+    if (r < rank) q_off += shard_rows_host[r];
+    S += shard_rows_host[r];
+  }
+  const int64_t S_local = shard_rows_host[rank];
+  if (S >= (1ll << 31) - 256) return GC_ERR_SHAPE;
+  if (S_local == 0) return GC_OK;
+  if (!Q || !O) return GC_ERR_NULL;
+  if (cu_seqlens != nullptr && n_docs < 1) return GC_ERR_ARG;
+  for (int r = 0; r < world; ++r) {
+    if (shard_rows_host[r] > 0 && (!K_shards_host[r] || !V_shards_host[r])) return GC_ERR_NULL;
+    if ((reinterpret_cast<uintptr_t>(K_shards_host[r]) & 15) || (reinterpret_cast<uintptr_t>(V_shards_host[r]) & 15))
+      return GC_ERR_ALIGN;
+  }
+  if ((reinterpret_cast<uintptr_t>(Q) & 15) || (reinterpret_cast<uintptr_t>(O) & 15)) return GC_ERR_ALIGN;
+  const int32_t hs = heads_per_step < Hkv ? heads_per_step : Hkv;
+  if (!workspace || workspace_bytes < gc_attention_workspace_bytes(S_local, S, hs)) return GC_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
+  {
+    int dev = 0, major = 0;
+    GC_CUDA_TRY(cudaGetDevice(&dev));
+    GC_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return GC_ERR_ARCH;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  attn::SideCtx* cx = nullptr;
+  GC_TRY(attn::get_side(&cx));
+  Carver c(workspace);
+  attn::Ws w;
+  attn::carve(c, S_local, S, hs, &w);
+  const int32_t n_q_tiles = (int32_t)ceil_div(S_local, attn::kBQ);
+  const int grp = Hq / Hkv;
+
+  attn::k_attn_rows<<<(unsigned)n_q_tiles, attn::kBQ, 0, st>>>(S_local, q_off, S, cu_seqlens, n_docs,
+                                                                causal ? 1 : 0, window, w.k_lo, w.k_hi,
+                                                                w.meta);
+  GC_CUDA_TRY(cudaGetLastError());
+
+  CUtensorMap tmQ;
+  GC_TRY(tc::make_tmap_bf16(&tmQ, Q, (int64_t)Hq * attn::kD, S_local, (int64_t)Hq * attn::kD, 64, attn::kBQ));
+  // fork: the gathers may start once earlier work on `st` (a previous call reading the buffers) is done
+  GC_CUDA_TRY(cudaEventRecord(cx->ev[0], st));
+  GC_CUDA_TRY(cudaStreamWaitEvent(cx->cs, cx->ev[0], 0));
+  const size_t src_pitch = (size_t)Hkv * attn::kD * 2;
+  const int n_steps = (int)ceil_div(Hkv, hs);
+  for (int s = 0; s < n_steps; ++s) {
+    const int b = s & 1;
+    const int h0 = s * hs;
+    const int nh = (Hkv - h0) < hs ? (Hkv - h0) : hs;
+    const size_t dst_pitch = (size_t)nh * attn::kD * 2;
+    // ---- all-gather of this head subset (copy engines, side stream) ----
+    if (s >= 2) GC_CUDA_TRY(cudaStreamWaitEvent(cx->cs, cx->ev[3 + b], 0));   // buffer b consumed
+    int64_t pos = 0;
+    for (int r = 0; r < world; ++r) {
+      const int64_t rows = shard_rows_host[r];
+      if (rows == 0) continue;
+      GC_CUDA_TRY(cudaMemcpy2DAsync(static_cast<char*>(w.Kg[b]) + (size_t)pos * dst_pitch, dst_pitch,
+                                    static_cast<const char*>(K_shards_host[r]) + (size_t)h0 * attn::kD * 2,
+                                    src_pitch, dst_pitch, (size_t)rows, cudaMemcpyDeviceToDevice, cx->cs));
+      GC_CUDA_TRY(cudaMemcpy2DAsync(static_cast<char*>(w.Vg[b]) + (size_t)pos * dst_pitch, dst_pitch,
+                                    static_cast<const char*>(V_shards_host[r]) + (size_t)h0 * attn::kD * 2,
+                                    src_pitch, dst_pitch, (size_t)rows, cudaMemcpyDeviceToDevice, cx->cs));
+      pos += rows;
+    }
+    GC_CUDA_TRY(cudaEventRecord(cx->ev[1 + b], cx->cs));
+    // ---- attention of this subset's query heads (main stream) ----
+    GC_CUDA_TRY(cudaStreamWaitEvent(st, cx->ev[1 + b], 0));
+    CUtensorMap tmK, tmV;
+    GC_TRY(tc::make_tmap_bf16(&tmK, w.Kg[b], (int64_t)nh * attn::kD, S, (int64_t)nh * attn::kD, 64, attn::kBK));
+    GC_TRY(tc::make_tmap_bf16(&tmV, w.Vg[b], (int64_t)nh * attn::kD, S, (int64_t)nh * attn::kD, 64, 64));
+    attn::Params p;
+    p.S_local = S_local; p.q_off = q_off; p.S = S; p.n_q_tiles = n_q_tiles;
+    p.h_begin = h0 * grp; p.n_q_heads = nh * grp; p.grp = grp;
+    p.scale2 = scale * kLog2e;
+    p.k_lo = w.k_lo; p.k_hi = w.k_hi; p.meta = w.meta;
+    p.O = static_cast<__nv_bfloat16*>(O); p.ldO = (int64_t)Hq * attn::kD; p.lse = lse;
+    attn::k_attn_fwd<<<(unsigned)(n_q_tiles * p.n_q_heads), attn::kThreads, attn::kSmemBytes, st>>>(tmQ, tmK, tmV, p);
+    GC_CUDA_TRY(cudaGetLastError());
+    GC_CUDA_TRY(cudaEventRecord(cx->ev[3 + b], st));
+  }
+  return GC_OK;
+}
+
+}  // extern "C"

@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2|cfg3|cfg4|cfg0]
                     [--impl ours|reference] [--no-extras] [--arm fused|nccl] [--dry-run]
+                    [--only hbm|attention]
 
 A step is one pass of the hot path over one synthetic micro-batch of the named workload.
 BASELINE.json:metric ("scored tokens/sec (fwd and fwd+bwd) on 1 B200") names no configuration, so
@@ -628,6 +629,41 @@ def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
     return out
 
 
+def attention_workload(B, device, peaks):
+    """NEXT-4: all-gather-KV attention forward, as the last of 8 context-parallel
+    ranks sees it (its 16384-query chunk against all 131072 gathered keys, causal, GQA 8/2 heads,
+    head_dim 128, one key/value head gathered at a time on the side stream), and a single-rank
+    32768-token causal case.  Algorithmic flops = 4 * allowed (q, k) pairs * head_dim * Hq."""
+    out = {}
+    for name, S, Hq, Hkv, world, hps in (("cp8_last_rank_131072", 131072, 8, 2, 8, 1),
+                                         ("single_rank_32768", 32768, 32, 8, 1, 2)):
+        g = torch.Generator(device=device).manual_seed(0)
+        K = torch.randn(S, Hkv, 128, device=device, generator=g).to(torch.bfloat16)
+        V = torch.randn(S, Hkv, 128, device=device, generator=g).to(torch.bfloat16)
+        cuts = [S * r // world for r in range(world + 1)]
+        rows = [b - a for a, b in zip(cuts[:-1], cuts[1:])]
+        Ks = [K[a:b].contiguous() for a, b in zip(cuts[:-1], cuts[1:])]
+        Vs = [V[a:b].contiguous() for a, b in zip(cuts[:-1], cuts[1:])]
+        rank = world - 1
+        Q = torch.randn(rows[rank], Hq, 128, device=device, generator=g).to(torch.bfloat16)
+        kp, vp = [k.data_ptr() for k in Ks], [v.data_ptr() for v in Vs]
+        ms = _event_time(lambda: B.gc_attention_allgather_kv(Q, kp, vp, rows, rank, Hkv, None, True, 0,
+                                                             None, hps, want_lse=True), 5, 3)
+        q0, n = cuts[rank], rows[rank]
+        pairs = n * q0 + n * (n + 1) // 2                   # causal: keys 0 .. q
+        flops = 4.0 * pairs * 128 * Hq
+        tf = flops / (ms * 1e-3) / 1e12
+        out[name] = {"tokens_total": S, "queries_local": n, "q_heads": Hq, "kv_heads": Hkv,
+                     "head_dim": 128, "world": world, "kv_heads_per_gather_step": hps, "mask": "causal",
+                     "ms": ms, "roofline": {"bound": "tensor", "kernel": "attn::k_attn_fwd",
+                                            "achieved": tf, "peak": peaks["burst"], "unit": "TFLOP/s",
+                                            "frac": tf / peaks["burst"], "flops_per_call": flops,
+                                            "gathered_bytes_per_call": 2 * S * Hkv * 128 * 2}}
+        del K, V, Ks, Vs, Q
+        torch.cuda.empty_cache()
+    return out
+
+
 # --------------------------------------------------------------------------------------------
 # N > 1 training arm: the dW exchange
 # --------------------------------------------------------------------------------------------
@@ -725,6 +761,8 @@ def main():
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
                     help="control-plane backend (gloo: ranks may share a GPU; the NCCL arm is skipped)")
     ap.add_argument("--dry-run", action="store_true")
+    ap.add_argument("--only", default=None, choices=["hbm", "attention"],
+                    help="run only that part of the extras and print it (profiling aid)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = I.CONFIGS[WORKLOADS[args.workload]]
@@ -754,6 +792,10 @@ def main():
     from paper_2507_22789_b200 import binding as B      # raises if libgcore.so is missing
     from paper_2507_22789_b200 import dp
     peaks = load_peaks()
+    if args.only:
+        part = hbm_kernels(B, device, peaks) if args.only == "hbm" else attention_workload(B, device, peaks)
+        print(json.dumps({args.only: part}))
+        return
 
     # every rank: its own tokens (seed = rank), the same W (seed 0)
     b = DeviceBatch(w, seed=rank, device=device, w_seed=0 if dist_on else None)
@@ -830,6 +872,7 @@ def main():
                     wl[name] = measure_workload(B, I.CONFIGS[WORKLOADS[name]], device, k, wu, peaks,
                                                 with_e2e=(name == "cfg2"))
                     out["rooflines"] = out["rooflines"] + wl[name]["rooflines"]
+                wl["attention_allgather_kv"] = attention_workload(B, device, peaks)
                 out["workloads"] = wl
                 out["fwd_bwd"] = {k: wl["cfg2"][k] for k in ("workload", "value", "unit", "ms_per_step",
                                                              "step_tflops", "gpu_launches_per_step")}

@@ -10,10 +10,13 @@
 //     attention kernel works on the previous subset out of the other buffer.
 //   * k_attn_fwd: a tcgen05 flash-attention forward for one (128-query tile, query head):
 //       S_j = Q K_j^T (UMMA 128x128x16, fp32 in TMEM, two buffers), online softmax by a
-//       4-warp group (thread = query row; exp2 domain), P_j -> bf16 -> 128B-swizzled smem,
-//       PV_j = P_j V_j (V is the MN-major B operand; fp32 in TMEM, two buffers), and the output
-//       row lives in REGISTERS: O = O * 2^(m_O - m_j) + PV_j.  The MMA warp issues S_{j+1} before
-//       PV_j, so the tensor core computes the next scores while the softmax group works.
+//       4-warp group (thread = query row; exp2 domain; the whole 128-column score row is read
+//       from TMEM in one round trip), P_j -> bf16 -> 128B-swizzled smem, O += P_j V_j accumulated
+//       IN TMEM by the second contraction (V is the MN-major B operand).  The reference maximum of
+//       a row is raised lazily -- only when the block's maximum exceeds it by more than 2^8 -- and
+//       only then is the row of O rescaled in TMEM (tcgen05.ld / st); P stays <= 2^8, exact in the
+//       end because l and O share the reference.  The MMA warp issues S_{j+1} before P_j V_j, so
+//       the tensor core computes the next scores while the softmax group works.
 //     Masks: per query row an allowed key interval [k_lo, k_hi) -- packed
 //     documents, causal, sliding window -- computed once by k_attn_rows; blocks outside the
 //     tile's interval are skipped, blocks inside every row's interval take no per-element test.
@@ -149,8 +152,7 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   auto s_empty = [&](int i) { return bar + 8u * (11 + i); };
   auto p_full = [&](int i) { return bar + 8u * (13 + i); };
   auto p_empty = [&](int i) { return bar + 8u * (15 + i); };
-  auto pv_full = [&](int i) { return bar + 8u * (17 + i); };
-  auto pv_empty = [&](int i) { return bar + 8u * (19 + i); };
+  const uint32_t o_done = bar + 8u * 17;    // one phase per key block: P_j V_j has been accumulated
   const uint32_t tmem_slot = bar + 8u * 21;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -177,9 +179,8 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       ptx::mbar_init(s_empty(i), 4);       // one arrive per softmax warp
       ptx::mbar_init(p_full(i), 4);
       ptx::mbar_init(p_empty(i), 1);
-      ptx::mbar_init(pv_full(i), 1);
-      ptx::mbar_init(pv_empty(i), 4);
     }
+    ptx::mbar_init(o_done, 1);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -191,7 +192,7 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-  // TMEM columns: S0 [0,128) S1 [128,256) PV0 [256,384) PV1 [384,512)
+  // TMEM columns: S0 [0,128) S1 [128,256) O [256,384)
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -257,14 +258,13 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
         ptx::umma_commit<1>(k_empty(st));      // the K stage is free once these MMAs have read it
         ptx::umma_commit<1>(s_full(st));
       };
-      auto issue_pv = [&](int j) {
+      auto issue_pv = [&](int j) {             // O (+)= P_j V_j
         const int st = j & 1;
         const uint32_t ph = ((uint32_t)j >> 1) & 1u;
         ptx::mbar_wait(v_full(st), ph);
-        ptx::mbar_wait(p_full(st), ph);
-        ptx::mbar_wait(pv_empty(st), ph ^ 1u);
+        ptx::mbar_wait(p_full(st), ph);          // P_j written, and O rescaled if it had to be
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + 256u + (uint32_t)st * 128u;
+        const uint32_t d_tmem = tmem_base + 256u;
 #pragma unroll
         for (int kb = 0; kb < 2; ++kb) {
           const uint64_t adesc = ptx::make_smem_desc(sP + st * kTileBytes + kb * 16384, false);
@@ -272,11 +272,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
 #pragma unroll
           for (int k = 0; k < 4; ++k)
             ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 128),
-                              idesc_pv, (uint32_t)(kb | k));
+                              idesc_pv, (uint32_t)(j | kb | k));
         }
         ptx::umma_commit<1>(v_empty(st));
         ptx::umma_commit<1>(p_empty(st));
-        ptx::umma_commit<1>(pv_full(st));
+        ptx::umma_commit<1>(o_done);
       };
       ptx::mbar_wait(q_full, 0);
       issue_s(0);
@@ -293,34 +293,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
     const bool valid = i < p.S_local;
     const int32_t lo = valid ? p.k_lo[i] : 0, hi = valid ? p.k_hi[i] : 0;
     const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
-    float O[kD];
-#pragma unroll
-    for (int c = 0; c < kD; ++c) O[c] = 0.f;
-    float m_run = -1e30f;     // running maximum (log2 domain)
-    float m_O = -1e30f;       // the maximum O is relative to
-    float m_prev = -1e30f;    // the maximum PV_{j-1} is relative to
+    float m_ref = -1e30f;     // the maximum P, l and O are relative to (log2 domain), raised lazily
     float l_run = 0.f;
     const uint32_t p_row = (uint32_t)row * 128u;
     const uint32_t sw = (uint32_t)(row & 7);
-
-    auto add_pv = [&](int j) {                 // O = O * 2^(m_O - m_j) + PV_j
-      const int st = j & 1;
-      ptx::mbar_wait(pv_full(st), ((uint32_t)j >> 1) & 1u);
-      ptx::tc_fence_after();
-      const float a = ptx::ex2(m_O - m_prev);
-      m_O = m_prev;
-#pragma unroll
-      for (int ch = 0; ch < 4; ++ch) {
-        uint32_t r[32];
-        ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(st * 128 + ch * 32), r);
-        ptx::tmem_wait_ld();
-#pragma unroll
-        for (int c = 0; c < 32; ++c) O[ch * 32 + c] = fmaf(O[ch * 32 + c], a, __uint_as_float(r[c]));
-      }
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(pv_empty(st));
-    };
+    constexpr float kLazy = 8.0f;              // P <= 2^8 between raises of the reference
 
     for (int j = 0; j < nb; ++j) {
       const int st = j & 1;
@@ -329,54 +306,48 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       const bool need_mask = k0 < tm.lo_max || k0 + kBK > tm.hi_min;
       ptx::mbar_wait(s_full(st), ph);
       ptx::tc_fence_after();
-      // pass 1: row maximum over the allowed keys of this block
-      float mx = -INFINITY;
+      // the whole score row in one TMEM round trip, then the S buffer goes back to the MMA warp
+      uint32_t r[4][32];
 #pragma unroll
-      for (int ch = 0; ch < 4; ++ch) {
-        uint32_t r[32];
-        ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r);
-        ptx::tmem_wait_ld();
-        if (need_mask) {
+      for (int ch = 0; ch < 4; ++ch) ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r[ch]);
+      ptx::tmem_wait_ld();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(s_empty(st));
+      if (need_mask) {
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch)
 #pragma unroll
           for (int c = 0; c < 32; ++c) {
             const int32_t k = k0 + ch * 32 + c;
-            mx = (k >= lo && k < hi) ? fmaxf(mx, __uint_as_float(r[c])) : mx;
+            r[ch][c] = (k >= lo && k < hi) ? r[ch][c] : 0xff800000u;      // -inf
           }
-        } else {
-#pragma unroll
-          for (int c = 0; c < 32; ++c) mx = fmaxf(mx, __uint_as_float(r[c]));
-        }
       }
-      const float m_new = fmaxf(m_run, mx * p.scale2);
-      l_run *= ptx::ex2(m_run - m_new);
-      m_run = m_new;
-      // pass 2: p = 2^(s * scale2 - m), row sum, P -> bf16 -> swizzled smem (A operand of P V)
+      float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch)
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) {
+          mx0 = fmaxf(mx0, __uint_as_float(r[ch][c]));
+          mx1 = fmaxf(mx1, __uint_as_float(r[ch][c + 1]));
+        }
+      const float mx = fmaxf(mx0, mx1) * p.scale2;
+      // lazy reference: raise it only when this block's maximum exceeds it by more than 2^kLazy
+      const bool raise = mx > m_ref + kLazy;
+      const float m_new = raise ? mx : m_ref;
+      const float factor = raise ? ptx::ex2(m_ref - m_new) : 1.0f;
+      m_ref = m_new;
+      l_run *= factor;
+      // p = 2^(s * scale2 - m_ref), row sum, P -> bf16 -> swizzled smem (A operand of P V)
       ptx::mbar_wait(p_empty(st), ph ^ 1u);
       float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
       for (int ch = 0; ch < 4; ++ch) {
-        uint32_t r[32];
-        ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r);
-        ptx::tmem_wait_ld();
-        if (ch == 3) {
-          // every read of this S buffer is done: hand it back to the MMA warp
-          ptx::tc_fence_before();
-          __syncwarp();
-          if (lane == 0) ptx::mbar_arrive(s_empty(st));
-        }
         float e[32];
 #pragma unroll
-        for (int c = 0; c < 32; ++c) {
-          float v = ptx::ex2(fmaf(__uint_as_float(r[c]), p.scale2, -m_new));
-          if (need_mask) {
-            const int32_t k = k0 + ch * 32 + c;
-            v = (k >= lo && k < hi) ? v : 0.f;
-          }
-          e[c] = v;
-        }
+        for (int c = 0; c < 32; ++c) e[c] = ptx::ex2(fmaf(__uint_as_float(r[ch][c]), p.scale2, -m_new));
 #pragma unroll
         for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
-        // 32 columns = 4 16-byte chunks of this row's 128-byte line in k-block ch / 2
         const uint32_t pb = sP + st * kTileBytes + (uint32_t)(ch >> 1) * 16384u + p_row;
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
@@ -388,14 +359,46 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
         }
       }
       l_run += sum0 + sum1;
+      // O holds blocks 0 .. j-1 relative to the old reference: wait for P_{j-1} V_{j-1} (long done:
+      // it ran under the exponentials above), rescale the rows whose reference was raised
+      if (j > 0) {
+        ptx::mbar_wait(o_done, (uint32_t)(j - 1) & 1u);
+        if (__any_sync(0xffffffffu, raise)) {
+          ptx::tc_fence_after();
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t o[32];
+            ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * factor);
+            ptx::tmem_st_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+          }
+          ptx::tmem_wait_st();
+          ptx::tc_fence_before();
+        }
+      }
       ptx::fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(p_full(st));
-      // the previous block's P V has been running under this softmax: fold it into O now
-      if (j > 0) add_pv(j - 1);
-      m_prev = m_new;
     }
-    if (nb > 0) add_pv(nb - 1);
+    float O[kD];
+    if (nb > 0) {
+      ptx::mbar_wait(o_done, (uint32_t)(nb - 1) & 1u);
+      ptx::tc_fence_after();
+#pragma unroll
+      for (int ch = 0; ch < 4; ++ch) {
+        uint32_t o[32];
+        ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+        ptx::tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 32; ++c) O[ch * 32 + c] = __uint_as_float(o[c]);
+      }
+    } else {
+#pragma unroll
+      for (int c = 0; c < kD; ++c) O[c] = 0.f;
+    }
+    const float m_run = m_ref;
     // out = O / l; lse = ln2 * (m + log2 l)
     if (valid) {
       const float inv = l_run > 0.f ? 1.0f / l_run : 0.f;

@@ -631,11 +631,11 @@ def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
 
 def attention_workload(B, device, peaks):
     """NEXT-4: all-gather-KV attention forward, as the last of 8 context-parallel
-    ranks sees it (its 16384-query chunk against all 131072 gathered keys, causal, GQA 8/2 heads,
-    head_dim 128, one key/value head gathered at a time on the side stream), and a single-rank
+    ranks sees it (its 16384-query chunk against all 131072 gathered keys, causal, GQA 16/4 heads,
+    head_dim 128, two of the four key/value heads gathered at a time on the side stream), and a single-rank
     32768-token causal case.  Algorithmic flops = 4 * allowed (q, k) pairs * head_dim * Hq."""
     out = {}
-    for name, S, Hq, Hkv, world, hps in (("cp8_last_rank_131072", 131072, 8, 2, 8, 1),
+    for name, S, Hq, Hkv, world, hps in (("cp8_last_rank_131072", 131072, 16, 4, 8, 2),
                                          ("single_rank_32768", 32768, 32, 8, 1, 2)):
         g = torch.Generator(device=device).manual_seed(0)
         K = torch.randn(S, Hkv, 128, device=device, generator=g).to(torch.bfloat16)

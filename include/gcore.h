@@ -381,6 +381,7 @@ int gc_kernel_timing_end(float* ms_by_kind_host, int32_t* launches_by_kind_host)
  *                 last, shorter run are allowed);
  *   n_band  >  0: items = (band of n_band N tiles, M tile, N tile in band), the dW order (a last,
  *                 narrower band is allowed);  c_major and n_band exclude each other;
+ *   c_major == 2: (N tile, M tile) -- the dH order when the dS chunk has fewer rows than D;
  *   both 0      : (M tile, N tile). */
 int gc_debug_gemm_bf16(const void* A, int64_t lda, int a_mn_major,
                        const void* B, int64_t ldb, int b_mn_major,

@@ -68,6 +68,10 @@ struct Sched {
                           // band): the band's B panels stay in L2 while the A panels stream past
   int skip_empty_k;       // 1: a launch whose K extent resolves to 0 does nothing (accumulating
                           // epilogues: adding zero)
+  int n_major;            // plain order only: 1: items ordered (N tile, M tile) -- a wave of pairs
+                          // then covers every M tile and few N tiles, so the A operand is what gets
+                          // re-read per wave; 0: (M tile, N tile), B is re-read per wave.  Pick the
+                          // order that re-reads the SMALLER operand (K-lockstep kernels: dH).
 };
 
 __device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t& K) {
@@ -115,6 +119,11 @@ __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt,
     const int64_t rem = it - b * per_band;
     x.m_tile = rem / w;
     x.n0 = n_start + (rem - x.m_tile * w);
+    x.n1 = x.n0 + 1;
+    x.c = 0;
+  } else if (s.n_major) {
+    x.n0 = it / Mt;
+    x.m_tile = it - x.n0 * Mt;
     x.n1 = x.n0 + 1;
     x.c = 0;
   } else {

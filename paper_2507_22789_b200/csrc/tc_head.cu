@@ -507,7 +507,7 @@ static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   Sched s;
   s.M = M; s.N = N; s.K = K;
   s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
-  s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0; s.n_band = 0; s.skip_empty_k = 0;
+  s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0; s.n_band = 0; s.skip_empty_k = 0; s.n_major = 0;
   s.counter = nullptr; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
   return s;
 }
@@ -610,6 +610,12 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
   Sched s = make_sched(n_rows_dev ? rows_cap : n_static, D, V);
   (void)counter;   // K-lockstep kernel: all pairs stream V together, static schedule
+  // Every wave of 74 tiles streams, over the whole of K = V, the dS rows of the M tiles it covers and
+  // the W columns of the N tiles it covers; the operand whose tiles a wave covers COMPLETELY is
+  // re-read by every wave.  Order the tiles so that this is the smaller one: dS chunk (rows x V)
+  // against W (V x D), i.e. N-major iff rows < D (cfg4: 4096 rows < D = 8192: W, 4.2 GB, is then
+  // read once per launch instead of once per wave).
+  s.n_major = rows_cap < D ? 1 : 0;
   if (n_rows_dev) { s.n_dyn = n_rows_dev; s.dyn_dim = 1; s.dyn_row0 = row0; s.dyn_cap = rows_cap; }
   EpiStoreBf16::Params ep;
   ep.out = static_cast<__nv_bfloat16*>(dH);
@@ -695,8 +701,8 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
                   int cta_group, int dynamic_schedule, int dual_n, int cluster4, int c_major,
                   int m_band, int chunk_ntiles, int n_band, cudaStream_t st) {
   if (cta_group != 1 && cta_group != 2) return GC_ERR_ARG;
-  if (c_major < 0 || c_major > 1 || m_band < 0 || chunk_ntiles < 0 || n_band < 0) return GC_ERR_ARG;
-  if (c_major && n_band) return GC_ERR_ARG;          // the two item orders exclude each other
+  if (c_major < 0 || c_major > 2 || m_band < 0 || chunk_ntiles < 0 || n_band < 0) return GC_ERR_ARG;
+  if (c_major && n_band) return GC_ERR_ARG;          // the item orders exclude each other
   if ((dual_n || cluster4) && cta_group != 2) return GC_ERR_ARG;
   const int ppc = cluster4 ? 2 : 1;
   if (N % 4 != 0) return GC_ERR_SHAPE;
@@ -706,7 +712,8 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
   Sched s = make_sched(M, N, K);
   // the item orders of the path's kernels (forward / recompute: c_major + m_band + chunk_ntiles;
   // dW: n_band), reachable here at any size
-  s.c_major = c_major;
+  s.c_major = c_major == 1 ? 1 : 0;
+  s.n_major = c_major == 2 ? 1 : 0;                  // c_major = 2: plain order, N-major (dH)
   s.m_band = m_band;
   s.chunk_ntiles = chunk_ntiles > 0 ? chunk_ntiles : 1;
   s.n_band = n_band;

@@ -119,6 +119,8 @@ SCHEDS = {
     "m_band_full_plus_rest_k3": dict(c_major=True, m_band=5, chunk_ntiles=3),   # 22 = 4x5 + 2; runs 3,3,3,1
     "m_band_one_band_k4": dict(c_major=True, m_band=0, chunk_ntiles=4),
     "m_band_7_k1": dict(c_major=True, m_band=7, chunk_ntiles=1),
+    "n_major": dict(c_major=2),                                 # (N tile, M tile): dH with rows < D
+    "n_major_dual": dict(c_major=2, dual_n=True),               # ... on 256 x 512 tiles, half-tile tail
 }
 
 

@@ -30,16 +30,31 @@ namespace attn {
 
 constexpr int kD = 128;            // head dimension
 constexpr int kBQ = 128;           // query rows per CTA
-constexpr int kBK = 128;           // keys per block
+#ifndef GC_ATTN_BK
+#define GC_ATTN_BK 64
+#endif
+constexpr int kBK = GC_ATTN_BK;    // keys per block.  64: 112 KB of shared memory and 256 TMEM columns
+                                   // per CTA, so TWO CTAs share an SM and one's softmax (MUFU-bound)
+                                   // runs under the other's TMEM round trips, barriers and P stores;
+                                   // 128: one CTA per SM (224 KB, 384 columns)
+static_assert(kBK == 64 || kBK == 128, "key block");
+constexpr int kKB = kBK / 64;      // 64-key k-blocks per block (second contraction)
+constexpr int kCH = kBK / 32;      // 32-column TMEM chunks of a score row
+constexpr int kPBufs = kBK == 64 ? 1 : 2;
+constexpr int kCtasPerSM = kBK == 64 ? 2 : 1;
+constexpr int kTmemCols = kBK == 64 ? 256 : 512;
 constexpr int kThreads = 256;
-constexpr int kTileBytes = kBQ * kD * 2;     // 32 KB: a 128 x 128 bf16 tile (two 64-wide k-blocks)
+constexpr int kQBytes = kBQ * kD * 2;        // 32 KB: 128 x 128 bf16 (two 64-wide k-blocks of 16 KB)
+constexpr int kKSub = kBK * 128;             // one 64-wide k-block of a K tile: kBK rows x 128 B
+constexpr int kKVBytes = kBK * kD * 2;       // a K or V stage
+constexpr int kPBytes = kBQ * kBK * 2;       // a P buffer: kKB k-blocks of 128 rows x 128 B
 constexpr int kSmemQ = 0;
-constexpr int kSmemK = kSmemQ + kTileBytes;
-constexpr int kSmemV = kSmemK + 2 * kTileBytes;
-constexpr int kSmemP = kSmemV + 2 * kTileBytes;
-constexpr int kSmemBar = kSmemP + 2 * kTileBytes;          // 224 KB of tiles, then the barriers
-constexpr int kSmemBytes = kSmemBar + 256 + 1024;          // + alignment slack
-static_assert(kSmemBytes <= 227 * 1024, "attention shared memory budget");
+constexpr int kSmemK = kSmemQ + kQBytes;
+constexpr int kSmemV = kSmemK + 2 * kKVBytes;
+constexpr int kSmemP = kSmemV + 2 * kKVBytes;
+constexpr int kSmemBar = kSmemP + kPBufs * kPBytes;        // tiles, then the barriers
+constexpr int kSmemBytes = kSmemBar + 256;                 // (the dynamic smem base is 1024-aligned)
+static_assert(kSmemBytes <= (kCtasPerSM == 2 ? 113 : 227) * 1024, "attention shared memory budget");
 
 struct TileMeta { int32_t kb_begin, kb_end, lo_max, hi_min; };
 
@@ -135,11 +150,12 @@ __device__ __forceinline__ void st_shared_v4_u32(uint32_t addr, uint32_t a, uint
 // One CTA = one (query tile, query head).  Warps: 0 TMA producer, 1 MMA issuer, 2 TMEM allocator,
 // 4..7 softmax / output group (thread = query row).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, kCtasPerSM)
 k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
            const __grid_constant__ CUtensorMap tmV, const Params p) {
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t base = ptx::smem_u32(smem_raw);
+  if (base & 1023u) __trap();              // the swizzled tiles need a 1024-byte aligned base
   const uint32_t sQ = base + kSmemQ, sK = base + kSmemK, sV = base + kSmemV, sP = base + kSmemP;
   const uint32_t bar = base + kSmemBar;
   // barriers (8 bytes each)
@@ -184,7 +200,7 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
-    ptx::tmem_alloc<1>(tmem_slot, 512);
+    ptx::tmem_alloc<1>(tmem_slot, kTmemCols);
     ptx::tmem_relinquish<1>();
   }
   ptx::tc_fence_before();
@@ -192,7 +208,8 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-  // TMEM columns: S0 [0,128) S1 [128,256) O [256,384)
+  // TMEM columns: S0 [0,kBK) S1 [kBK,2 kBK) O [2 kBK, 2 kBK + 128)
+  constexpr uint32_t kOCol = 2u * kBK;
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -202,27 +219,27 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       const int32_t q_row = q_tile * kBQ;
       const int32_t q_col = hq * kD;
       const int32_t kv_col = g_local * kD;
-      ptx::mbar_arrive_expect_tx(q_full, kTileBytes);
+      ptx::mbar_arrive_expect_tx(q_full, kQBytes);
       ptx::tma_load_2d(sQ, &tmQ, q_col, q_row, q_full, pol_q);
       ptx::tma_load_2d(sQ + 16384, &tmQ, q_col + 64, q_row, q_full, pol_q);
       auto load_k = [&](int j) {
         const int st = j & 1;
         ptx::mbar_wait(k_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
-        ptx::mbar_arrive_expect_tx(k_full(st), kTileBytes);
+        ptx::mbar_arrive_expect_tx(k_full(st), kKVBytes);
         const int32_t row = (tm.kb_begin + j) * kBK;
-        const uint32_t dst = sK + st * kTileBytes;
+        const uint32_t dst = sK + st * kKVBytes;
         ptx::tma_load_2d(dst, &tmK, kv_col, row, k_full(st), pol_kv);
-        ptx::tma_load_2d(dst + 16384, &tmK, kv_col + 64, row, k_full(st), pol_kv);
+        ptx::tma_load_2d(dst + kKSub, &tmK, kv_col + 64, row, k_full(st), pol_kv);
       };
       auto load_v = [&](int j) {
         const int st = j & 1;
         ptx::mbar_wait(v_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
-        ptx::mbar_arrive_expect_tx(v_full(st), kTileBytes);
+        ptx::mbar_arrive_expect_tx(v_full(st), kKVBytes);
         const int32_t row = (tm.kb_begin + j) * kBK;
-        const uint32_t dst = sV + st * kTileBytes;
+        const uint32_t dst = sV + st * kKVBytes;
         // MN-major B operand: per 64-key k-block two 64(d) x 64(keys) boxes, 8 KB apart
 #pragma unroll
-        for (int kb = 0; kb < 2; ++kb)
+        for (int kb = 0; kb < kKB; ++kb)
 #pragma unroll
           for (int nbx = 0; nbx < 2; ++nbx)
             ptx::tma_load_2d(dst + kb * 16384 + nbx * 8192, &tmV, kv_col + 64 * nbx, row + 64 * kb,
@@ -245,11 +262,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
         ptx::mbar_wait(k_full(st), ph);
         ptx::mbar_wait(s_empty(st), ph ^ 1u);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)st * 128u;
+        const uint32_t d_tmem = tmem_base + (uint32_t)(st * kBK);
 #pragma unroll
-        for (int kb = 0; kb < 2; ++kb) {
+        for (int kb = 0; kb < 2; ++kb) {            // the two 64-wide halves of head_dim
           const uint64_t adesc = ptx::make_smem_desc(sQ + kb * 16384, false);
-          const uint64_t bdesc = ptx::make_smem_desc(sK + st * kTileBytes + kb * 16384, false);
+          const uint64_t bdesc = ptx::make_smem_desc(sK + st * kKVBytes + kb * kKSub, false);
 #pragma unroll
           for (int k = 0; k < 4; ++k)
             ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 2), idesc_qk,
@@ -261,21 +278,23 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       auto issue_pv = [&](int j) {             // O (+)= P_j V_j
         const int st = j & 1;
         const uint32_t ph = ((uint32_t)j >> 1) & 1u;
+        const int pst = j % kPBufs;
+        const uint32_t pph = ((uint32_t)(j / kPBufs)) & 1u;
         ptx::mbar_wait(v_full(st), ph);
-        ptx::mbar_wait(p_full(st), ph);          // P_j written, and O rescaled if it had to be
+        ptx::mbar_wait(p_full(pst), pph);        // P_j written, and O rescaled if it had to be
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + 256u;
+        const uint32_t d_tmem = tmem_base + kOCol;
 #pragma unroll
-        for (int kb = 0; kb < 2; ++kb) {
-          const uint64_t adesc = ptx::make_smem_desc(sP + st * kTileBytes + kb * 16384, false);
-          const uint64_t bdesc = ptx::make_smem_desc(sV + st * kTileBytes + kb * 16384, true);
+        for (int kb = 0; kb < kKB; ++kb) {
+          const uint64_t adesc = ptx::make_smem_desc(sP + pst * kPBytes + kb * 16384, false);
+          const uint64_t bdesc = ptx::make_smem_desc(sV + st * kKVBytes + kb * 16384, true);
 #pragma unroll
           for (int k = 0; k < 4; ++k)
             ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 128),
                               idesc_pv, (uint32_t)(j | kb | k));
         }
         ptx::umma_commit<1>(v_empty(st));
-        ptx::umma_commit<1>(p_empty(st));
+        ptx::umma_commit<1>(p_empty(pst));
         ptx::umma_commit<1>(o_done);
       };
       ptx::mbar_wait(q_full, 0);
@@ -307,16 +326,18 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       ptx::mbar_wait(s_full(st), ph);
       ptx::tc_fence_after();
       // the whole score row in one TMEM round trip, then the S buffer goes back to the MMA warp
-      uint32_t r[4][32];
+      const int pst = j % kPBufs;
+      const uint32_t pph = ((uint32_t)(j / kPBufs)) & 1u;
+      uint32_t r[kCH][32];
 #pragma unroll
-      for (int ch = 0; ch < 4; ++ch) ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * 128 + ch * 32), r[ch]);
+      for (int ch = 0; ch < kCH; ++ch) ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * kBK + ch * 32), r[ch]);
       ptx::tmem_wait_ld();
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(s_empty(st));
       if (need_mask) {
 #pragma unroll
-        for (int ch = 0; ch < 4; ++ch)
+        for (int ch = 0; ch < kCH; ++ch)
 #pragma unroll
           for (int c = 0; c < 32; ++c) {
             const int32_t k = k0 + ch * 32 + c;
@@ -325,7 +346,7 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       }
       float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-      for (int ch = 0; ch < 4; ++ch)
+      for (int ch = 0; ch < kCH; ++ch)
 #pragma unroll
         for (int c = 0; c < 32; c += 2) {
           mx0 = fmaxf(mx0, __uint_as_float(r[ch][c]));
@@ -339,16 +360,16 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       m_ref = m_new;
       l_run *= factor;
       // p = 2^(s * scale2 - m_ref), row sum, P -> bf16 -> swizzled smem (A operand of P V)
-      ptx::mbar_wait(p_empty(st), ph ^ 1u);
+      ptx::mbar_wait(p_empty(pst), pph ^ 1u);
       float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
-      for (int ch = 0; ch < 4; ++ch) {
+      for (int ch = 0; ch < kCH; ++ch) {
         float e[32];
 #pragma unroll
         for (int c = 0; c < 32; ++c) e[c] = ptx::ex2(fmaf(__uint_as_float(r[ch][c]), p.scale2, -m_new));
 #pragma unroll
         for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
-        const uint32_t pb = sP + st * kTileBytes + (uint32_t)(ch >> 1) * 16384u + p_row;
+        const uint32_t pb = sP + pst * kPBytes + (uint32_t)(ch >> 1) * 16384u + p_row;
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) {
           const uint32_t chunk = (uint32_t)((ch & 1) * 4 + cc);
@@ -368,11 +389,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
 #pragma unroll
           for (int ch = 0; ch < 4; ++ch) {
             uint32_t o[32];
-            ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+            ptx::tmem_ld_32x32(lane_base + kOCol + (uint32_t)(ch * 32), o);
             ptx::tmem_wait_ld();
 #pragma unroll
             for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * factor);
-            ptx::tmem_st_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+            ptx::tmem_st_32x32(lane_base + kOCol + (uint32_t)(ch * 32), o);
           }
           ptx::tmem_wait_st();
           ptx::tc_fence_before();
@@ -380,42 +401,42 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       }
       ptx::fence_proxy_async_smem();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full(st));
+      if (lane == 0) ptx::mbar_arrive(p_full(pst));
     }
-    float O[kD];
+    // out = O / l; lse = ln2 * (m + log2 l): read O from TMEM 32 columns at a time and store
     if (nb > 0) {
       ptx::mbar_wait(o_done, (uint32_t)(nb - 1) & 1u);
       ptx::tc_fence_after();
+    }
+    const float inv = (nb > 0 && l_run > 0.f) ? 1.0f / l_run : 0.f;
 #pragma unroll
-      for (int ch = 0; ch < 4; ++ch) {
-        uint32_t o[32];
-        ptx::tmem_ld_32x32(lane_base + 256u + (uint32_t)(ch * 32), o);
+    for (int ch = 0; ch < 4; ++ch) {
+      uint32_t o[32];
+      if (nb > 0) {
+        ptx::tmem_ld_32x32(lane_base + kOCol + (uint32_t)(ch * 32), o);
         ptx::tmem_wait_ld();
+      } else {
 #pragma unroll
-        for (int c = 0; c < 32; ++c) O[ch * 32 + c] = __uint_as_float(o[c]);
+        for (int c = 0; c < 32; ++c) o[c] = 0u;
       }
-    } else {
+      if (valid) {
+        uint4* dst = reinterpret_cast<uint4*>(p.O + i * p.ldO + (int64_t)hq * kD + ch * 32);
 #pragma unroll
-      for (int c = 0; c < kD; ++c) O[c] = 0.f;
+        for (int c = 0; c < 32; c += 8)
+          dst[c >> 3] = make_uint4(
+              pack_bf16x2(__uint_as_float(o[c]) * inv, __uint_as_float(o[c + 1]) * inv),
+              pack_bf16x2(__uint_as_float(o[c + 2]) * inv, __uint_as_float(o[c + 3]) * inv),
+              pack_bf16x2(__uint_as_float(o[c + 4]) * inv, __uint_as_float(o[c + 5]) * inv),
+              pack_bf16x2(__uint_as_float(o[c + 6]) * inv, __uint_as_float(o[c + 7]) * inv));
+      }
     }
-    const float m_run = m_ref;
-    // out = O / l; lse = ln2 * (m + log2 l)
-    if (valid) {
-      const float inv = l_run > 0.f ? 1.0f / l_run : 0.f;
-      uint4* dst = reinterpret_cast<uint4*>(p.O + i * p.ldO + (int64_t)hq * kD);
-#pragma unroll
-      for (int c = 0; c < kD; c += 8)
-        dst[c >> 3] = make_uint4(pack_bf16x2(O[c] * inv, O[c + 1] * inv),
-                                 pack_bf16x2(O[c + 2] * inv, O[c + 3] * inv),
-                                 pack_bf16x2(O[c + 4] * inv, O[c + 5] * inv),
-                                 pack_bf16x2(O[c + 6] * inv, O[c + 7] * inv));
-      if (p.lse) p.lse[(int64_t)hq * p.S_local + i] = l_run > 0.f ? kLn2 * (m_run + log2f(l_run)) : -INFINITY;
-    }
+    if (valid && p.lse)
+      p.lse[(int64_t)hq * p.S_local + i] = l_run > 0.f ? kLn2 * (m_ref + log2f(l_run)) : -INFINITY;
   }
 
   ptx::tc_fence_before();
   __syncthreads();
-  if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
+  if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, kTmemCols);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -598,8 +598,8 @@ def e2e_train_step(B, b: DeviceBatch, steps, warmup):
               if t is not None)
     return {"value": b.n_scored / (ms * 1e-3), "unit": "scored tokens/s", "h2d_bytes_per_step": h2d,
             "d2h_bytes_per_step": dHh.numel() * dHh.element_size() + 20, "ms_per_step": ms,
-            "pass": "fwd+bwd (gc_grpo_step_host: H copy overlapped with the forward; dH copied back "
-                    "after the backward; dW stays on the device)",
+            "pass": "fwd+bwd (gc_grpo_step_host: H copy overlapped with the forward, dH copied back "
+                    "under the last dW contraction; dW stays on the device)",
             "loss": float(out5h[0])}
 
 

@@ -118,8 +118,10 @@ int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int d
  * copies H, targets, mask, cu_seqlens, rewards, group_offsets, old / ref log-probs to the device
  * (H band by band, overlapped with the forward as above), then gc_grpo_advantages (population
  * std, no group drop) -> forward -> loss -> backward, and copies out5 [5], logp (nullable) and
- * dH [T,D] back to the host.  dW [V,D] (lddW, dW_dtype, accumulate_dW as in gc_grpo_loss_bwd) is
- * model state and stays on the device.  Everything is ordered on `cuda_stream`.
+ * dH [T,D] back to the host -- dH on the side stream as soon as the last non-empty chunk's dH
+ * contraction has finished, i.e. under the last dW contraction.  dW [V,D] (lddW, dW_dtype,
+ * accumulate_dW as in gc_grpo_loss_bwd) is model state and stays on the device.  Everything is
+ * ordered on `cuda_stream` when the call's work completes there.
  * workspace: gc_step_host_workspace_bytes(T, D, V, dtype, R, G, dW_dtype). */
 size_t gc_step_host_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype, int32_t R, int32_t G,
                                     int dW_dtype);

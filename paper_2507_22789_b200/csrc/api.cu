@@ -6,6 +6,13 @@
 using namespace gc;
 
 namespace gc {
+// host_api.cu: an event to record right after the LAST chunk's dH launch of the calling thread's
+// next backward (dH is complete from there on; the step-from-host entry point starts its
+// device -> host copy of dH under the last dW contraction).  Consumed by that backward.
+static thread_local cudaEvent_t t_dh_done_event = nullptr;
+static thread_local int64_t t_dh_done_rows = 0;     // scored rows of the batch (chunks past them are empty)
+void set_bwd_dh_done_event(cudaEvent_t e, int64_t n_scored) { t_dh_done_event = e; t_dh_done_rows = n_scored; }
+
 static thread_local cudaError_t t_last_cuda_error = cudaSuccess;
 void note_cuda_error(cudaError_t e) {
   t_last_cuda_error = e;
@@ -433,6 +440,9 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
     rows = w.rows; n_rows = w.n_rows;
   }
   GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
+  cudaEvent_t dh_done = gc::t_dh_done_event;
+  const int64_t dh_rows = compact ? gc::t_dh_done_rows : T;   // rows that reach the contractions
+  gc::t_dh_done_event = nullptr;
   int ci = 0;
   for (int64_t row0 = 0; row0 < T; row0 += chunk) {
     if (ci + 3 > kTcCounters) {
@@ -449,6 +459,8 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
     // a11: dH rows of this chunk
     GC_TRY(tc_dh(w.dS, ldS, rows_cap, n_static, W, ldW, D, V, rows ? rows + row0 : nullptr, n_rows,
                  row0, dH, lddH, w.counters + ci + 1, st));
+    if (dh_done && row0 < (dh_rows > 0 ? dh_rows : 1) && row0 + chunk >= dh_rows)
+      GC_CUDA_TRY(cudaEventRecord(dh_done, st));     // the last non-empty chunk: dH is complete
     // a12: dW accumulates over chunks in fp32
     if (sink.shards)
       GC_TRY(tc_dw_reduce_scatter(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,

@@ -7,7 +7,10 @@
 #include "../../include/gcore.h"
 
 // the CUDA error behind the calling thread's last GC_ERR_CUDA (api.cu; gc_last_cuda_error)
-namespace gc { void note_cuda_error(cudaError_t e); }
+namespace gc {
+void note_cuda_error(cudaError_t e);
+void set_bwd_dh_done_event(cudaEvent_t e, int64_t n_scored);     // api.cu: see there
+}
 
 #define GC_CUDA_TRY(expr)                         \
   do {                                            \

@@ -12,7 +12,7 @@ using namespace gc;
 
 namespace {
 
-constexpr int kHostEvents = 66;        // fork + small inputs + up to 64 H bands
+constexpr int kHostEvents = 68;        // fork + small inputs + up to 64 H bands + dH done / copied
 
 // Side stream + events, per device, created on first use and kept (process-global state (iv) of
 // gcore.h): creating them per call would cost more than the copy they hide.
@@ -232,12 +232,30 @@ int gc_grpo_step_host(const void* H_host, const void* W, int64_t ldW, int dtype,
   GC_CUDA_TRY(cudaMemcpyAsync(out5_host, w.out5, 5 * sizeof(float), cudaMemcpyDeviceToHost, st));
   if (logp_host)
     GC_CUDA_TRY(cudaMemcpyAsync(logp_host, w.sg.logp, (size_t)T * 4, cudaMemcpyDeviceToHost, st));
-  GC_TRY(gc_grpo_loss_bwd(w.sg.H, D, W, ldW, dtype, w.sg.y, m, T, D, V, temperature, w.cu, R, w.adv,
-                          w.old_lp, rf, clip_lo, clip_hi, beta, agg, w.sg.logp, w.sg.lse, grad_loss,
-                          w.dH, D, dW, lddW, dW_dtype, accumulate_dW, 0, nullptr, w.bwd, w.bwd_bytes,
-                          st));
-  GC_CUDA_TRY(cudaMemcpyAsync(dH_host, w.dH, (size_t)T * (size_t)D * elem_bytes(dtype),
-                              cudaMemcpyDeviceToHost, st));
+  // dH is complete after the last chunk's dH contraction: its copy back to the host runs on the
+  // side stream under the last dW contraction (bf16 tcgen05 path; the SIMT path copies at the end)
+  const bool overlap_dh = dtype == GC_BF16;
+  if (overlap_dh) {
+    int64_t n_scored = 0;          // host-side count: which chunk is the last non-empty one
+    for (int64_t t = 0; t < T; ++t)
+      n_scored += (targets_host[t] >= 0 && (!mask_host || mask_host[t] != 0)) ? 1 : 0;
+    gc::set_bwd_dh_done_event(cx->ev[kHostEvents - 1], n_scored);
+  }
+  const int bs = gc_grpo_loss_bwd(w.sg.H, D, W, ldW, dtype, w.sg.y, m, T, D, V, temperature, w.cu, R,
+                                  w.adv, w.old_lp, rf, clip_lo, clip_hi, beta, agg, w.sg.logp,
+                                  w.sg.lse, grad_loss, w.dH, D, dW, lddW, dW_dtype, accumulate_dW, 0,
+                                  nullptr, w.bwd, w.bwd_bytes, st);
+  gc::set_bwd_dh_done_event(nullptr, 0);
+  GC_TRY(bs);
+  const size_t dh_bytes = (size_t)T * (size_t)D * elem_bytes(dtype);
+  if (overlap_dh) {
+    GC_CUDA_TRY(cudaStreamWaitEvent(cx->cs, cx->ev[kHostEvents - 1], 0));
+    GC_CUDA_TRY(cudaMemcpyAsync(dH_host, w.dH, dh_bytes, cudaMemcpyDeviceToHost, cx->cs));
+    GC_CUDA_TRY(cudaEventRecord(cx->ev[kHostEvents - 2], cx->cs));
+    GC_CUDA_TRY(cudaStreamWaitEvent(st, cx->ev[kHostEvents - 2], 0));     // join: ordered on `st`
+  } else {
+    GC_CUDA_TRY(cudaMemcpyAsync(dH_host, w.dH, dh_bytes, cudaMemcpyDeviceToHost, st));
+  }
   return GC_OK;
 }
 

@@ -21,7 +21,7 @@
  *     exceptions, no abort(), no environment variables.  Process-global state is limited to:
  *     (i) a write-once, atomically published cache of launch attributes per kernel and device
  *     (idempotent: host threads may race on a first launch); (ii) the measurement aid
- *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter of
+ *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter and progress ring of
  *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently); (iv) one side
  *     stream and a few events per device for the *_host entry points.  None of it changes results.  Calls on different streams need different workspaces.
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,

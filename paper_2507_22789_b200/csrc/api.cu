@@ -445,7 +445,7 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
   gc::t_dh_done_event = nullptr;
   int ci = 0;
   for (int64_t row0 = 0; row0 < T; row0 += chunk) {
-    if (ci + 3 > kTcCounters) {
+    if (ci + kCountersPerChunk > kTcCounters) {
       GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
       ci = 0;
     }
@@ -458,19 +458,19 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
                            w.counters + ci, st));
     // a11: dH rows of this chunk
     GC_TRY(tc_dh(w.dS, ldS, rows_cap, n_static, W, ldW, D, V, rows ? rows + row0 : nullptr, n_rows,
-                 row0, dH, lddH, w.counters + ci + 1, st));
+                 row0, dH, lddH, w.counters + ci + 2, st));
     if (dh_done && row0 < (dh_rows > 0 ? dh_rows : 1) && row0 + chunk >= dh_rows)
       GC_CUDA_TRY(cudaEventRecord(dh_done, st));     // the last non-empty chunk: dH is complete
     // a12: dW accumulates over chunks in fp32
     if (sink.shards)
       GC_TRY(tc_dw_reduce_scatter(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
                                   sink.shards, sink.world, sink.shard_rows, lddW,
-                                  w.counters + ci + 2, st));
+                                  w.counters + ci + 1, st));
     else
       GC_TRY(tc_dw(w.dS, ldS, rows_cap, n_static, Hc, ldHs, D, V, n_rows, row0,
                    static_cast<float*>(dW), lddW, (accumulate_dW || row0 > 0) ? 1 : 0,
-                   w.counters + ci + 2, st));
-    ci += 3;
+                   w.counters + ci + 1, st));
+    ci += kCountersPerChunk;
   }
   if (dW_bf16) GC_TRY(launch_cast_f32_bf16(w.dW_acc, D, dW_out, lddW_out, V, D, accumulate_out, st));
   return GC_OK;

@@ -132,8 +132,11 @@ int simt_backward(const void* H, int64_t ldH, const void* W, int64_t ldW, bool b
                   float* dW, int64_t lddW, int accumulate, cudaStream_t st);
 
 // tc_head.cu (tcgen05 engine).  `counter`: a zeroed device word per launch (dynamic item
-// schedule, tc_gemm.cuh); the API zeroes kTcCounters of them once per call.
+// schedule, tc_gemm.cuh) -- for tc_dh kDhLockWords of them (the K-lockstep progress ring); the API
+// zeroes kTcCounters words once per call (again when a long chunk loop runs out of them).
 constexpr int kTcCounters = 1024;
+constexpr int kDhLockWords = 32;                       // == tc::kLockRing
+constexpr int kCountersPerChunk = 2 + kDhLockWords;    // recompute, dW, dH ring
 struct TcPlan {            // forward / recompute schedule: items = (vocab chunk c, M tile)
   int n_vtiles;            // ceil(V / 256)
   int chunk_vtiles;        // vocab tiles per item

@@ -508,7 +508,7 @@ static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   s.M = M; s.N = N; s.K = K;
   s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
   s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0; s.n_band = 0; s.skip_empty_k = 0; s.n_major = 0;
-  s.counter = nullptr; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
+  s.counter = nullptr; s.lockstep = nullptr; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
   return s;
 }
 
@@ -609,7 +609,10 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
   GC_TRY(tc::make_operand_tmap(&ta, dS, rows_cap, V, ldS, false, tc::BM_CTA));
   GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
   Sched s = make_sched(n_rows_dev ? rows_cap : n_static, D, V);
-  (void)counter;   // K-lockstep kernel: all pairs stream V together, static schedule
+  // K-lockstep kernel: all pairs stream V together -- static schedule, paced through `counter`
+  // (tc::kLockRing zeroed words; NULL: unpaced)
+  static_assert(kDhLockWords == tc::kLockRing, "dH progress ring size");
+  s.lockstep = counter;
   // Every wave of 74 tiles streams, over the whole of K = V, the dS rows of the M tiles it covers and
   // the W columns of the N tiles it covers; the operand whose tiles a wave covers COMPLETELY is
   // re-read by every wave.  Order the tiles so that this is the smaller one: dS chunk (rows x V)
@@ -685,8 +688,10 @@ int tc_dw_reduce_scatter(const void* dS, int64_t ldS, int64_t rows_cap, int64_t 
   return tc::launch_tc_gemm<2, true, true, EpiReduceScatterF32, 1, kPpc>(ta, tb, s, ep, st);
 }
 
-// one counter for the debug GEMM (not safe for concurrent debug calls on different streams)
+// one counter and one K-lockstep progress ring for the debug GEMM (not safe for concurrent debug
+// calls on different streams)
 __device__ uint32_t g_debug_counter;
+__device__ uint32_t g_debug_lockstep[tc::kLockRing];
 
 // dH tile waves of a chunk of `rows` rows (api.cu's chunk picker): items of kPpc x (256 x 512) tiles
 // over the scheduling units; a last wave that is at most half full costs half a wave.
@@ -722,6 +727,13 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
     GC_CUDA_TRY(cudaGetSymbolAddress(&ctr, g_debug_counter));
     GC_CUDA_TRY(cudaMemsetAsync(ctr, 0, sizeof(uint32_t), st));
     s.counter = static_cast<uint32_t*>(ctr);
+  }
+  if (dual_n && !dynamic_schedule && c_major != 1) {
+    // the static dual-N launch is dH's: paced like it (K-lockstep window, tc_gemm.cuh)
+    void* ls = nullptr;
+    GC_CUDA_TRY(cudaGetSymbolAddress(&ls, g_debug_lockstep));
+    GC_CUDA_TRY(cudaMemsetAsync(ls, 0, sizeof(uint32_t) * tc::kLockRing, st));
+    s.lockstep = static_cast<uint32_t*>(ls);
   }
   EpiStoreF32::Params ep;
   GC_TRY(make_f32_out_tmap(&ep.tm, C, M, N, ldc));

@@ -107,6 +107,24 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 
+// ---- progress counters in global memory (pacing only: no data is published through them) ----
+__device__ __forceinline__ void red_add_relaxed_gpu(uint32_t* p, uint32_t v) {
+  asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_relaxed_gpu(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// spin until *p >= target (wrap-safe compare), with the same watchdog as the mbarrier waits
+__device__ __forceinline__ void wait_counter_ge(const uint32_t* p, uint32_t target) {
+  if ((int32_t)(ld_relaxed_gpu(p) - target) >= 0) return;
+  const long long t0 = clock64();
+  while ((int32_t)(ld_relaxed_gpu(p) - target) < 0) {
+    if (clock64() - t0 > (1ll << 32)) __trap();
+  }
+}
+
 // ---- TMA -----------------------------------------------------------------------------------
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");

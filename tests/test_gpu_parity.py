@@ -113,6 +113,25 @@ def test_engine_gemm_many_tiles(B, dyn, dual):
     assert torch.equal(C1, C2)
 
 
+@pytest.mark.parametrize("order", [0, 2])
+@pytest.mark.parametrize("cluster4", [False, True])
+def test_engine_gemm_dual_n_paced_long_k(B, order, cluster4):
+    """The dH launch shape with a K long enough for several K-lockstep progress segments
+    (tc_gemm.cuh Sched::lockstep: 16 k-blocks each, here 49 k-blocks = 4 segments, the last one
+    short) over two waves: 110 dual tiles = a full wave of 74 + 36 tiles issued as 72 half tiles,
+    so two pairs have no tile in the last wave and only keep the progress counts going.  Both tile
+    orders; reruns bit-identical."""
+    M, N, K = 256 * 21 + 40, 256 * 9 + 8, 64 * 48 + 40
+    g = torch.Generator(device="cuda").manual_seed(23)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    kw = dict(cta_group=2, dynamic_schedule=False, dual_n=True, c_major=order, cluster4=cluster4)
+    C = B.gc_debug_gemm_bf16(A, Bm.T.contiguous(), 0, 1, **kw)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    assert torch.equal(C, B.gc_debug_gemm_bf16(A, Bm.T.contiguous(), 0, 1, **kw))
+
+
 SCHEDS = {
     "n_band_narrow_last": dict(n_band=4),                       # 10 N tiles -> bands 4, 4, 2
     "n_band_3": dict(n_band=3),                                 # 3, 3, 3, 1

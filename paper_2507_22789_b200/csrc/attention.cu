@@ -40,19 +40,18 @@ constexpr int kBK = GC_ATTN_BK;    // keys per block.  64: 112 KB of shared memo
 static_assert(kBK == 64 || kBK == 128, "key block");
 constexpr int kKB = kBK / 64;      // 64-key k-blocks per block (second contraction)
 constexpr int kCH = kBK / 32;      // 32-column TMEM chunks of a score row
-constexpr int kPBufs = kBK == 64 ? 1 : 2;
 constexpr int kCtasPerSM = kBK == 64 ? 2 : 1;
 constexpr int kTmemCols = kBK == 64 ? 256 : 512;
 constexpr int kThreads = 256;
 constexpr int kQBytes = kBQ * kD * 2;        // 32 KB: 128 x 128 bf16 (two 64-wide k-blocks of 16 KB)
 constexpr int kKSub = kBK * 128;             // one 64-wide k-block of a K tile: kBK rows x 128 B
 constexpr int kKVBytes = kBK * kD * 2;       // a K or V stage
-constexpr int kPBytes = kBQ * kBK * 2;       // a P buffer: kKB k-blocks of 128 rows x 128 B
+constexpr int kKStages = kBK == 64 ? 3 : 2;  // P lives in tensor memory, so shared memory holds only
+constexpr int kVStages = 2;                  // Q and the K / V rings
 constexpr int kSmemQ = 0;
 constexpr int kSmemK = kSmemQ + kQBytes;
-constexpr int kSmemV = kSmemK + 2 * kKVBytes;
-constexpr int kSmemP = kSmemV + 2 * kKVBytes;
-constexpr int kSmemBar = kSmemP + kPBufs * kPBytes;        // tiles, then the barriers
+constexpr int kSmemV = kSmemK + kKStages * kKVBytes;
+constexpr int kSmemBar = kSmemV + kVStages * kKVBytes;     // tiles, then the barriers
 constexpr int kSmemBytes = kSmemBar + 256;                 // (the dynamic smem base is 1024-aligned)
 static_assert(kSmemBytes <= (kCtasPerSM == 2 ? 113 : 227) * 1024, "attention shared memory budget");
 
@@ -156,20 +155,19 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t base = ptx::smem_u32(smem_raw);
   if (base & 1023u) __trap();              // the swizzled tiles need a 1024-byte aligned base
-  const uint32_t sQ = base + kSmemQ, sK = base + kSmemK, sV = base + kSmemV, sP = base + kSmemP;
+  const uint32_t sQ = base + kSmemQ, sK = base + kSmemK, sV = base + kSmemV;
   const uint32_t bar = base + kSmemBar;
   // barriers (8 bytes each)
   const uint32_t q_full = bar;
   auto k_full = [&](int i) { return bar + 8u * (1 + i); };
-  auto k_empty = [&](int i) { return bar + 8u * (3 + i); };
-  auto v_full = [&](int i) { return bar + 8u * (5 + i); };
-  auto v_empty = [&](int i) { return bar + 8u * (7 + i); };
-  auto s_full = [&](int i) { return bar + 8u * (9 + i); };
-  auto s_empty = [&](int i) { return bar + 8u * (11 + i); };
-  auto p_full = [&](int i) { return bar + 8u * (13 + i); };
-  auto p_empty = [&](int i) { return bar + 8u * (15 + i); };
-  const uint32_t o_done = bar + 8u * 17;    // one phase per key block: P_j V_j has been accumulated
-  const uint32_t tmem_slot = bar + 8u * 21;
+  auto k_empty = [&](int i) { return bar + 8u * (5 + i); };
+  auto v_full = [&](int i) { return bar + 8u * (9 + i); };
+  auto v_empty = [&](int i) { return bar + 8u * (13 + i); };
+  auto s_full = [&](int i) { return bar + 8u * (17 + i); };
+  auto p_full = [&](int i) { return bar + 8u * (19 + i); };
+  const uint32_t o_done = bar + 8u * 21;    // one phase per key block: P_j V_j has been accumulated
+  const uint32_t tmem_slot = bar + 8u * 23;
+  static_assert(kKStages <= 4 && kVStages <= 4, "barrier slots");
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int head_local = (int)(blockIdx.x % (unsigned)p.n_q_heads);
@@ -186,15 +184,17 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   }
   if (warp == 1 && lane == 0) {
     ptx::mbar_init(q_full, 1);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kKStages; ++i) {
       ptx::mbar_init(k_full(i), 1);
       ptx::mbar_init(k_empty(i), 1);
+    }
+    for (int i = 0; i < kVStages; ++i) {
       ptx::mbar_init(v_full(i), 1);
       ptx::mbar_init(v_empty(i), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
       ptx::mbar_init(s_full(i), 1);
-      ptx::mbar_init(s_empty(i), 4);       // one arrive per softmax warp
-      ptx::mbar_init(p_full(i), 4);
-      ptx::mbar_init(p_empty(i), 1);
+      ptx::mbar_init(p_full(i), 4);        // one arrive per softmax warp
     }
     ptx::mbar_init(o_done, 1);
     ptx::fence_barrier_init();
@@ -208,7 +208,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
   ptx::tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-  // TMEM columns: S0 [0,kBK) S1 [kBK,2 kBK) O [2 kBK, 2 kBK + 128)
+  // TMEM columns: S0 [0,kBK) S1 [kBK,2 kBK) O [2 kBK, 2 kBK + 128).  P_j (bf16, two per column)
+  // is written IN PLACE over the first kBK / 2 columns of S_j by the rows' owners and read from
+  // there as the A operand of the second contraction: no shared-memory round trip, and the two
+  // S buffers double-buffer P for free.  Buffer j & 1 is written again by S_{j+2}, which the MMA
+  // thread issues after P_j V_j -- the tensor pipe executes in issue order, so no barrier guards it.
   constexpr uint32_t kOCol = 2u * kBK;
 
   if (warp == 0) {
@@ -223,8 +227,8 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       ptx::tma_load_2d(sQ, &tmQ, q_col, q_row, q_full, pol_q);
       ptx::tma_load_2d(sQ + 16384, &tmQ, q_col + 64, q_row, q_full, pol_q);
       auto load_k = [&](int j) {
-        const int st = j & 1;
-        ptx::mbar_wait(k_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
+        const int st = j % kKStages;
+        ptx::mbar_wait(k_empty(st), (((uint32_t)(j / kKStages)) & 1u) ^ 1u);
         ptx::mbar_arrive_expect_tx(k_full(st), kKVBytes);
         const int32_t row = (tm.kb_begin + j) * kBK;
         const uint32_t dst = sK + st * kKVBytes;
@@ -232,8 +236,8 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
         ptx::tma_load_2d(dst + kKSub, &tmK, kv_col + 64, row, k_full(st), pol_kv);
       };
       auto load_v = [&](int j) {
-        const int st = j & 1;
-        ptx::mbar_wait(v_empty(st), (((uint32_t)j >> 1) & 1u) ^ 1u);
+        const int st = j % kVStages;
+        ptx::mbar_wait(v_empty(st), (((uint32_t)(j / kVStages)) & 1u) ^ 1u);
         ptx::mbar_arrive_expect_tx(v_full(st), kKVBytes);
         const int32_t row = (tm.kb_begin + j) * kBK;
         const uint32_t dst = sV + st * kKVBytes;
@@ -245,9 +249,9 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
             ptx::tma_load_2d(dst + kb * 16384 + nbx * 8192, &tmV, kv_col + 64 * nbx, row + 64 * kb,
                              v_full(st), pol_kv);
       };
-      load_k(0);
+      for (int j = 0; j < kKStages - 1 && j < nb; ++j) load_k(j);
       for (int j = 0; j < nb; ++j) {
-        if (j + 1 < nb) load_k(j + 1);
+        if (j + kKStages - 1 < nb) load_k(j + kKStages - 1);
         load_v(j);
       }
     }
@@ -257,12 +261,10 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       constexpr uint32_t idesc_qk = ptx::make_idesc_bf16(kBQ, kBK, false, false);
       constexpr uint32_t idesc_pv = ptx::make_idesc_bf16(kBQ, kD, false, true);
       auto issue_s = [&](int j) {
-        const int st = j & 1;
-        const uint32_t ph = ((uint32_t)j >> 1) & 1u;
-        ptx::mbar_wait(k_full(st), ph);
-        ptx::mbar_wait(s_empty(st), ph ^ 1u);
+        const int st = j % kKStages;
+        ptx::mbar_wait(k_full(st), ((uint32_t)(j / kKStages)) & 1u);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)(st * kBK);
+        const uint32_t d_tmem = tmem_base + (uint32_t)((j & 1) * kBK);
 #pragma unroll
         for (int kb = 0; kb < 2; ++kb) {            // the two 64-wide halves of head_dim
           const uint64_t adesc = ptx::make_smem_desc(sQ + kb * 16384, false);
@@ -273,28 +275,24 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
                               (uint32_t)(kb | k));
         }
         ptx::umma_commit<1>(k_empty(st));      // the K stage is free once these MMAs have read it
-        ptx::umma_commit<1>(s_full(st));
+        ptx::umma_commit<1>(s_full(j & 1));
       };
-      auto issue_pv = [&](int j) {             // O (+)= P_j V_j
-        const int st = j & 1;
-        const uint32_t ph = ((uint32_t)j >> 1) & 1u;
-        const int pst = j % kPBufs;
-        const uint32_t pph = ((uint32_t)(j / kPBufs)) & 1u;
-        ptx::mbar_wait(v_full(st), ph);
-        ptx::mbar_wait(p_full(pst), pph);        // P_j written, and O rescaled if it had to be
+      auto issue_pv = [&](int j) {             // O (+)= P_j V_j, P_j read from tensor memory
+        const int st = j % kVStages;
+        ptx::mbar_wait(v_full(st), ((uint32_t)(j / kVStages)) & 1u);
+        ptx::mbar_wait(p_full(j & 1), ((uint32_t)j >> 1) & 1u);   // P_j written, O rescaled if it had to be
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + kOCol;
+        const uint32_t a_tmem = tmem_base + (uint32_t)((j & 1) * kBK);
 #pragma unroll
         for (int kb = 0; kb < kKB; ++kb) {
-          const uint64_t adesc = ptx::make_smem_desc(sP + pst * kPBytes + kb * 16384, false);
           const uint64_t bdesc = ptx::make_smem_desc(sV + st * kKVBytes + kb * 16384, true);
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            ptx::umma_bf16<1>(d_tmem, adesc + (uint64_t)(k * 2), bdesc + (uint64_t)(k * 128),
+            ptx::umma_bf16_ts(d_tmem, a_tmem + (uint32_t)((kb * 4 + k) * 8), bdesc + (uint64_t)(k * 128),
                               idesc_pv, (uint32_t)(j | kb | k));
         }
         ptx::umma_commit<1>(v_empty(st));
-        ptx::umma_commit<1>(p_empty(pst));
         ptx::umma_commit<1>(o_done);
       };
       ptx::mbar_wait(q_full, 0);
@@ -314,8 +312,6 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
     const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16);
     float m_ref = -1e30f;     // the maximum P, l and O are relative to (log2 domain), raised lazily
     float l_run = 0.f;
-    const uint32_t p_row = (uint32_t)row * 128u;
-    const uint32_t sw = (uint32_t)(row & 7);
     constexpr float kLazy = 8.0f;              // P <= 2^8 between raises of the reference
 
     for (int j = 0; j < nb; ++j) {
@@ -325,16 +321,11 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       const bool need_mask = k0 < tm.lo_max || k0 + kBK > tm.hi_min;
       ptx::mbar_wait(s_full(st), ph);
       ptx::tc_fence_after();
-      // the whole score row in one TMEM round trip, then the S buffer goes back to the MMA warp
-      const int pst = j % kPBufs;
-      const uint32_t pph = ((uint32_t)(j / kPBufs)) & 1u;
+      // the whole score row in one TMEM round trip
       uint32_t r[kCH][32];
 #pragma unroll
       for (int ch = 0; ch < kCH; ++ch) ptx::tmem_ld_32x32(lane_base + (uint32_t)(st * kBK + ch * 32), r[ch]);
       ptx::tmem_wait_ld();
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(s_empty(st));
       if (need_mask) {
 #pragma unroll
         for (int ch = 0; ch < kCH; ++ch)
@@ -359,29 +350,28 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       const float factor = raise ? ptx::ex2(m_ref - m_new) : 1.0f;
       m_ref = m_new;
       l_run *= factor;
-      // p = 2^(s * scale2 - m_ref), row sum, P -> bf16 -> swizzled smem (A operand of P V)
-      ptx::mbar_wait(p_empty(pst), pph ^ 1u);
+      // p = 2^(s * scale2 - m_ref), row sum, P -> bf16 pairs -> tensor memory, over S_j
       float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
-      for (int ch = 0; ch < kCH; ++ch) {
-        float e[32];
+      for (int cp = 0; cp < kCH / 2; ++cp) {
+        uint32_t pk[32];
 #pragma unroll
-        for (int c = 0; c < 32; ++c) e[c] = ptx::ex2(fmaf(__uint_as_float(r[ch][c]), p.scale2, -m_new));
+        for (int h = 0; h < 2; ++h) {
+          const int ch = 2 * cp + h;
+          float e[32];
 #pragma unroll
-        for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
-        const uint32_t pb = sP + pst * kPBytes + (uint32_t)(ch >> 1) * 16384u + p_row;
+          for (int c = 0; c < 32; ++c) e[c] = ptx::ex2(fmaf(__uint_as_float(r[ch][c]), p.scale2, -m_new));
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          const uint32_t chunk = (uint32_t)((ch & 1) * 4 + cc);
-          st_shared_v4_u32(pb + ((chunk ^ sw) << 4), pack_bf16x2(e[8 * cc], e[8 * cc + 1]),
-                           pack_bf16x2(e[8 * cc + 2], e[8 * cc + 3]),
-                           pack_bf16x2(e[8 * cc + 4], e[8 * cc + 5]),
-                           pack_bf16x2(e[8 * cc + 6], e[8 * cc + 7]));
+          for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
+#pragma unroll
+          for (int c = 0; c < 16; ++c) pk[16 * h + c] = pack_bf16x2(e[2 * c], e[2 * c + 1]);
         }
+        ptx::tmem_st_32x32(lane_base + (uint32_t)(st * kBK + cp * 32), pk);
       }
       l_run += sum0 + sum1;
       // O holds blocks 0 .. j-1 relative to the old reference: wait for P_{j-1} V_{j-1} (long done:
       // it ran under the exponentials above), rescale the rows whose reference was raised
+      // (the wait is taken every block: it keeps this thread on o_done's current phase)
       if (j > 0) {
         ptx::mbar_wait(o_done, (uint32_t)(j - 1) & 1u);
         if (__any_sync(0xffffffffu, raise)) {
@@ -395,13 +385,12 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
             for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * factor);
             ptx::tmem_st_32x32(lane_base + kOCol + (uint32_t)(ch * 32), o);
           }
-          ptx::tmem_wait_st();
-          ptx::tc_fence_before();
         }
       }
-      ptx::fence_proxy_async_smem();
+      ptx::tmem_wait_st();
+      ptx::tc_fence_before();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(p_full(pst));
+      if (lane == 0) ptx::mbar_arrive(p_full(st));
     }
     // out = O / l; lse = ln2 * (m + log2 l): read O from TMEM 32 columns at a time and store
     if (nb > 0) {

@@ -258,6 +258,18 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint6
         : "memory");
 }
 
+// D[tmem] (+)= A[tmem] * B[smem desc] (cta_group::1): the A operand is read from tensor memory --
+// row m of the 128 x 16 A slice in lane m, its 16 bf16 elements packed two per 32-bit column
+// (element 2c in the low half of column c), 8 columns per UMMA_K = 16.
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc,
+                                             uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
 // Arrive on an mbarrier when all previously issued MMAs of this thread have completed.
 // CG == 2: arrives on the barrier at the same offset in every CTA of `cta_mask`.
 template <int CG>

@@ -139,6 +139,26 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&v);
 }
+// packed fp32 pairs (Blackwell FFMA2 / FADD2): one issue slot for two scores
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+  uint64_t v;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi));
+  return v;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
 __device__ __forceinline__ void st_shared_v4_u32(uint32_t addr, uint32_t a, uint32_t b, uint32_t c,
                                                  uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d)
@@ -351,23 +371,28 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
       m_ref = m_new;
       l_run *= factor;
       // p = 2^(s * scale2 - m_ref), row sum, P -> bf16 pairs -> tensor memory, over S_j
-      float sum0 = 0.f, sum1 = 0.f;
+      const uint64_t scale_2 = pack2(p.scale2, p.scale2), neg_m2 = pack2(-m_new, -m_new);
+      uint64_t sum_a = pack2(0.f, 0.f), sum_b = sum_a;
 #pragma unroll
       for (int cp = 0; cp < kCH / 2; ++cp) {
         uint32_t pk[32];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int ch = 2 * cp + h;
-          float e[32];
 #pragma unroll
-          for (int c = 0; c < 32; ++c) e[c] = ptx::ex2(fmaf(__uint_as_float(r[ch][c]), p.scale2, -m_new));
-#pragma unroll
-          for (int c = 0; c < 32; c += 2) { sum0 += e[c]; sum1 += e[c + 1]; }
-#pragma unroll
-          for (int c = 0; c < 16; ++c) pk[16 * h + c] = pack_bf16x2(e[2 * c], e[2 * c + 1]);
+          for (int c = 0; c < 32; c += 2) {
+            float x0, x1;
+            unpack2(ffma2(pack2(__uint_as_float(r[ch][c]), __uint_as_float(r[ch][c + 1])), scale_2, neg_m2),
+                    x0, x1);
+            const float e0 = ptx::ex2(x0), e1 = ptx::ex2(x1);
+            if (c & 2) sum_b = fadd2(sum_b, pack2(e0, e1)); else sum_a = fadd2(sum_a, pack2(e0, e1));
+            pk[16 * h + (c >> 1)] = pack_bf16x2(e0, e1);
+          }
         }
         ptx::tmem_st_32x32(lane_base + (uint32_t)(st * kBK + cp * 32), pk);
       }
+      float sum0, sum1;
+      unpack2(fadd2(sum_a, sum_b), sum0, sum1);
       l_run += sum0 + sum1;
       // O holds blocks 0 .. j-1 relative to the old reference: wait for P_{j-1} V_{j-1} (long done:
       // it ran under the exponentials above), rescale the rows whose reference was raised

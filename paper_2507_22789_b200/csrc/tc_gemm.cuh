@@ -72,6 +72,8 @@ struct Sched {
                           // then covers every M tile and few N tiles, so the A operand is what gets
                           // re-read per wave; 0: (M tile, N tile), B is re-read per wave.  Pick the
                           // order that re-reads the SMALLER operand (K-lockstep kernels: dH).
+  int a_slab, b_slab;     // MN-major operand whose tensor map is the 3-D slab form (make_operand_tmap):
+                          // the stage's 64-wide slabs come in ONE TMA box instead of one per slab
   uint32_t* lockstep;     // static schedule, NSUB == 2 only (nullable): kLockRing zeroed device words.
                           // The pairs of a wave stream the same K range of both operands; left alone
                           // they drift apart by more k-blocks than the L2 holds and every pair
@@ -338,6 +340,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               const uint32_t fb = full_bar(stage);
               if constexpr (!A_MN) ptx::tma_load_2d(sa, &tmA, k_coord, m_coord, fb, polA);
+              else if (s.a_slab) ptx::tma_load_3d(sa, &tmA, 0, k_coord, m_coord >> 6, fb, polA);
               else {
                 ptx::tma_load_2d(sa, &tmA, m_coord, k_coord, fb, polA);
                 ptx::tma_load_2d(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
@@ -348,6 +351,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                 const uint32_t sbs = sb + sub * C::kBBytes;
                 const int32_t nc = n_coord + sub * BN;
                 if constexpr (!B_MN) ptx::tma_load_2d(sbs, &tmB, k_coord, nc, fb, polB);
+                else if (s.b_slab) ptx::tma_load_3d(sbs, &tmB, 0, k_coord, nc >> 6, fb, polB);
                 else {
 #pragma unroll
                   for (int b = 0; b < C::kBRows / 64; ++b)
@@ -359,6 +363,7 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
               if (prank == 0) ptx::mbar_arrive_expect_tx(full_bar(stage), stage_tx * 2);
               const uint32_t fb = ptx::mapa(full_bar(stage), lead);
               if constexpr (!A_MN) ptx::tma_load_2d_cg2(sa, &tmA, k_coord, m_coord, fb, polA);
+              else if (s.a_slab) ptx::tma_load_3d_cg2(sa, &tmA, 0, k_coord, m_coord >> 6, fb, polA);
               else {
                 ptx::tma_load_2d_cg2(sa, &tmA, m_coord, k_coord, fb, polA);
                 ptx::tma_load_2d_cg2(sa + 8192, &tmA, m_coord + 64, k_coord, fb, polA);
@@ -379,6 +384,8 @@ k_tc_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUten
                                             b_mask, polB);
                 } else if constexpr (!B_MN) {
                   ptx::tma_load_2d_cg2(sbs, &tmB, k_coord, nc, fb, polB);
+                } else if (s.b_slab) {
+                  ptx::tma_load_3d_cg2(sbs, &tmB, 0, k_coord, nc >> 6, fb, polB);
                 } else {
 #pragma unroll
                   for (int b = 0; b < C::kBRows / 64; ++b)
@@ -570,6 +577,28 @@ inline int make_operand_tmap(CUtensorMap* m, const void* base, int64_t rows, int
                              bool mn_major, int box_rows) {
   if (!mn_major) return make_tmap_bf16(m, base, K, rows, ld, BK, box_rows);
   return make_tmap_bf16(m, base, rows, K, ld, 64, BK);
+}
+
+// MN-major operand in slab form: memory [K, rows] with rows % 64 == 0 seen as the 3-D tensor
+// {64 mn in a slab, K, rows / 64 slabs} (strides: ld elements between k, 64 elements between slabs);
+// a box of `slabs` slabs x 64 k lands in shared memory as `slabs` consecutive 8 KB [64 k][64 mn]
+// tiles -- exactly what `slabs` 2-D boxes would write, in one TMA instruction.  Slabs past the
+// extent are zero-filled.  (rows % 64 != 0 cannot take this form: the last slab would run into
+// the next k row.)
+inline int make_slab_tmap_bf16(CUtensorMap* m, const void* base, int64_t rows, int64_t K, int64_t ld,
+                               int slabs) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return GC_ERR_CUDA;
+  if (rows <= 0 || K <= 0 || rows % 64 != 0 || slabs < 1) return GC_ERR_SHAPE;
+  if ((reinterpret_cast<uintptr_t>(base) & 15) || ((ld * 2) & 15)) return GC_ERR_ALIGN;
+  cuuint64_t dims[3] = {64, (cuuint64_t)K, (cuuint64_t)(rows / 64)};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * 2, 128};
+  cuuint32_t box[3] = {64, (cuuint32_t)BK, (cuuint32_t)slabs};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box,
+                  estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? GC_OK : GC_ERR_CUDA;
 }
 
 inline int num_sms() {

@@ -505,12 +505,23 @@ static int launch_any(int cg, bool dual_n, int ppc, const CUtensorMap& a, const 
 // K-major B operand: rows of one TMA box = the share of the 256-row tile one CTA fetches
 static int b_box_rows(int cg, int ppc) { return tc::BN / cg / ppc; }
 
+// MN-major operand [K, rows]: the slab form (one TMA box per stage, tc_gemm.cuh) when rows is a
+// multiple of 64 -- `padded_rows` >= rows says how far the buffer's rows really extend (zero-filled
+// padding, e.g. the dS chunk buffer) -- else one 2-D box per 64-wide slab.  *slab tells which.
+static int make_mn_tmap(CUtensorMap* m, const void* base, int64_t rows, int64_t padded_rows, int64_t K,
+                        int64_t ld, int slabs, bool allow_slab, int* slab) {
+  const int64_t r64 = ceil_div(rows, 64) * 64;
+  *slab = (allow_slab && r64 <= padded_rows) ? 1 : 0;
+  if (*slab) return tc::make_slab_tmap_bf16(m, base, r64, K, ld, slabs);
+  return tc::make_operand_tmap(m, base, rows, K, ld, true, 0);
+}
+
 static Sched make_sched(int64_t M, int64_t N, int64_t K) {
   Sched s;
   s.M = M; s.N = N; s.K = K;
   s.n_dyn = nullptr; s.dyn_row0 = 0; s.dyn_cap = 0; s.dyn_dim = 0; s.dyn_round = 1;
   s.chunk_ntiles = 1; s.c_major = 0; s.m_band = 0; s.n_band = 0; s.skip_empty_k = 0; s.n_major = 0;
-  s.counter = nullptr; s.lockstep = nullptr; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
+  s.counter = nullptr; s.lockstep = nullptr; s.a_slab = 0; s.b_slab = 0; s.a_hint = ptx::kL2Normal; s.b_hint = ptx::kL2Normal;
   return s;
 }
 
@@ -609,8 +620,10 @@ int tc_dh(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
           int64_t row0, void* dH, int64_t lddH, uint32_t* counter, cudaStream_t st) {
   CUtensorMap ta, tb;
   GC_TRY(tc::make_operand_tmap(&ta, dS, rows_cap, V, ldS, false, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, W, D, V, ldW, true, 0));
+  int b_slab = 0;                            // W as 64-wide slabs: one TMA box per B sub-tile and stage
+  GC_TRY(make_mn_tmap(&tb, W, D, D, V, ldW, tc::BN / 2 / 64, kPpc == 1, &b_slab));
   Sched s = make_sched(n_rows_dev ? rows_cap : n_static, D, V);
+  s.b_slab = b_slab;
   // K-lockstep kernel: all pairs stream V together -- static schedule, paced through `counter`
   // (tc::kLockRing zeroed words; NULL: unpaced)
   static_assert(kDhLockWords == tc::kLockRing, "dH progress ring size");
@@ -638,9 +651,14 @@ int tc_dw(const void* dS, int64_t ldS, int64_t rows_cap, int64_t n_static, const
           int64_t lddW, int accumulate, uint32_t* counter, cudaStream_t st) {
   const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
   CUtensorMap ta, tb;
-  GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
-  GC_TRY(tc::make_operand_tmap(&tb, Hs, D, k_rows, ldH, true, 0));
+  // both operands MN-major; in slab form (one TMA box per operand and stage instead of two) when
+  // their row counts allow: dS is padded with zero columns up to ldS = ceil(V / 64) 64
+  int a_slab = 0, b_slab = 0;
+  GC_TRY(make_mn_tmap(&ta, dS, V, ldS, rows_cap, ldS, tc::BM_CTA / 64, true, &a_slab));
+  GC_TRY(make_mn_tmap(&tb, Hs, D, D, k_rows, ldH, tc::BN / 2 / 64, kPpc == 1, &b_slab));
   Sched s = make_sched(V, D, k_rows);
+  s.a_slab = a_slab;
+  s.b_slab = b_slab;
   // items (D band, vocab tile, D tile in band): the band's H panels stay in L2, the D tiles of a
   // vocab tile run together and share its dS^T panel, which streams past once per band
   s.counter = counter;
@@ -665,9 +683,12 @@ int tc_dw_reduce_scatter(const void* dS, int64_t ldS, int64_t rows_cap, int64_t 
   if (shard_rows * world < V) return GC_ERR_SHAPE;
   const int64_t k_rows = n_rows_dev ? rows_cap : n_static;
   CUtensorMap ta, tb;
-  GC_TRY(tc::make_operand_tmap(&ta, dS, V, rows_cap, ldS, true, 0));
-  GC_TRY(tc::make_operand_tmap(&tb, Hs, D, k_rows, ldH, true, 0));
+  int a_slab = 0, b_slab = 0;
+  GC_TRY(make_mn_tmap(&ta, dS, V, ldS, rows_cap, ldS, tc::BM_CTA / 64, true, &a_slab));
+  GC_TRY(make_mn_tmap(&tb, Hs, D, D, k_rows, ldH, tc::BN / 2 / 64, kPpc == 1, &b_slab));
   Sched s = make_sched(V, D, k_rows);
+  s.a_slab = a_slab;
+  s.b_slab = b_slab;
   s.counter = counter;
   s.a_hint = ptx::kL2Normal;
   s.b_hint = ptx::kL2EvictLast;
@@ -714,9 +735,16 @@ int tc_debug_gemm(const void* A, int64_t lda, int a_mn, const void* B, int64_t l
   const int ppc = cluster4 ? 2 : 1;
   if (N % 4 != 0) return GC_ERR_SHAPE;
   CUtensorMap ta, tb;
-  GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, a_mn != 0, tc::BM_CTA));
-  GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, b_mn != 0, b_box_rows(cta_group, ppc)));
+  // MN-major operands take the slab form whenever their extent is a multiple of 64 (as the path's
+  // kernels do), the per-slab 2-D boxes otherwise
+  int a_slab = 0, b_slab = 0;
+  if (a_mn) GC_TRY(make_mn_tmap(&ta, A, M, M, K, lda, tc::BM_CTA / 64, true, &a_slab));
+  else GC_TRY(tc::make_operand_tmap(&ta, A, M, K, lda, false, tc::BM_CTA));
+  if (b_mn) GC_TRY(make_mn_tmap(&tb, B, N, N, K, ldb, tc::BN / cta_group / 64, ppc == 1, &b_slab));
+  else GC_TRY(tc::make_operand_tmap(&tb, B, N, K, ldb, false, b_box_rows(cta_group, ppc)));
   Sched s = make_sched(M, N, K);
+  s.a_slab = a_slab;
+  s.b_slab = b_slab;
   // the item orders of the path's kernels (forward / recompute: c_major + m_band + chunk_ntiles;
   // dW: n_band), reachable here at any size
   s.c_major = c_major == 1 ? 1 : 0;

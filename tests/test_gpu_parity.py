@@ -113,6 +113,26 @@ def test_engine_gemm_many_tiles(B, dyn, dual):
     assert torch.equal(C1, C2)
 
 
+@pytest.mark.parametrize("cg,dual", [(1, False), (2, False), (2, True)])
+@pytest.mark.parametrize("a_mn,b_mn", [(0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K", [(256 * 5 + 64, 256 * 3 + 128, 328), (256 * 21 + 192, 256 * 9 + 64, 200)])
+def test_engine_gemm_mn_major_slab_maps(B, cg, dual, a_mn, b_mn, M, N, K):
+    """MN-major operands whose extent is a multiple of 64 are fetched through the 3-D slab tensor map
+    (one TMA box per operand and stage; tc_gemm.cuh make_slab_tmap_bf16) -- the form the dH and dW
+    launches use at every config: several tiles, edge tiles with whole slabs out of bounds
+    (zero-filled), K not a multiple of 64, store and accumulate."""
+    g = torch.Generator(device="cuda").manual_seed(M + N + K + 3)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    args = (A.T.contiguous() if a_mn else A, Bm.T.contiguous() if b_mn else Bm, a_mn, b_mn)
+    kw = dict(cta_group=cg, dynamic_schedule=not dual, dual_n=dual)
+    C = B.gc_debug_gemm_bf16(*args, C_out=torch.full((M, N), 3.0, device="cuda"), **kw)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    C2 = B.gc_debug_gemm_bf16(*args, C_out=C.clone(), accumulate=True, **kw)
+    assert (C2.double() - 2 * ref).abs().max().item() < 2e-3 * K ** 0.5
+
+
 @pytest.mark.parametrize("order", [0, 2])
 @pytest.mark.parametrize("cluster4", [False, True])
 def test_engine_gemm_dual_n_paced_long_k(B, order, cluster4):

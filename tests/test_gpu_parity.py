@@ -152,6 +152,21 @@ def test_engine_gemm_dual_n_paced_long_k(B, order, cluster4):
     assert torch.equal(C, B.gc_debug_gemm_bf16(A, Bm.T.contiguous(), 0, 1, **kw))
 
 
+def test_engine_gemm_dual_n_paced_ring_wraps(B):
+    """K long enough for 37 progress segments, more than the 32 slots of the counter ring
+    (tc_gemm.cuh kLockRing), so every slot is used a second time; 6 dual tiles issued as 12 half
+    tiles on 12 of the 74 pairs, the other 62 only keep the counts going."""
+    M, N, K = 256 * 3, 512 * 2, 64 * 16 * 36 + 40
+    g = torch.Generator(device="cuda").manual_seed(29)
+    A = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+    Bm = torch.randn(N, K, device="cuda", generator=g).to(torch.bfloat16)
+    ref = A.double() @ Bm.double().T
+    kw = dict(cta_group=2, dynamic_schedule=False, dual_n=True)
+    C = B.gc_debug_gemm_bf16(A, Bm.T.contiguous(), 0, 1, **kw)
+    assert (C.double() - ref).abs().max().item() < 1e-3 * K ** 0.5
+    assert torch.equal(C, B.gc_debug_gemm_bf16(A, Bm.T.contiguous(), 0, 1, **kw))
+
+
 SCHEDS = {
     "n_band_narrow_last": dict(n_band=4),                       # 10 N tiles -> bands 4, 4, 2
     "n_band_3": dict(n_band=3),                                 # 3, 3, 3, 1

@@ -622,7 +622,7 @@ def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
         out["tokens_kept_after_group_filter"] = b.T_kept
         out["flow"] = "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"
     if with_e2e and w.backward and not w.drop_constant_groups:
-        out["e2e"] = e2e_train_step(B, b, max(2, steps // 2), 2)
+        out["e2e"] = e2e_train_step(B, b, steps, 3)     # as many timed steps as the device figure
     del b, step
     gc.collect()
     torch.cuda.empty_cache()
@@ -868,7 +868,7 @@ def main():
                 torch.cuda.empty_cache()
                 # the metric's fwd+bwd half and the largest configs, each with its rooflines
                 wl = {}
-                for name, k, wu in (("cfg2", max(4, args.steps // 4), 3), ("cfg4", 4, 3), ("cfg3", 3, 2)):
+                for name, k, wu in (("cfg2", max(4, args.steps // 4), 3), ("cfg4", 4, 3), ("cfg3", 3, 3)):
                     wl[name] = measure_workload(B, I.CONFIGS[WORKLOADS[name]], device, k, wu, peaks,
                                                 with_e2e=(name == "cfg2"))
                     out["rooflines"] = out["rooflines"] + wl[name]["rooflines"]

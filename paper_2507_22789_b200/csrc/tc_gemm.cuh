@@ -29,8 +29,8 @@ constexpr int kABytes = BM_CTA * BK * 2;   // 16 KB
 // cuts the L2 -> smem operand traffic per flop by a quarter; the epilogue then cannot overlap
 // the next tile's MMAs, so it is for contractions with a very long K (dH: K = V).
 // kEpiSmem = staging bytes the epilogue functor wants per CTA; the operand ring takes the stages
-// that fit in what is left of the 227 KB (7 x 32 KB with no staging, 5 with the fp32 TMA-store
-// epilogue's 64 KB, 4 x 48 KB for dual-N).
+// that fit in what is left of the 227 KB (7 x 32 KB with no staging, 6 with the fp32 TMA-store
+// epilogue's 16 KB, 4 x 48 KB for dual-N).
 template <int CG, int NSUB = 1, int kEpiSmem = 0> struct Cfg {
   static_assert(NSUB == 1 || (NSUB == 2 && CG == 2), "dual-N needs the CTA pair");
   static constexpr int kBRows = BN / CG;                 // B rows of one sub-tile staged by one CTA

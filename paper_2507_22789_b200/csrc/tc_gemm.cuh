@@ -103,17 +103,24 @@ __device__ __forceinline__ void resolve_dims(const Sched& s, int64_t& M, int64_t
 
 struct Item { int64_t m_tile, n0, n1, c; int half; };   // half: dual-N tail, see k_tc_gemm
 
-__device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt, int64_t Nt) {
+// Item index -> tile coordinates.  Every role of every CTA calls this once per item -- the MMA
+// lane before it can issue the item's first MMA -- so the arithmetic is 32-bit (tile counts and
+// item indices are far below 2^31; a 64-bit division is a ~100-instruction subroutine on the GPU,
+// and three of them per item were a measurable bubble on short items: dW at K = 4096).
+__device__ __forceinline__ Item get_item(const Sched& s, int64_t it64, int64_t Mt64, int64_t Nt64) {
+  const uint32_t it = (uint32_t)it64, Mt = (uint32_t)Mt64, Nt = (uint32_t)Nt64;
+  const uint32_t ck = (uint32_t)s.chunk_ntiles;
   Item x;
   x.half = -1;
+  uint32_t m_tile, n0, n1, c = 0;
   if (s.c_major) {
-    const int64_t C = (Nt + s.chunk_ntiles - 1) / s.chunk_ntiles;
-    const int64_t band = s.m_band > 0 ? s.m_band : Mt;
-    const int64_t full_bands = Mt / band;
-    const int64_t items_full = full_bands * C * band;
-    int64_t rem, mb, m0;
+    const uint32_t C = (Nt + ck - 1) / ck;
+    const uint32_t band = s.m_band > 0 ? (uint32_t)s.m_band : Mt;
+    const uint32_t full_bands = Mt / band;
+    const uint32_t items_full = full_bands * C * band;
+    uint32_t rem, mb, m0;
     if (it < items_full) {
-      const int64_t b = it / (C * band);
+      const uint32_t b = it / (C * band);
       rem = it - b * C * band;
       mb = band;
       m0 = b * band;
@@ -122,31 +129,30 @@ __device__ __forceinline__ Item get_item(const Sched& s, int64_t it, int64_t Mt,
       mb = Mt - full_bands * band;
       m0 = full_bands * band;
     }
-    x.c = rem / mb;
-    x.m_tile = m0 + (rem - x.c * mb);
-    x.n0 = x.c * s.chunk_ntiles;
-    x.n1 = x.n0 + s.chunk_ntiles < Nt ? x.n0 + s.chunk_ntiles : Nt;
-  } else if (s.n_band > 0 && s.n_band < Nt) {
-    const int64_t per_band = Mt * s.n_band;
-    const int64_t b = it / per_band;
-    const int64_t n_start = b * s.n_band;
-    const int64_t w = Nt - n_start < s.n_band ? Nt - n_start : s.n_band;   // last band: narrower
-    const int64_t rem = it - b * per_band;
-    x.m_tile = rem / w;
-    x.n0 = n_start + (rem - x.m_tile * w);
-    x.n1 = x.n0 + 1;
-    x.c = 0;
+    c = rem / mb;
+    m_tile = m0 + (rem - c * mb);
+    n0 = c * ck;
+    n1 = n0 + ck < Nt ? n0 + ck : Nt;
+  } else if (s.n_band > 0 && (uint32_t)s.n_band < Nt) {
+    const uint32_t nbw = (uint32_t)s.n_band;
+    const uint32_t per_band = Mt * nbw;
+    const uint32_t b = it / per_band;
+    const uint32_t n_start = b * nbw;
+    const uint32_t w = Nt - n_start < nbw ? Nt - n_start : nbw;   // last band: narrower
+    const uint32_t rem = it - b * per_band;
+    m_tile = rem / w;
+    n0 = n_start + (rem - m_tile * w);
+    n1 = n0 + 1;
   } else if (s.n_major) {
-    x.n0 = it / Mt;
-    x.m_tile = it - x.n0 * Mt;
-    x.n1 = x.n0 + 1;
-    x.c = 0;
+    n0 = it / Mt;
+    m_tile = it - n0 * Mt;
+    n1 = n0 + 1;
   } else {
-    x.m_tile = it / Nt;
-    x.n0 = it - x.m_tile * Nt;
-    x.n1 = x.n0 + 1;
-    x.c = 0;
+    m_tile = it / Nt;
+    n0 = it - m_tile * Nt;
+    n1 = n0 + 1;
   }
+  x.m_tile = m_tile; x.n0 = n0; x.n1 = n1; x.c = c;
   return x;
 }
 

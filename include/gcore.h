@@ -24,6 +24,12 @@
  *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter and progress ring of
  *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently); (iv) one side
  *     stream and a few events per device for the *_host entry points.  None of it changes results.  Calls on different streams need different workspaces.
+ *   - The tensor-core kernels are persistent (one CTA per SM) and the CTA pairs of the dH launch
+ *     pace one another through progress counters: they are meant to own the GPU.  A kernel of
+ *     another stream or process that holds some SMs only delays them, but every wait inside the
+ *     kernels carries a watchdog of 2^32 cycles (~2-3 s) that turns a wait longer than that --
+ *     a protocol bug, or SMs withheld for that long -- into a launch failure (GC_ERR_CUDA at the
+ *     next call that checks) instead of a hang.
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V

@@ -116,6 +116,35 @@ def test_long_sequence_sampled_rows(B):
         assert np.abs(lse[:, q].cpu().numpy() - l_ref[:, 0]).max() <= 2e-3, q
 
 
+def test_bench_configuration_sampled_rows(B):
+    """The launch bench.py times (attention_workload, cp8_last_rank_131072): the last of 8
+    context-parallel ranks, its 16384 queries against all 131072 gathered keys, causal, 16 / 4 heads,
+    two key/value heads gathered per step -- sampled query rows (tile edges, the chunk's first and
+    last rows, random) against the oracle."""
+    S, Hq, Hkv, world, hps = 131072, 16, 4, 8, 2
+    g = torch.Generator(device="cuda").manual_seed(0)
+    K = torch.randn(S, Hkv, 128, device="cuda", generator=g).to(torch.bfloat16)
+    V = torch.randn(S, Hkv, 128, device="cuda", generator=g).to(torch.bfloat16)
+    cuts = [S * r // world for r in range(world + 1)]
+    rows = [b - a for a, b in zip(cuts[:-1], cuts[1:])]
+    Ks = [K[a:b].contiguous() for a, b in zip(cuts[:-1], cuts[1:])]
+    Vs = [V[a:b].contiguous() for a, b in zip(cuts[:-1], cuts[1:])]
+    rank = world - 1
+    Q = torch.randn(rows[rank], Hq, 128, device="cuda", generator=g).to(torch.bfloat16)
+    O, lse = B.gc_attention_allgather_kv(Q, [k.data_ptr() for k in Ks], [v.data_ptr() for v in Vs], rows,
+                                         rank, Hkv, None, True, 0, None, hps)
+    torch.cuda.synchronize()
+    r = np.random.default_rng(1)
+    n = rows[rank]
+    sample = sorted({0, 1, 63, 64, 127, 128, n // 2, n - 129, n - 128, n - 1} | {int(x) for x in r.integers(0, n, 6)})
+    Kf, Vf = f64(K), f64(V)
+    for i in sample:
+        o_ref, l_ref = A.attention(f64(Q[i:i + 1]), Kf, Vf, cuts[rank] + i, None, True, 0)
+        o = O[i].float().cpu().numpy().reshape(1, -1)
+        assert elem_excess(o, o_ref.reshape(1, -1), a=4e-3, b=1.2e-2) <= 1.0, i
+        assert np.abs(lse[:, i].cpu().numpy() - l_ref[:, 0]).max() <= 2e-3, i
+
+
 def _free_port():
     s = socket.socket()
     s.bind(("127.0.0.1", 0))

@@ -279,6 +279,38 @@ def test_token_loss_kernels(B, agg, T, R):
     assert near.sum() < 0.001 * T + 2
 
 
+@pytest.mark.parametrize("agg", [O.AGG_TOKEN_MEAN, O.AGG_SEQ_MEAN])
+@pytest.mark.parametrize("R", [5003, 190001])
+def test_token_loss_kernel_more_tiles_than_blocks(B, agg, R):
+    """T = 3,000,017 tokens = 2930 tiles of 1024 on a persistent grid of at most 1184 blocks: every
+    block walks several tiles (double-buffered slices of cu_seqlens / advantages / weights, count
+    batches striding the grid) -- the regime of bench.py's 2^26-token stand-ins, which no smaller
+    case reaches.  Long responses (~600 tokens) and short ones (~16 tokens), both aggregations,
+    element-wise against the oracle."""
+    T = 3_000_017
+    logp, old, ref, adv, mask, y, cu = _loss_inputs(T, R, 41 + R)
+    out5, g = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu),
+                                   dev(adv), 0.2, 0.2, 0.04, agg, grad_loss=1.0)
+    scored = (mask != 0) & (y >= 0)
+    res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg)
+    g_ref = O.grpo_loss_grad_logp(logp, old, ref, scored, adv, cu, 0.2, 0.2, 0.04, agg, 1.0)
+    o = out5.cpu().numpy().astype(np.float64)
+    assert o[4] == res["n_scored"]
+    assert abs(o[0] - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+    assert abs(o[1] - res["pg_loss"]) <= 1e-5 * max(abs(res["pg_loss"]), 1e-2)
+    assert abs(o[2] - res["kl_mean"]) <= 1e-5 * max(abs(res["kl_mean"]), 1e-3)
+    assert abs(o[3] - res["clip_frac"]) <= 5e-6
+    gg = g.cpu().numpy().astype(np.float64)
+    rho = np.exp(logp.astype(np.float64) - old)
+    near = (np.abs(rho - 1.2) < 1e-5) | (np.abs(rho - 0.8) < 1e-5)
+    assert np.all(gg[~scored] == 0.0)
+    assert np.allclose(gg[~near], g_ref[~near], rtol=2e-5, atol=2e-6 * np.abs(g_ref).max())
+    assert near.sum() < 0.001 * T
+    out5b, gb = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu),
+                                     dev(adv), 0.2, 0.2, 0.04, agg, grad_loss=1.0)
+    assert torch.equal(out5, out5b) and torch.equal(g, gb)              # reruns bit-identical
+
+
 def test_token_loss_edge_cases(B):
     logp, old, ref, adv, mask, y, cu = _loss_inputs(1000, 10, 5)
     # sum m = 0 -> loss 0, g 0 (reading 12)

@@ -223,8 +223,8 @@ def test_advantages_and_filter(B, unbiased, drop):
 
 
 # ------------------------------------------------------------------ a1 row selection
-@pytest.mark.parametrize("T,p", [(1, 1.0), (5000, 0.75), (70001, 0.3), (4096, 0.0)])
-def test_compaction_bit_exact(B, T, p):
+@pytest.mark.parametrize("T,p", [(1, 1.0), (5000, 0.75), (70001, 0.3), (4096, 0.0), (2_500_003, 0.6)])
+def test_compaction_bit_exact(B, T, p):      # the last case: more count blocks than one scan pass takes
     r = np.random.default_rng(T)
     mask = (r.random(T) < p).astype(np.uint8)
     y = r.integers(0, 100, T).astype(np.int32)

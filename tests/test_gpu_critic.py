@@ -37,8 +37,10 @@ def layout(R, seed, max_len=300):
 
 
 @pytest.mark.parametrize("dtype", [torch.bfloat16, torch.float32])
-@pytest.mark.parametrize("T,D", [(1, 8), (333, 264), (2000, 4096), (70, 2048 + 8)])
+@pytest.mark.parametrize("T,D", [(1, 8), (333, 264), (2000, 4096), (70, 2048 + 8), (40013, 520)])
 def test_value_head_fwd_bwd(B, dtype, T, D):
+    # (40013 rows: more 64-row tiles than the backward's 296 persistent row blocks -- each block walks
+    # several tiles, as on bench.py's 524288-row stand-in)
     g = torch.Generator(device="cuda").manual_seed(T + D)
     H = torch.randn(T, D, device="cuda", generator=g).to(dtype)
     w = (torch.randn(D, device="cuda", generator=g) / D ** 0.5).to(dtype)
@@ -78,7 +80,7 @@ def test_gae_matches_oracle(B, R, seed, use_mask):
             assert np.all(adv.cpu().numpy()[m == 0] == 0)
 
 
-@pytest.mark.parametrize("T", [1, 1000, 70001])
+@pytest.mark.parametrize("T", [1, 1000, 70001, 3_000_001])   # the last: count blocks stride the grid
 def test_value_loss_and_grad(B, T):
     r = np.random.default_rng(T)
     v = r.normal(size=T).astype(np.float32)

@@ -204,6 +204,15 @@ def check_full(B, b, n_random=64, seed=0):
                        w.clip_lo, w.clip_hi, w.beta, dH=b.dH, dW=b.dW)
     assert torch.equal(f2["logp"], logp) and torch.equal(f2["entropy"], ent)
     assert torch.equal(b.dH, dH1) and torch.equal(b.dW, dW1)
+    # bf16 dW output at full size (fp32 staging in the workspace, cast kernel striding its grid):
+    # equals the fp32 dW rounded once, bit for bit
+    if w.V * w.D <= 6e8:
+        _, dW16 = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f2["logp"],
+                                     f2["lse"], w.clip_lo, w.clip_hi, w.beta, dH=b.dH,
+                                     dW_dtype=torch.bfloat16)
+        assert dW16.dtype == torch.bfloat16 and torch.equal(dW16, dW1.to(torch.bfloat16))
+        assert torch.equal(b.dH, dH1)
+        del dW16
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 4])

@@ -439,6 +439,35 @@ def test_bf16_small_forward_backward(B, name):
     check_against_oracle(b, got2, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
 
 
+def test_bf16_forward_more_rows_than_the_helper_grids(B):
+    """T = 400,001 rows: the 1-D helper kernels of the forward (target / lse gathers, zero-fill of
+    unscored outputs) run capped grids of 1184 x 256 threads and stride them beyond 303,104 rows --
+    past every config (cfg3: 281,898).  Random mask, negative targets; sampled rows against the
+    oracle, unscored rows exactly zero, and the masked call equals the dense call on scored rows."""
+    T, D, V = 400_001, 64, 512 + 24
+    H, W = I.make_hw(T, D, V, "bf16", 21, "cuda")
+    y = I.sample_targets(H, W, 1.0, 21)
+    mask_np = I.random_mask(T, 0.7, 21)
+    y_np = y.cpu().numpy().copy()
+    y_np[::13] = -100
+    y = torch.from_numpy(y_np).cuda()
+    mask = torch.from_numpy(mask_np).cuda()
+    lp, en, ls = B.gc_token_logprobs(H, W, y, mask, 1.0)
+    lp_d, en_d, ls_d = B.gc_token_logprobs(H, W, y, None, 1.0)
+    torch.cuda.synchronize()
+    scored = (mask_np != 0) & (y_np >= 0)
+    st = torch.from_numpy(scored).cuda()
+    assert float(lp[~st].abs().sum()) == 0.0 and float(en[~st].abs().sum()) == 0.0 and float(ls[~st].abs().sum()) == 0.0
+    assert torch.equal(lp[st], lp_d[st]) and torch.equal(en[st], en_d[st]) and torch.equal(ls[st], ls_d[st])
+    r = np.random.default_rng(3)
+    S = np.array(sorted({0, 1, 255, 256, 303_103, 303_104, 303_105, T - 2, T - 1} | {int(x) for x in r.integers(0, T, 300)}))
+    St = torch.from_numpy(S).cuda()
+    lp_o, en_o, ls_o = O.token_logprobs(to_f64(H[St]), to_f64(W), y_np[S], mask_np[S], 1.0)
+    assert np.abs(lp[St].cpu().numpy() - lp_o).max() <= TOL_LOGP_BF16
+    assert np.abs(ls[St].cpu().numpy() - ls_o).max() <= TOL_LOGP_BF16
+    assert np.abs(en[St].cpu().numpy() - en_o).max() <= 2 * TOL_LOGP_BF16
+
+
 def test_bf16_random_mask_negative_targets_chunks_accumulate(B):
     w = I.reduced(I.CONFIGS[2], D=256, V=2048 + 8, groups=4, group_size=4, seq_len=40, prompt_len=0,
                   old_std=0.3)

@@ -673,6 +673,29 @@ def test_bf16_production_schedules_vs_oracle(B, V, masked):
         assert torch.equal(again[k], got[k]), k
 
 
+@pytest.mark.parametrize("masked", [True, False])
+def test_bf16_backward_more_chunks_than_one_counter_zeroing(B, masked):
+    """34 backward chunks of 256 rows: a chunk takes 34 of the 1024 zeroed counter words (two tile
+    tickets + the dH progress ring), so the chunk loop re-zeroes the area after 30 chunks -- a
+    regime real batches reach beyond 30 x 8192 scored tokens.  Against the dense oracle, and
+    bit-identical on a rerun."""
+    if masked:
+        w = I.reduced(I.CONFIGS[2], D=128, V=520, groups=2, group_size=4, seq_len=1420, prompt_len=355,
+                      old_std=0.3)
+    else:
+        w = I.reduced(I.CONFIGS[2], D=128, V=520, groups=1, group_size=4, seq_len=2125, prompt_len=0,
+                      old_std=0.3)
+    b = make_batch(w, seed=5, device="cuda")
+    assert b.scored_np.sum() > 30 * 256
+    adv_ref, _ = O.grpo_advantages(b.rewards_np, b.lay.group_offsets, 1e-6)
+    ref = oracle_run(b, adv_ref)
+    got = run_gpu(B, b, chunk_tokens=256)
+    check_against_oracle(b, got, ref, TOL_LOGP_BF16, TOL_GRAD_BF16)
+    again = run_gpu(B, b, chunk_tokens=256)
+    for k in ("dH", "dW"):
+        assert torch.equal(again[k], got[k]), k
+
+
 def test_token_loss_offset_mask_and_garbage_at_unscored_positions(B):
     """A mask view at a 4-byte (not 8-byte) offset must take the whole-tile fast path safely, and
     inf / NaN stored at unscored positions of logp / old / ref must not reach the loss (only scored

@@ -284,6 +284,38 @@ int gc_value_head_bwd(const void* H, int64_t ldH, int dtype, const void* w, cons
                       int64_t T, int64_t D, void* dH, int64_t lddH, float* dw, float* dbias,
                       void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- gc_value_loss without a workspace, for callers that have no way to get device memory.
+ * Every other entry point takes its scratch from a `workspace` the caller allocated.  Some callers
+ * cannot do that: a hook or plug-in that runs inside another framework's training step and is
+ * handed only the tensors it reads and writes; a process whose memory pool has claimed the whole
+ * HBM at start-up, so that a later cudaMalloc simply fails; a step loop that must not stall,
+ * because cudaMalloc / cudaFree synchronise the whole device.  For them this call computes exactly
+ * what gc_value_loss computes (same kernels, bit-identical out3 and g; PPO value loss, PAPER.md:96,
+ * PAPER.md:102-103, formulas above) with the scratch -- the scored / clipped counters and one fp64
+ * partial sum per 1024-token tile -- in a fixed array that is part of the library image.
+ *   Arguments: as gc_value_loss, minus workspace / workspace_bytes.  values, old_values, returns
+ *   [T] f32, mask [T] uint8 nullable, out3 [3] f32, g [T] f32 nullable: DEVICE pointers, owned by
+ *   the caller.  Work is enqueued on `cuda_stream`; no synchronisation.
+ *   Limit: T <= GC_VALUE_LOSS_STATIC_MAX_T (4,194,304 tokens).  A larger T returns GC_ERR_SHAPE
+ *   before anything is launched -- use gc_value_loss with a workspace instead.  Other errors as
+ *   gc_value_loss (GC_ERR_NULL, GC_ERR_ARG for clip_v < 0, GC_ERR_CUDA).
+ *   Cost: the array is 33,024 bytes of device memory on every GPU that loads the library, held
+ *   from load until the process exits, whether or not this call is ever made.
+ *   No allocation: the call makes no cudaMalloc / cudaFree / cudaMallocAsync and calls no library
+ *   routine that allocates; it issues one cudaMemsetAsync of 24 bytes and two kernel launches.
+ *   First call on a device: looks up the array's address on the CURRENT device
+ *   (cudaGetSymbolAddress; the address is per device and is cached per device).  Make that first
+ *   call with the right device current and before starting any stream capture on it.
+ *   Sharing: there is ONE array per device and every call uses it.  It keeps the previous call's
+ *   contents; the call clears what has to start at zero (the counters), the partials are rewritten
+ *   before they are read.  Two calls that can overlap on the GPU (different streams, no event
+ *   between them; or two host threads on two streams) RACE on the array and give wrong results:
+ *   keep all calls on one stream per device, or order them with events. */
+#define GC_VALUE_LOSS_STATIC_MAX_T 4194304
+int gc_value_loss_static_scratch(const float* values, const float* old_values, const float* returns,
+                                 const uint8_t* mask, int64_t T, float clip_v, float grad_loss,
+                                 float* out3, float* g, void* cuda_stream);
+
 /* ---- verdict-token scoring for a generative reward model.
  * PAPER.md:144 (sec 3.2): "Generative rewarding using standard next-token prediction, represents
  * solution correctness using the LLM's probability distribution over tokens ... the verification

@@ -31,6 +31,7 @@ EXPORTS = [
     "gc_step_host_workspace_bytes", "gc_grpo_step_host",
     "gc_attention_workspace_bytes", "gc_attention_allgather_kv",
     "gc_value_head_fwd", "gc_gae", "gc_critic_workspace_bytes", "gc_value_loss", "gc_value_head_bwd",
+    "gc_value_loss_static_scratch",
 ]
 
 
@@ -102,6 +103,7 @@ def _load() -> C.CDLL:
     lib.gc_critic_workspace_bytes.argtypes = [i64, i64]
     lib.gc_value_loss.argtypes = [vp, vp, vp, vp, i64, f32, f32, vp, vp, vp, sz, vp]
     lib.gc_value_head_bwd.argtypes = [vp, i64, ci, vp, vp, i64, i64, vp, i64, vp, vp, vp, sz, vp]
+    lib.gc_value_loss_static_scratch.argtypes = [vp, vp, vp, vp, i64, f32, f32, vp, vp, vp]
     lib.gc_kernel_timing_begin.argtypes = []
     lib.gc_kernel_timing_end.argtypes = [C.POINTER(f32), C.POINTER(i32)]
     for name in EXPORTS:
@@ -474,6 +476,32 @@ def gc_value_loss(values, old_values, returns, mask=None, clip_v=0.2, grad_loss=
     _check(_lib.gc_value_loss(_ptr(values), _ptr(old_values), _ptr(returns), _ptr(mask), T,
                               float(clip_v), float(grad_loss), _ptr(out3), _ptr(g), _ptr(ws),
                               ws.numel(), _stream()))
+    return out3, g
+
+
+GC_VALUE_LOSS_STATIC_MAX_T = 4194304     # include/gcore.h
+
+
+def gc_value_loss_static_scratch(values, old_values, returns, mask=None, clip_v=0.2, grad_loss=1.0,
+                                 *, out3, g=None):
+    """gc_value_loss for a caller that cannot allocate device memory (a hook inside someone else's
+    training step that owns only its inputs and outputs, a process whose pool already holds all of
+    HBM, a loop that must not hit cudaMalloc's device-wide sync): the scratch is a fixed 33 KB array
+    inside libgcore.so, so there is no workspace and this wrapper allocates nothing either -- the
+    caller passes the outputs: out3 [3] float32 (loss, clip_frac, n_scored) and optionally g [T]
+    float32.  T <= GC_VALUE_LOSS_STATIC_MAX_T, else GcoreError.  One array per device, shared by
+    all calls: calls that may overlap on the GPU race; keep them on one stream.  The first call on
+    a device looks up the array's address: make it with that device current, outside any capture."""
+    T = values.numel()
+    if T > GC_VALUE_LOSS_STATIC_MAX_T:
+        raise GcoreError(f"gc_value_loss_static_scratch: T = {T} exceeds the fixed scratch array's "
+                         f"limit GC_VALUE_LOSS_STATIC_MAX_T = {GC_VALUE_LOSS_STATIC_MAX_T}; use "
+                         "gc_value_loss (caller workspace) for larger batches")
+    assert out3.is_cuda and out3.dtype == torch.float32 and out3.numel() == 3 and out3.is_contiguous()
+    assert g is None or (g.is_cuda and g.dtype == torch.float32 and g.numel() == T and g.is_contiguous())
+    _check(_lib.gc_value_loss_static_scratch(_ptr(values), _ptr(old_values), _ptr(returns), _ptr(mask),
+                                             T, float(clip_v), float(grad_loss), _ptr(out3), _ptr(g),
+                                             _stream()))
     return out3, g
 
 

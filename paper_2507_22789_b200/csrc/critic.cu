@@ -5,6 +5,7 @@
 // sec 11 and written out in oracle/critic_oracle.py.  All kernels here are HBM-bound (the value
 // head reads H once, its backward reads H once and writes dH once) or latency-bound (GAE, loss).
 #include "common.cuh"
+#include <atomic>
 
 namespace gc {
 
@@ -367,3 +368,68 @@ int launch_value_bwd(const void* H, int64_t ldH, bool bf16, const void* w, const
 }
 
 }  // namespace gc
+
+// ---- gc_value_loss_static_scratch: the value loss for callers that cannot obtain device memory --
+// The scratch of the value loss (the counters block and one fp64 partial per 1024-token tile) lives
+// in this file-scope device array instead of a caller workspace.  It is part of the library image:
+// every GPU that loads libgcore.so carries these 33,024 bytes from module load until the process
+// exits.  Its size fixes the largest T the entry point takes (GC_VALUE_LOSS_STATIC_MAX_T).
+namespace gc {
+namespace {
+
+constexpr int64_t kStaticMaxT = GC_VALUE_LOSS_STATIC_MAX_T;
+constexpr size_t kStaticScratchBytes = 256 + (size_t)(kStaticMaxT / kVTile) * sizeof(VPartial);
+static_assert(kStaticMaxT % kVTile == 0, "the limit is a whole number of tiles");
+static_assert(sizeof(VCounters) <= 256, "counters fit the first 256-byte granule");
+
+static __device__ __align__(256) unsigned char g_vloss_static_scratch[kStaticScratchBytes];
+
+// On the host `g_vloss_static_scratch` is only a handle for the runtime's symbol table: it is NOT
+// the array's device address and must never be handed to a kernel.  The real address differs per
+// device (each device has its own copy of the array) and comes from cudaGetSymbolAddress, asked
+// once per device with that device current and remembered here.
+constexpr int kStaticMaxDevices = 64;
+std::atomic<void*> g_vloss_static_addr[kStaticMaxDevices];
+
+int static_scratch_address(void** out) {
+  int dev = 0;
+  GC_CUDA_TRY(cudaGetDevice(&dev));
+  const bool cached = dev >= 0 && dev < kStaticMaxDevices;
+  void* p = cached ? g_vloss_static_addr[dev].load(std::memory_order_acquire) : nullptr;
+  if (!p) {
+    GC_CUDA_TRY(cudaGetSymbolAddress(&p, g_vloss_static_scratch));   // device `dev` is current
+    if (!p) return GC_ERR_CUDA;
+    // two host threads may both get here on a first call: they publish the same address
+    if (cached) g_vloss_static_addr[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return GC_OK;
+}
+
+}  // namespace
+}  // namespace gc
+
+extern "C" int gc_value_loss_static_scratch(const float* values, const float* old_values,
+                                            const float* returns, const uint8_t* mask, int64_t T,
+                                            float clip_v, float grad_loss, float* out3, float* g,
+                                            void* cuda_stream) {
+  using namespace gc;
+  if (T < 0) return GC_ERR_SHAPE;
+  if (T > kStaticMaxT) return GC_ERR_SHAPE;        // the fixed array has no room for more tiles
+  if (!(clip_v >= 0.f)) return GC_ERR_ARG;
+  if (!out3) return GC_ERR_NULL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (T == 0) {
+    GC_CUDA_TRY(cudaMemsetAsync(out3, 0, 3 * sizeof(float), st));
+    return GC_OK;
+  }
+  if (!values || !old_values || !returns) return GC_ERR_NULL;
+  void* scratch = nullptr;
+  GC_TRY(static_scratch_address(&scratch));
+  // Same two kernels and the same carving as gc_value_loss, so the results are bit-identical to it.
+  // The array still holds the previous call's counters and partials: launch_value_loss clears the
+  // counters block on the stream (a memset node, no allocation) and every partial that is read is
+  // written first by its own block in this launch.
+  return launch_value_loss(values, old_values, returns, mask, T, clip_v, grad_loss, out3, g, scratch,
+                           st);
+}

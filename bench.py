@@ -7,12 +7,15 @@
 
 A step is one pass of the hot path over one synthetic micro-batch of the named workload.
 BASELINE.json:metric ("scored tokens/sec (fwd and fwd+bwd) on 1 B200") names no configuration, so
-the headline workload is configs[1] (the tier rule's default: forward-only scoring of 16384 tokens,
-hidden 3584, vocab 152064, bf16).  The same JSON line carries, under "workloads", the metric's
-fwd+bwd half on configs[2] (8B-class training micro-batch), configs[4] (large-vocab stress) and
-configs[3] (long-tail dynamic-sampling step), each with one roofline object per contraction kind
-and -- for configs[2] -- the end-to-end figure from host buffers.  Backward-capable workloads run
-advantages -> loss forward -> loss backward per step.  One JSON line on stdout.
+the headline workload is the largest single-GPU configuration that has a host-buffer entry point:
+configs[4] (hidden 8192, vocab 256000, 8192 tokens, forward + backward, dW in fp32).  The ONE JSON
+line on stdout is compact (< 4 KB, asserted): the headline's value, ONE roofline object (the
+dominant contraction), e2e (gc_grpo_step_host from pinned host buffers), cpu_baseline, and under
+"workloads" a few scalars for each other configuration: configs[1] (the metric's forward half),
+configs[2], configs[3] (dynamic-sampling step).  Everything else -- every roofline object of every
+workload, the HBM-bound kernels, the cuBLAS/torch library baseline, the attention workload -- goes
+to stderr as one JSON object per line ({"detail": name, ...}), never into the stdout line.
+Backward-capable workloads run advantages -> loss forward -> loss backward per step.
 
 N > 1: one rank per GPU under torch.distributed.run (bench.py re-executes itself under it when
 --gpus N > 1 and WORLD_SIZE is not set).  Whole groups are sharded across ranks -- every rank
@@ -45,6 +48,8 @@ sys.path.insert(0, ROOT)
 from paper_2507_22789_b200 import inputs as I  # noqa: E402
 
 WORKLOADS = {"cfg0": 0, "cfg1": 1, "cfg2": 2, "cfg3": 3, "cfg4": 4}
+HEADLINE = "cfg4"        # the largest single-GPU configuration with a host-buffer entry point
+MAX_LINE_BYTES = 4096    # the driver parses the stdout line; round 2's 22 KB line was unreadable
 KIND_NAMES = {"fwd_stats": "a2+a3 forward H.W^T + online log-softmax epilogue",
               "recompute_ds": "a10 recompute H.W^T + dS epilogue",
               "dh": "a11 dH = dS.W", "dw": "a12 dW += dS^T.H"}
@@ -350,7 +355,7 @@ def run_reference(args, w):
     if rank != 0:
         return
     from threadpoolctl import threadpool_info
-    n_tok = 64 if w.D * w.V > 1e8 else 1 << 30
+    n_tok = 32 if w.D * w.V > 1e9 else 64 if w.D * w.V > 1e8 else 1 << 30
     step, T, ws = _oracle_sample(w, n_tok)
     for _ in range(args.warmup):
         step()
@@ -447,6 +452,67 @@ def dominant(roofs, step_ms):
     return d
 
 
+ROOFLINE_KEYS = ("workload", "kind", "kernel", "bound", "achieved", "peak", "unit", "frac",
+                 "peak_kind", "frac_of_burst", "frac_of_sustained", "flops_per_launch", "launch_ms",
+                 "launches_per_step", "traffic", "contraction_share_of_step")
+
+
+def detail(name, **kw):
+    """Everything that is not the headline goes to stderr, one JSON object per line."""
+    print(json.dumps(dict({"detail": name}, **kw)), file=sys.stderr, flush=True)
+
+
+def workload_scalars(m):
+    """A measured workload (measure_workload) reduced to the scalars the stdout line carries."""
+    roofs = m.get("rooflines") or []
+    worst = min(roofs, key=lambda r: r["frac_of_burst"]) if roofs else None
+    out = {"ms_per_step": round(m["ms_per_step"], 4), "value": round(m["value"], 1),
+           "step_tflops": round(m["step_tflops"], 1),
+           "worst_kind": worst["kind"] if worst else None,
+           "worst_frac_of_burst": round(worst["frac_of_burst"], 4) if worst else None,
+           "e2e_ms": round(m["e2e"]["ms_per_step"], 4) if m.get("e2e") else None}
+    if m.get("library_baseline"):
+        out["cublas_gemm_only_ms"] = round(m["library_baseline"]["cublas_gemm_only"]["ms_per_step"], 4)
+    return out
+
+
+def assemble_line(w, *, value, ms_per_step, T, world, steps, warmup, exchange, clocks, gpu_launches,
+                  roofs, step_ms, e2e, cpu, workloads, extra_config=None, dp_info=None):
+    """The ONE stdout line: headline scalars, one roofline object, e2e, cpu_baseline, and scalars per
+    other workload.  No lists of objects, nothing twice (tests/test_bench_line.py feeds it fakes)."""
+    dom = dominant(roofs, step_ms)
+    out = {
+        "metric": metric_name(w), "value": value, "unit": "scored tokens/s",
+        "n_gpus": world, "steps": steps, "warmup": warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic",
+        "config": dict(workload_config(w, T, world, exchange), **(extra_config or {})),
+        "clocks": clocks, "gpu_launches": gpu_launches,
+        "roofline": {k: dom[k] for k in ROOFLINE_KEYS if k in dom} if dom.get("achieved") else dom,
+    }
+    if e2e:
+        out["e2e"] = {k: e2e[k] for k in ("value", "unit", "ms_per_step", "h2d_bytes_per_step",
+                                          "d2h_bytes_per_step") if k in e2e}
+    if cpu:
+        out["cpu_baseline"] = {"value": cpu["value"], "unit": cpu["unit"], "cores": cpu["cores"],
+                               "kind": cpu["kind"], "sample": cpu["sample"]}
+        if cpu.get("one_thread"):
+            out["cpu_baseline"]["one_thread"] = {"value": cpu["one_thread"]["value"], "cores": 1}
+    if workloads:
+        out["workloads"] = workloads
+    if dp_info:
+        out["dp_exchange"] = {k: v for k, v in dp_info.items() if not isinstance(v, (dict, list))}
+        if isinstance(dp_info.get("other_arm"), dict):
+            out["dp_exchange"]["other_arm_ms_per_step"] = dp_info["other_arm"].get("ms_per_step")
+    return out
+
+
+def emit(out) -> str:
+    line = json.dumps(out)
+    assert len(line) < MAX_LINE_BYTES, f"stdout line is {len(line)} bytes (limit {MAX_LINE_BYTES})"
+    return line
+
+
 def hbm_kernels(B, device, peaks):
     """The HBM-bound kernels of the path (rows a1, a8, a9) on scaled-up stand-ins -- at the configs'
     own sizes they move < 6 MB (loss) / 0.4 GB (gather) and are launch-latency bound (DESIGN.md
@@ -478,14 +544,16 @@ def hbm_kernels(B, device, peaks):
         adv = torch.randn(R, device=device, generator=g)
         for agg, agg_name in ((0, "token_mean"), (1, "seq_mean")):
             ms = timeit(lambda: B.gc_grpo_token_loss(logp, old, ref, y, mask, cu, adv, agg=agg))
-            # per token: logp, old, ref, target (4 B each) + mask (1 B) read, g (4 B) written, and
-            # the count phase that fixes the normaliser re-reads target + mask (5 B) = 26 B; per
-            # response: cu_seqlens + advantage (8 B), and for seq-mean the per-response count
-            # (zeroed, added to, read twice: 16 B) and cu_seqlens once more (4 B)
-            per_tok = 26.0 + (8.0 + (20.0 if agg else 0.0)) / seqlen
+            # ALGORITHMIC bytes: per token logp, old, ref, target
+            # (4 B each) + mask (1 B) read, g (4 B) written = 21 B; per response cu_seqlens +
+            # advantage (8 B), and for seq-mean the per-response count written and read (8 B).
+            # What the kernel really moves is more (its count phase re-reads target + mask:
+            # 25.8 B/token in profiles/r2_loss_*): that is `traffic_bytes_per_token`, not the numerator
+            per_tok = 21.0 + (8.0 + (8.0 if agg else 0.0)) / seqlen
             gbs = per_tok * T / ms / 1e6
             out[f"loss_and_grad_{agg_name}_{seqlen}_token_responses"] = {
-                "tokens": T, "responses": R, "bytes_per_token": per_tok, "ms": ms, "gbs": gbs,
+                "tokens": T, "responses": R, "bytes_per_token": per_tok,
+                "traffic_bytes_per_token": 25.8, "ms": ms, "gbs": gbs,
                 "frac": gbs / peaks["hbm"], "launches": 1}
     del logp, old, ref, y, mask, cu, adv
     T2, D = 1 << 19, 4096
@@ -606,7 +674,7 @@ def e2e_train_step(B, b: DeviceBatch, steps, warmup):
 # --------------------------------------------------------------------------------------------
 # one workload, measured
 # --------------------------------------------------------------------------------------------
-def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
+def measure_workload(B, w, device, steps, warmup, peaks, with_e2e, with_library=False):
     b = DeviceBatch(w, seed=0, device=device)
     step, launches = make_step(B, b)
     total_ms, per, kinds = timed_region(step, steps, warmup, False, B)
@@ -621,8 +689,10 @@ def measure_workload(B, w, device, steps, warmup, peaks, with_e2e):
     if hasattr(b, "T_kept"):
         out["tokens_kept_after_group_filter"] = b.T_kept
         out["flow"] = "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"
-    if with_e2e and w.backward and not w.drop_constant_groups:
-        out["e2e"] = e2e_train_step(B, b, steps, 3)     # as many timed steps as the device figure
+    if with_e2e and not w.drop_constant_groups:         # as many timed steps as the device figure
+        out["e2e"] = e2e_train_step(B, b, steps, 3) if w.backward else e2e_forward(B, b, steps, 3)
+    if with_library:
+        out["library_baseline"] = library_baseline(b)
     del b, step
     gc.collect()
     torch.cuda.empty_cache()
@@ -752,7 +822,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default="cfg1", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default=HEADLINE, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the cpu_baseline / e2e / other-workload extras (rank 0, N=1 only)")
@@ -816,6 +886,7 @@ def main():
     total_ms, per, kinds = timed_region(step, args.steps, args.warmup, dist_on, B)
     clocks = sampler.stop() if rank == 0 else None
     tokens = b.n_scored
+    T_rank = b.T
     total_ms_max, tokens_all = dp.reduce_step_stats(total_ms, tokens)   # max time, summed tokens
     ms_per_step = total_ms_max / args.steps
     value = tokens_all / (ms_per_step * 1e-3)
@@ -839,44 +910,39 @@ def main():
     if rank == 0:
         step_ms = float(np.mean(per))
         roofs = rooflines(w, tokens, args.steps, kinds, total_ms, peaks)
-        out = {
-            "metric": metric_name(w), "value": value, "unit": "scored tokens/s",
-            "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16" if w.dtype == "bf16" else "f32",
-            "data": "synthetic",
-            "config": dict(workload_config(w, b.T, world, exchange),
-                           **({"tokens_kept_after_group_filter": b.T_kept,
-                               "flow": "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"}
-                              if hasattr(b, "T_kept") else {})),
-            "clocks": clocks, "gpu_launches": launches * args.steps,
-            "roofline": dominant(roofs, step_ms), "rooflines": roofs,
-        }
+        extra_cfg = ({"tokens_kept_after_group_filter": b.T_kept,
+                      "flow": "advantages(drop) -> gc_balance_plan -> gathers -> fwd+bwd"}
+                     if hasattr(b, "T_kept") else {})
+        e2e = cpu = None
+        others = {}
+        detail("rooflines", workload=w.name, rooflines=roofs)
         if dp_info:
-            out["dp_exchange"] = dp_info
+            detail("dp_exchange", **dp_info)
         if world == 1 and not args.no_extras:
             half = max(3, args.steps // 2)
             if w.dtype == "bf16" and not w.drop_constant_groups:
-                out["e2e"] = e2e_train_step(B, b, half, 3) if w.backward else e2e_forward(B, b, half, 3)
-            out["cpu_baseline"] = cpu_baseline(w, 256 if w.D * w.V > 1e8 else 1 << 30)
-            if args.workload == "cfg1":
-                out["library_baseline"] = library_baseline(b)
+                e2e = e2e_train_step(B, b, half, 3) if w.backward else e2e_forward(B, b, half, 3)
+            cpu = cpu_baseline(w, 64 if w.D * w.V > 1e9 else 256 if w.D * w.V > 1e8 else 1 << 30)
+            detail("cpu_baseline", **cpu)
+            if args.workload == HEADLINE:
                 del b, step
                 gc.collect()
                 torch.cuda.empty_cache()
-                out["hbm_kernels"] = hbm_kernels(B, device, peaks)
+                # the metric's forward half, the 8B-class step and the dynamic-sampling step
+                for name, k, wu in (("cfg1", args.steps, 3), ("cfg2", max(4, args.steps // 4), 3),
+                                    ("cfg3", 3, 3)):
+                    m = measure_workload(B, I.CONFIGS[WORKLOADS[name]], device, k, wu, peaks,
+                                         with_e2e=(name != "cfg3"), with_library=(name == "cfg1"))
+                    detail("workload", **m)
+                    others[name] = workload_scalars(m)
+                detail("hbm_kernels", **hbm_kernels(B, device, peaks))
                 torch.cuda.empty_cache()
-                # the metric's fwd+bwd half and the largest configs, each with its rooflines
-                wl = {}
-                for name, k, wu in (("cfg2", max(4, args.steps // 4), 3), ("cfg4", 4, 3), ("cfg3", 3, 3)):
-                    wl[name] = measure_workload(B, I.CONFIGS[WORKLOADS[name]], device, k, wu, peaks,
-                                                with_e2e=(name == "cfg2"))
-                    out["rooflines"] = out["rooflines"] + wl[name]["rooflines"]
-                wl["attention_allgather_kv"] = attention_workload(B, device, peaks)
-                out["workloads"] = wl
-                out["fwd_bwd"] = {k: wl["cfg2"][k] for k in ("workload", "value", "unit", "ms_per_step",
-                                                             "step_tflops", "gpu_launches_per_step")}
-        print(json.dumps(out))
+                detail("attention_allgather_kv", **attention_workload(B, device, peaks))
+        out = assemble_line(w, value=value, ms_per_step=ms_per_step, T=T_rank, world=world,
+                            steps=args.steps, warmup=args.warmup, exchange=exchange, clocks=clocks,
+                            gpu_launches=launches * args.steps, roofs=roofs, step_ms=step_ms, e2e=e2e,
+                            cpu=cpu, workloads=others, extra_config=extra_cfg, dp_info=dp_info)
+        print(emit(out))
     if dist_on:
         import torch.distributed as dist
         dist.barrier()

@@ -107,13 +107,21 @@ int gc_token_logprobs(const void* H, int64_t ldH, const void* W, int64_t ldW, in
 /* Same computation with the per-step inputs and outputs in HOST memory (pinned for async
  * copies): H_host [T,D] dense, targets_host, mask_host (nullable) are copied to the device,
  * logp_host / entropy_host (nullable) are copied back, staged in `workspace`
- * (gc_workspace_bytes(GC_OP_LOGPROBS,...) + gc_host_staging_bytes(T, D, dtype)).  W is model state
+ * (gc_logprobs_host_workspace_bytes(T, D, V, dtype): the staging buffers,
+ * gc_host_staging_bytes(T, D, dtype), plus the LARGEST gc_workspace_bytes(GC_OP_LOGPROBS, rows, ...)
+ * over the bands below -- each band is planned on its own and a band can need more scratch than the
+ * whole batch would).  W is model state
  * and stays a device pointer.  The H copy overlaps the contraction: H travels band by band (the
  * forward schedule's M bands, after a short first band) on a library-owned side stream and each
  * band is scored on `cuda_stream` as soon as it has arrived; the results are complete in stream
  * order on `cuda_stream`.  Process-global state (iv): one side stream and a few events per device,
  * created on first use.  Used for the end-to-end measurement. */
 size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype);
+size_t gc_logprobs_host_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype);
+/* The bands the *_host entry points cut H into: writes starts_host[0..n] (HOST array of 65 entries),
+ * band b = rows [starts_host[b], starts_host[b+1]), and returns n (<= 64; 0 on invalid arguments).
+ * Host-only arithmetic; exposed so that the workspace sizing above can be checked without a GPU. */
+int32_t gc_host_band_plan(int64_t T, int64_t D, int64_t V, int dtype, int64_t* starts_host);
 int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int dtype,
                            const int32_t* targets_host, const uint8_t* mask_host,
                            int64_t T, int64_t D, int64_t V, float temperature,

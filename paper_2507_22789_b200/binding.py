@@ -21,7 +21,8 @@ GC_OP_LOGPROBS, GC_OP_LOSS_FWD, GC_OP_LOSS_BWD = 0, 1, 2
 
 EXPORTS = [
     "gc_status_string", "gc_last_cuda_error", "gc_version", "gc_workspace_bytes", "gc_token_logprobs",
-    "gc_host_staging_bytes", "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
+    "gc_host_staging_bytes", "gc_logprobs_host_workspace_bytes", "gc_host_band_plan",
+    "gc_token_logprobs_host", "gc_grpo_advantages", "gc_grpo_loss_fwd",
     "gc_grpo_loss_bwd", "gc_validate_targets", "gc_compact_rows", "gc_grpo_token_loss",
     "gc_debug_gemm_bf16", "gc_kernel_timing_begin", "gc_kernel_timing_end",
     "gc_balance_workspace_bytes", "gc_balance_plan", "gc_gather_rows", "gc_gather_1d",
@@ -59,6 +60,9 @@ def _load() -> C.CDLL:
     lib.gc_token_logprobs.argtypes = head + [vp, vp, vp, vp, sz, vp]
     lib.gc_host_staging_bytes.restype = sz
     lib.gc_host_staging_bytes.argtypes = [i64, i64, ci]
+    lib.gc_logprobs_host_workspace_bytes.restype = sz
+    lib.gc_logprobs_host_workspace_bytes.argtypes = [i64, i64, i64, ci]
+    lib.gc_host_band_plan.argtypes = [i64, i64, i64, ci, C.POINTER(i64)]
     lib.gc_token_logprobs_host.argtypes = [vp, vp, i64, ci, vp, vp, i64, i64, i64, f32, vp, vp,
                                            vp, sz, vp]
     lib.gc_step_host_workspace_bytes.restype = sz
@@ -109,6 +113,7 @@ def _load() -> C.CDLL:
     for name in EXPORTS:
         fn = getattr(lib, name)
         if name not in ("gc_status_string", "gc_last_cuda_error", "gc_workspace_bytes", "gc_host_staging_bytes",
+                        "gc_logprobs_host_workspace_bytes",
                         "gc_balance_workspace_bytes", "gc_multi_workspace_bytes",
                         "gc_loss_workspace_bytes", "gc_bwd_workspace_bytes",
                         "gc_step_host_workspace_bytes", "gc_attention_workspace_bytes",
@@ -207,7 +212,7 @@ def gc_token_logprobs_host(H_host, W, targets_host, mask_host=None, temperature=
     assert not H_host.is_cuda and H_host.is_contiguous() and W.is_cuda
     if logp_host is None:
         logp_host = torch.empty(T, dtype=torch.float32).pin_memory()
-    nb = workspace_bytes(GC_OP_LOGPROBS, T, D, V, dt) + int(_lib.gc_host_staging_bytes(T, D, dt))
+    nb = int(_lib.gc_logprobs_host_workspace_bytes(T, D, V, dt))
     ws = workspace(nb, W.device)
     _check(_lib.gc_token_logprobs_host(_ptr(H_host), _ptr(W), W.stride(0), dt, _ptr(targets_host),
                                        _ptr(mask_host), T, D, V, float(temperature),

@@ -59,6 +59,21 @@ int plan_bands(int64_t T, int64_t D, int64_t V, int dtype, int64_t* start /*[65]
   return n;     // bands are [start[i], start[i+1])
 }
 
+// Workspace the band-by-band forward needs: every band is its own gc_token_logprobs call and is
+// planned on its own (vocab splits, partial statistics), and that plan is not monotonic in the row
+// count -- a band can need more than the whole batch would.  So: the largest query over the bands.
+size_t banded_inner_bytes(int64_t T, int64_t D, int64_t V, int dtype) {
+  size_t need = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
+  if (T <= 0) return need;
+  int64_t start[65];
+  const int nb = plan_bands(T, D, V, dtype, start);
+  for (int b = 0; b < nb; ++b) {
+    const size_t n = gc_workspace_bytes(GC_OP_LOGPROBS, start[b + 1] - start[b], D, V, dtype, 0);
+    if (n > need) need = n;
+  }
+  return need;
+}
+
 struct Staging {
   void* H; int32_t* y; uint8_t* m; float* logp; float* ent; float* lse;
 };
@@ -107,6 +122,18 @@ int banded_forward(HostCtx* cx, const void* H_host, const void* W, int64_t ldW, 
 
 extern "C" {
 
+int32_t gc_host_band_plan(int64_t T, int64_t D, int64_t V, int dtype, int64_t* starts_host) {
+  if (T <= 0 || D <= 0 || V <= 0 || !starts_host) return 0;
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return 0;
+  return plan_bands(T, D, V, dtype, starts_host);
+}
+
+size_t gc_logprobs_host_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype) {
+  if (T < 0 || D <= 0 || V <= 0) return 0;
+  if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return 0;
+  return align_up(banded_inner_bytes(T, D, V, dtype), 256) + gc_host_staging_bytes(T, D, dtype);
+}
+
 size_t gc_host_staging_bytes(int64_t T, int64_t D, int dtype) {
   if (T < 0 || D <= 0) return 0;
   Carver c(nullptr);
@@ -122,8 +149,8 @@ int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int d
   if (dtype != GC_F32 && dtype != GC_BF16 && dtype != GC_BF16_SIMT) return GC_ERR_DTYPE;
   if (T == 0) return GC_OK;
   if (!H_host || !targets_host || !logp_host || !W) return GC_ERR_NULL;
-  const size_t inner = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
-  if (!workspace || workspace_bytes < inner + gc_host_staging_bytes(T, D, dtype))
+  const size_t inner = banded_inner_bytes(T, D, V, dtype);
+  if (!workspace || workspace_bytes < align_up(inner, 256) + gc_host_staging_bytes(T, D, dtype))
     return GC_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -153,7 +180,11 @@ struct StepWs {
 };
 size_t carve_step(Carver& c, int64_t T, int64_t D, int64_t V, int dtype, int32_t R, int32_t G,
                   int dW_dtype, StepWs* w) {
-  const size_t fb = align_up(gc_workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dtype, 0), 256);
+  // forward workspace: the banded forward's need (max over bands), then the loss scratch -- the
+  // part of the GC_OP_LOSS_FWD query that lies behind its GC_OP_LOGPROBS part
+  const size_t lp = align_up(gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0), 256);
+  const size_t lf = align_up(gc_workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dtype, 0), 256);
+  const size_t fb = align_up(banded_inner_bytes(T, D, V, dtype), 256) + (lf > lp ? lf - lp : 0) + 256;
   const size_t bb = align_up(gc_bwd_workspace_bytes(T, D, V, dtype, 0, dW_dtype), 256);
   void* f = c.take<uint8_t>(fb);
   void* b = c.take<uint8_t>(bb);
@@ -218,7 +249,7 @@ int gc_grpo_step_host(const void* H_host, const void* W, int64_t ldW, int dtype,
     GC_CUDA_TRY(cudaMemcpyAsync(w.ref_lp, ref_logp_host, (size_t)T * 4, cudaMemcpyHostToDevice, cx->cs));
   GC_CUDA_TRY(cudaEventRecord(cx->ev[1], cx->cs));
   // forward, band by band as H arrives (logp, lse kept for the backward)
-  const size_t fwd_inner = gc_workspace_bytes(GC_OP_LOGPROBS, T, D, V, dtype, 0);
+  const size_t fwd_inner = banded_inner_bytes(T, D, V, dtype);
   GC_TRY(banded_forward(cx, H_host, W, ldW, dtype, targets_host, mask_host, T, D, V, temperature,
                         w.sg, false, true, w.fwd, fwd_inner, st, 2));
   GC_CUDA_TRY(cudaStreamWaitEvent(st, cx->ev[1], 0));

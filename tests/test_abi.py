@@ -86,3 +86,31 @@ def test_host_checkable_errors_before_any_launch(lib):
     assert lib.gc_grpo_advantages(None, None, 0, 1e-6, 0, 0, None, None, None) == 0   # empty batch
     assert lib.gc_token_logprobs(None, 8, one, 8, B.GC_F32, None, None, 0, 8, 8, 1.0, None, None,
                                  None, None, 0, None) == 0                             # T = 0
+
+
+def test_host_entry_workspace_covers_every_band(lib):
+    """The *_host entry points score H band by band, one gc_token_logprobs call per band, each with
+    its own plan; the plan is not monotonic in the row count, so the carved forward workspace has to
+    be the largest query over the bands (it used to be the full-T query: GC_ERR_WORKSPACE at e.g.
+    T=6144, D=4096, V=50304).  Host arithmetic only."""
+    import itertools
+    from paper_2507_22789_b200 import binding as B
+    starts = (ctypes.c_int64 * 65)()
+    saw_band_above_full = False
+    Ts = [1, 300, 513, 5000, 6144, 9000, 16384, 26000, 40000]
+    for T, D, V in itertools.product(Ts, (1024, 3584, 4096), (32000, 50304, 152064)):
+        n = lib.gc_host_band_plan(T, D, V, B.GC_BF16, starts)
+        assert 1 <= n <= 64 and starts[0] == 0 and starts[n] == T
+        assert all(starts[b] < starts[b + 1] for b in range(n))
+        carved = lib.gc_logprobs_host_workspace_bytes(T, D, V, B.GC_BF16) \
+            - lib.gc_host_staging_bytes(T, D, B.GC_BF16)
+        full = B.workspace_bytes(B.GC_OP_LOGPROBS, T, D, V, B.GC_BF16)
+        assert carved >= full
+        for b in range(n):
+            need = B.workspace_bytes(B.GC_OP_LOGPROBS, starts[b + 1] - starts[b], D, V, B.GC_BF16)
+            assert need <= carved, (T, D, V, b)
+            saw_band_above_full |= need > full
+        step = lib.gc_step_host_workspace_bytes(T, D, V, B.GC_BF16, 8, 2, B.GC_F32)
+        assert step >= carved + lib.gc_bwd_workspace_bytes(T, D, V, B.GC_BF16, 0, B.GC_F32)
+    assert saw_band_above_full                  # the sweep does reach the non-monotonic case
+    assert lib.gc_host_band_plan(0, 8, 8, B.GC_BF16, starts) == 0

@@ -839,3 +839,27 @@ def test_host_entry_points_banded_copy_and_training_step(B):
         assert rel_fro(dW.float().cpu().numpy(), ref["dW"]) <= TOL_GRAD_BF16 + (3e-3 if dw_dtype == torch.bfloat16 else 0)
         assert np.allclose(o[:4], dev_run["out5"].cpu().numpy()[:4], rtol=2e-5, atol=1e-7)
         assert elem_excess(dH_h.float().numpy(), ref["dH"], **ELEM_BF16) <= 1.0
+
+
+def test_host_logprobs_at_a_shape_whose_band_needs_more_scratch_than_the_batch(B):
+    """T=6144, D=4096, V=50304: the second H band (5376 rows) plans more vocab splits than the whole
+    batch does, so its partial statistics need more workspace than the full-T query returns; the
+    host entry point used to answer GC_ERR_WORKSPACE here.  Host path against the device path
+    (itself oracle-checked) and against the oracle on sampled rows."""
+    T, D, V = 6144, 4096, 50304
+    g = torch.Generator(device="cuda").manual_seed(77)
+    H = (torch.randn(T, D, device="cuda", generator=g)).to(torch.bfloat16)
+    W = (torch.randn(V, D, device="cuda", generator=g) / D ** 0.5).to(torch.bfloat16)
+    y = torch.randint(0, V, (T,), device="cuda", generator=g, dtype=torch.int32)
+    lp_d, en_d, _ = B.gc_token_logprobs(H, W, y, None, 1.0)
+    lph = torch.empty(T, dtype=torch.float32).pin_memory()
+    enh = torch.empty(T, dtype=torch.float32).pin_memory()
+    B.gc_token_logprobs_host(H.cpu().pin_memory(), W, y.cpu().pin_memory(), None, 1.0,
+                             logp_host=lph, entropy_host=enh)
+    torch.cuda.synchronize()
+    assert np.abs(lph.numpy() - lp_d.cpu().numpy()).max() <= TOL_LOGP_BF16
+    assert np.abs(enh.numpy() - en_d.cpu().numpy()).max() <= 2 * TOL_LOGP_BF16
+    rows = [0, 511, 512, 767, 768, 5000, T - 1]          # both bands, their edges
+    lp_o, en_o, _ = O.token_logprobs(to_f64(H[rows]), to_f64(W), y[rows].cpu().numpy(), None, 1.0)
+    assert np.abs(lph.numpy()[rows] - lp_o).max() <= TOL_LOGP_BF16
+    assert np.abs(enh.numpy()[rows] - en_o).max() <= 2 * TOL_LOGP_BF16

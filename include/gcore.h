@@ -23,13 +23,16 @@
  *     (idempotent: host threads may race on a first launch); (ii) the measurement aid
  *     gc_kernel_timing_* (mutex-guarded, off by default); (iii) the tile counter and progress ring of
  *     gc_debug_gemm_bf16 (a test entry point; do not run two of them concurrently); (iv) one side
- *     stream and a few events per device for the *_host entry points.  None of it changes results.  Calls on different streams need different workspaces.
+ *     stream and a few events per device for the *_host and attention entry points (their enqueue
+ *     is serialised per device by a mutex, so host threads may call them on different streams);
+ *     (v) the 33 KB scratch array of gc_value_loss_static_scratch.  None of it changes results.  Calls on different streams need different workspaces.
  *   - The tensor-core kernels are persistent (one CTA per SM) and the CTA pairs of the dH launch
  *     pace one another through progress counters: they are meant to own the GPU.  A kernel of
  *     another stream or process that holds some SMs only delays them, but every wait inside the
- *     kernels carries a watchdog of 2^32 cycles (~2-3 s) that turns a wait longer than that --
+ *     kernels carries a watchdog of 2^36 cycles (35-60 s) that turns a wait longer than that --
  *     a protocol bug, or SMs withheld for that long -- into a launch failure (GC_ERR_CUDA at the
- *     next call that checks) instead of a hang.
+ *     next call that checks) instead of a hang.  The bound is that long because the cycle counter
+ *     keeps running while the context is time-sliced out or slowed by a profiler / sanitizer.
  *   - Matrices are row-major; ld* are row strides in ELEMENTS.  For GC_BF16: D % 8 == 0,
  *     ld % 8 == 0, base pointers 16-byte aligned (TMA).
  *   - A token is SCORED iff (mask == NULL or mask[t] != 0) and targets[t] >= 0.  targets[t] >= V

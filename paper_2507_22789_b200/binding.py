@@ -169,6 +169,38 @@ def workspace(nbytes: int, device, slot: str = "") -> torch.Tensor:
     return buf
 
 
+_fwd_generation: dict = {}
+
+
+class FwdState:
+    """What gc_grpo_loss_fwd leaves for the backward: its workspace (row list, compacted targets and
+    H) plus the facts needed to tell whether it still describes the same batch.  The workspace is
+    cached per (device, stream), so the NEXT forward on that stream -- another micro-batch --
+    overwrites it; a backward handed a state that is no longer the latest one of its slot, or one made
+    for other shapes / another mask, silently falls back to recomputing the row selection (the C call
+    gets fwd_state = NULL), which is always correct."""
+
+    def __init__(self, ws, key, sig):
+        self.ws, self.key, self.sig = ws, key, sig
+        self.gen = _fwd_generation[key] = _fwd_generation.get(key, 0) + 1
+
+    def usable_for(self, sig) -> bool:
+        return (_fwd_generation.get(self.key) == self.gen and self.sig == sig
+                and _ws_cache.get(self.key) is self.ws)
+
+
+def _state_sig(H, targets, mask, T, D, V, dt):
+    return (H.data_ptr(), targets.data_ptr(), None if mask is None else mask.data_ptr(), T, D, V, dt)
+
+
+def _state_ptr(fwd_state, sig):
+    if fwd_state is None:
+        return None
+    if isinstance(fwd_state, FwdState):
+        return _ptr(fwd_state.ws) if fwd_state.usable_for(sig) else None
+    return _ptr(fwd_state)          # a raw workspace tensor: the caller vouches for it
+
+
 def workspace_bytes(op: int, T: int, D: int, V: int, dtype: int, chunk_tokens: int = 0) -> int:
     return int(_lib.gc_workspace_bytes(op, T, D, V, dtype, chunk_tokens))
 
@@ -285,7 +317,9 @@ def gc_grpo_loss_fwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp
                                  ws.numel(), _stream()))
     # state: the forward's workspace (row list, compacted H), valid until the next forward on this
     # stream; pass it to gc_grpo_loss_bwd(fwd_state=...) to skip the row selection there
-    return dict(out5=out5, logp=logp, entropy=ent, lse=lse, state=ws)
+    key = (str(dev), int(torch.cuda.current_stream(dev).cuda_stream), "fwd")
+    state = FwdState(ws, key, _state_sig(H, targets, mask, T, D, V, dt))
+    return dict(out5=out5, logp=logp, entropy=ent, lse=lse, state=state)
 
 
 def gc_grpo_loss_bwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp, ref_logp,
@@ -308,8 +342,9 @@ def gc_grpo_loss_bwd(H, W, targets, mask, temperature, cu_seqlens, adv, old_logp
                                                     clip_hi, beta, agg),
                                  _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH),
                                  dH.stride(0) if T > 0 else D, _ptr(dW), dW.stride(0), dwt,
-                                 int(accumulate_dW), int(chunk_tokens), _ptr(fwd_state), _ptr(ws),
-                                 ws.numel(), _stream()))
+                                 int(accumulate_dW), int(chunk_tokens),
+                                 _state_ptr(fwd_state, _state_sig(H, targets, mask, T, D, V, dt)),
+                                 _ptr(ws), ws.numel(), _stream()))
     return dH, dW
 
 
@@ -543,7 +578,8 @@ def gc_grpo_loss_bwd_reduce_scatter(H, W, targets, mask, temperature, cu_seqlens
         *args, *_loss_args(cu_seqlens, adv, old_logp, ref_logp, clip_lo, clip_hi, beta, agg),
         _ptr(logp), _ptr(lse), float(grad_loss), _ptr(dH), dH.stride(0) if T > 0 else D, arr, world,
         int(shard_rows), int(ld_shard if ld_shard is not None else D), int(chunk_tokens),
-        _ptr(fwd_state), _ptr(ws), ws.numel(), _stream()))
+        _state_ptr(fwd_state, _state_sig(H, targets, mask, T, D, V, dt)), _ptr(ws), ws.numel(),
+        _stream()))
     return dH
 
 

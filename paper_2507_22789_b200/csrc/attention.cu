@@ -456,7 +456,10 @@ k_attn_fwd(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUte
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-struct SideCtx { cudaStream_t cs = nullptr; cudaEvent_t ev[6] = {}; bool ok = false; bool attr = false; };
+struct SideCtx {
+  cudaStream_t cs = nullptr; cudaEvent_t ev[6] = {}; bool ok = false; bool attr = false;
+  std::mutex use;      // held for the whole enqueue of one call: the events are re-recorded per call
+};
 std::mutex g_mu;
 SideCtx g_ctx[64];
 
@@ -544,6 +547,9 @@ int gc_attention_allgather_kv(const void* Q, const void* const* K_shards_host,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   attn::SideCtx* cx = nullptr;
   GC_TRY(attn::get_side(&cx));
+  // one enqueue at a time per device: two host threads on two streams would otherwise re-record
+  // each other's events between a record and the wait that is meant to see it
+  std::lock_guard<std::mutex> use_lock(cx->use);
   Carver c(workspace);
   attn::Ws w;
   attn::carve(c, S_local, S, hs, &w);

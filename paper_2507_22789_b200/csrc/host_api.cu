@@ -20,6 +20,7 @@ struct HostCtx {
   cudaStream_t cs = nullptr;
   cudaEvent_t ev[kHostEvents] = {};
   bool ok = false;
+  std::mutex use;      // held for the whole enqueue of one *_host call (events are re-recorded per call)
 };
 std::mutex g_ctx_mu;
 HostCtx g_ctx[64];
@@ -156,6 +157,9 @@ int gc_token_logprobs_host(const void* H_host, const void* W, int64_t ldW, int d
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   HostCtx* cx = nullptr;
   GC_TRY(get_ctx(&cx));
+  // one enqueue at a time per device: a second host thread on another stream would re-record the
+  // events between this call's record and the wait that is meant to see it
+  std::lock_guard<std::mutex> use_lock(cx->use);
   Carver c(static_cast<char*>(workspace) + align_up(inner, 256));
   Staging sg;
   carve_staging(c, T, D, dtype, &sg);
@@ -235,6 +239,9 @@ int gc_grpo_step_host(const void* H_host, const void* W, int64_t ldW, int dtype,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   HostCtx* cx = nullptr;
   GC_TRY(get_ctx(&cx));
+  // one enqueue at a time per device: a second host thread on another stream would re-record the
+  // events between this call's record and the wait that is meant to see it
+  std::lock_guard<std::mutex> use_lock(cx->use);
   Carver c(workspace);
   StepWs w;
   carve_step(c, T, D, V, dtype, R, G, dW_dtype, &w);

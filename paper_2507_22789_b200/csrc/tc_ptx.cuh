@@ -80,11 +80,16 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
       : "memory");
   return ok != 0;
 }
+// Watchdog of every blocking wait: 2^36 SM cycles (35-60 s at 1.2-1.97 GHz).  clock64 keeps counting
+// while the context is time-sliced out (two processes sharing the GPU) and under ncu replay or
+// compute-sanitizer slow-downs, so the bound is far above anything a correct run can wait; it only
+// turns a real protocol deadlock into a launch failure instead of a hung GPU.
+constexpr long long kWatchdogCycles = 1ll << 36;
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait_cluster(bar, parity)) return;
   const long long t0 = clock64();
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if (clock64() - t0 > (1ll << 32)) __trap();
+    if (clock64() - t0 > kWatchdogCycles) __trap();
   }
 }
 __device__ __forceinline__ void st_shared_cluster_u32(uint32_t cluster_addr, uint32_t v) {
@@ -103,7 +108,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
   while (!mbar_try_wait(bar, parity)) {
-    if (clock64() - t0 > (1ll << 32)) __trap();
+    if (clock64() - t0 > kWatchdogCycles) __trap();
   }
 }
 
@@ -121,7 +126,7 @@ __device__ __forceinline__ void wait_counter_ge(const uint32_t* p, uint32_t targ
   if ((int32_t)(ld_relaxed_gpu(p) - target) >= 0) return;
   const long long t0 = clock64();
   while ((int32_t)(ld_relaxed_gpu(p) - target) < 0) {
-    if (clock64() - t0 > (1ll << 32)) __trap();
+    if (clock64() - t0 > kWatchdogCycles) __trap();
   }
 }
 

@@ -11,7 +11,7 @@ import torch
 
 import oracle as O
 from paper_2507_22789_b200 import inputs as I
-from bench import detie_old
+from tests.harness import detie_old
 
 
 def to_f64(t: torch.Tensor) -> np.ndarray:

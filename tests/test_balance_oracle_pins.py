@@ -3,6 +3,7 @@ dynamic-sampling repack + workload-balancing step (DESIGN
 import os
 
 import numpy as np
+import pytest
 
 from oracle import balance_oracle as BO
 
@@ -97,3 +98,19 @@ def test_sorting_reduces_wasted_compute():
     w_unsorted = BO.wasted_fraction(L, unsorted, 1, 0)
     assert w_sorted < 0.10 < w_unsorted
     assert BO.wasted_fraction(L, sorted_plan["buckets"], 0, 1) < BO.wasted_fraction(L, unsorted, 0, 1)
+
+
+def test_wasted_fraction_hand_values():
+    """By hand.  Lengths [1, 3] in one bucket, linear cost: both samples cost the maximum 3, so
+    padded = 2*3 = 6 against 1 + 3 = 4 of useful work: waste = 1 - 4/6 = 1/3.  Quadratic cost:
+    w = [1, 9], padded 18, useful 10: 1 - 10/18 = 4/9.  Two buckets [[0], [1]]: nothing is padded,
+    waste 0.  Mixed model w = 2 L + L^2 = [3, 15]: 1 - 18/30 = 2/5.  Three samples [2, 2, 5] in
+    buckets [[0, 1], [2]]: padded 2*2 + 5 = 9 = useful: 0; in one bucket: 1 - 9/15 = 2/5."""
+    L = [1, 3]
+    assert BO.wasted_fraction(L, [[0, 1]], 1, 0) == pytest.approx(1 / 3, abs=1e-15)
+    assert BO.wasted_fraction(L, [[0, 1]], 0, 1) == pytest.approx(4 / 9, abs=1e-15)
+    assert BO.wasted_fraction(L, [[0], [1]], 1, 0) == 0.0
+    assert BO.wasted_fraction(L, [[0, 1]], 2, 1) == pytest.approx(2 / 5, abs=1e-15)
+    assert BO.wasted_fraction([2, 2, 5], [[0, 1], [2]], 1, 0) == 0.0
+    assert BO.wasted_fraction([2, 2, 5], [[0, 1, 2]], 1, 0) == pytest.approx(2 / 5, abs=1e-15)
+    assert BO.wasted_fraction([], [], 1, 0) == 0.0

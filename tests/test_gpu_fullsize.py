@@ -15,7 +15,7 @@ The oracle cannot materialise [T,V] here, so (SURVEY.md sec 8(c) "parity protoco
         that hold at any size: every column sum of dW is 0, <dH,H> = <dW,W>, unscored dH rows are
         0, and the north_star invariant loss = -sum(mA)/sum(m) when policy = old and beta = 0.
 No oracle input or expected value is produced by the CUDA path except where (iv)/(v) say so
-(GPU logp / lse fed to the oracle's formulas): old/ref are synthesised by bench.synth_policy_logp
+(GPU logp / lse fed to the oracle's formulas): old/ref are synthesised by tests.harness.synth_policy_logp
 (plain torch, harness side).
 """
 import gc
@@ -27,7 +27,7 @@ import torch
 
 import oracle as O
 from paper_2507_22789_b200 import inputs as I
-from bench import DeviceBatch
+from tests.harness import DeviceBatch
 from tests.helpers import ELEM_BF16, elem_excess
 
 pytestmark = pytest.mark.gpu

@@ -280,6 +280,50 @@ def test_token_loss_kernels(B, agg, T, R):
 
 
 @pytest.mark.parametrize("agg", [O.AGG_TOKEN_MEAN, O.AGG_SEQ_MEAN])
+def test_token_loss_exact_ties_take_the_unclipped_branch(B, agg):
+    """The clip decision AT a tie (reading 7: s1 <= s2 counts as unclipped), on inputs
+    where fp32 and fp64 provably agree, so nothing has to be excluded:
+      * clip_lo = clip_hi = 0 and logp == old bit for bit: rho = exp(0) = 1 exactly, which is both
+        clip bounds at once -- a kernel that treated rho >= 1 + clip_hi (or <= 1 - clip_lo) as
+        clipped would zero these gradients and count them in clip_frac;
+      * advantage 0 with rho far outside the band: s1 = s2 = 0 whatever rho is -- a kernel that
+        decided from rho alone would count these as clipped;
+      * rho = exp(+-0.5), far from the bound, both signs of the advantage: the ordinary branches."""
+    R, L = 12, 100
+    T = R * L
+    cu = np.arange(0, T + 1, L, dtype=np.int32)
+    adv = np.array([1.0, -1.0, 0.0, 0.5, -2.0, 0.0] * 2, dtype=np.float32)
+    r = np.random.default_rng(5)
+    logp = (-(1 + r.integers(0, 24, T)) / 8.0).astype(np.float32)        # multiples of 1/8: exact
+    shift = r.choice(np.array([0.0, 0.0, 0.5, -0.5], dtype=np.float32), T)
+    old = (logp - shift).astype(np.float32)                              # exact in fp32
+    assert np.all(old.astype(np.float64) == logp.astype(np.float64) - shift)
+    ref = (logp + r.choice(np.array([0.0, 0.25, -0.25], dtype=np.float32), T)).astype(np.float32)
+    mask = np.ones(T, np.uint8)
+    y = np.zeros(T, np.int32)
+    scored = np.ones(T, bool)
+    out5, g = B.gc_grpo_token_loss(dev(logp), dev(old), dev(ref), dev(y), dev(mask), dev(cu),
+                                   dev(adv), 0.0, 0.0, 0.04, agg, grad_loss=1.0)
+    res = O.grpo_loss(logp, old, ref, scored, adv, cu, 0.0, 0.0, 0.04, agg)
+    g_ref = O.grpo_loss_grad_logp(logp, old, ref, scored, adv, cu, 0.0, 0.0, 0.04, agg, 1.0)
+    adv_t = np.repeat(adv, L)
+    tie_rho1 = (shift == 0) & (adv_t != 0)
+    tie_adv0 = (adv_t == 0) & (shift != 0)
+    assert tie_rho1.sum() > 100 and tie_adv0.sum() > 50
+    # the oracle itself: ties are unclipped, so exactly the off-band tokens with A != 0 whose
+    # min() picks the clipped term are counted
+    n_clipped = int((((shift > 0) & (adv_t > 0)) | ((shift < 0) & (adv_t < 0))).sum())
+    assert abs(res["clip_frac"] - n_clipped / T) < 1e-12
+    o = out5.cpu().numpy().astype(np.float64)
+    assert o[4] == T
+    assert abs(o[3] - res["clip_frac"]) <= 1e-6                 # no near-tie allowance here
+    assert abs(o[0] - res["loss"]) <= 1e-5 * max(abs(res["loss"]), 1e-2)
+    gg = g.cpu().numpy().astype(np.float64)
+    assert np.allclose(gg, g_ref, rtol=2e-5, atol=2e-6 * np.abs(g_ref).max())     # every token
+    assert np.all(np.abs(gg[tie_rho1]) > 0.1 * np.abs(g_ref[tie_rho1]))           # not zeroed
+
+
+@pytest.mark.parametrize("agg", [O.AGG_TOKEN_MEAN, O.AGG_SEQ_MEAN])
 @pytest.mark.parametrize("R", [5003, 190001])
 def test_token_loss_kernel_more_tiles_than_blocks(B, agg, R):
     """T = 3,000,017 tokens = 2930 tiles of 1024 on a persistent grid of at most 1184 blocks: every
@@ -800,6 +844,37 @@ def test_bf16_dw_output_and_forward_state_reuse(B):
     _, d32 = B.gc_grpo_loss_bwd(*a0)
     _, d16 = B.gc_grpo_loss_bwd(*a0, dW_dtype=torch.bfloat16)
     assert torch.equal(d16, d32.to(torch.bfloat16))
+
+
+def test_stale_forward_state_is_not_used(B):
+    """Micro-batches A then B forwarded on the same stream share the cached forward workspace, so
+    after B's forward A's state describes B's row selection.  The binding must notice (generation
+    counter + shapes + input pointers) and let A's backward recompute its own selection: results
+    bit-identical to a backward without any state; B's state, the latest, is still used."""
+    def batch(seed, seq_len):
+        w = I.reduced(I.CONFIGS[2], D=256, V=2048, groups=2, group_size=4, seq_len=seq_len,
+                      prompt_len=40, old_std=0.3)
+        b = make_batch(w, seed=seed, device="cuda")
+        adv, _ = B.gc_grpo_advantages(b.rewards_t, b.go_t)
+        return w, b, adv
+    wa, a, adv_a = batch(21, 160)
+    wb, bb, adv_b = batch(22, 130)
+    fa = B.gc_grpo_loss_fwd(a.H, a.W, a.y, a.mask_t, wa.tau, a.cu_t, adv_a, a.old_t, a.ref_t)
+    args_a = (a.H, a.W, a.y, a.mask_t, wa.tau, a.cu_t, adv_a, a.old_t, a.ref_t, fa["logp"], fa["lse"])
+    sig_a = B._state_sig(a.H, a.y, a.mask_t, a.T, wa.D, wa.V, B.GC_BF16)
+    assert fa["state"].usable_for(sig_a)
+    dH_ref, dW_ref = B.gc_grpo_loss_bwd(*args_a)                          # no state: recomputes
+    fb = B.gc_grpo_loss_fwd(bb.H, bb.W, bb.y, bb.mask_t, wb.tau, bb.cu_t, adv_b, bb.old_t, bb.ref_t)
+    assert not fa["state"].usable_for(sig_a)                              # overwritten by B
+    dH_a, dW_a = B.gc_grpo_loss_bwd(*args_a, fwd_state=fa["state"])       # stale: must be ignored
+    assert torch.equal(dH_a, dH_ref) and torch.equal(dW_a, dW_ref)
+    # a state offered for other inputs than it was made for is ignored as well
+    assert not fb["state"].usable_for(sig_a)
+    args_b = (bb.H, bb.W, bb.y, bb.mask_t, wb.tau, bb.cu_t, adv_b, bb.old_t, bb.ref_t, fb["logp"],
+              fb["lse"])
+    dH_b0, dW_b0 = B.gc_grpo_loss_bwd(*args_b)
+    dH_b1, dW_b1 = B.gc_grpo_loss_bwd(*args_b, fwd_state=fb["state"])     # latest: used
+    assert torch.equal(dH_b0, dH_b1) and torch.equal(dW_b0, dW_b1)
 
 
 def test_host_entry_points_banded_copy_and_training_step(B):

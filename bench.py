@@ -491,13 +491,14 @@ def hbm_kernels(B, device, peaks):
             # ALGORITHMIC bytes: per token logp, old, ref, target
             # (4 B each) + mask (1 B) read, g (4 B) written = 21 B; per response cu_seqlens +
             # advantage (8 B), and for seq-mean the per-response count written and read (8 B).
-            # What the kernel really moves is more (its count phase re-reads target + mask:
-            # 25.8 B/token in profiles/r2_loss_*): that is `traffic_bytes_per_token`, not the numerator
+            # What the kernel really moves (ncu, profiles/r3_loss.md: 20.9-22.9 B/token since phase 1
+            # keeps the scored flags in a bitmap; 25.8 in round 2) is `traffic_bytes_per_token`
             per_tok = 21.0 + (8.0 + (8.0 if agg else 0.0)) / seqlen
             gbs = per_tok * T / ms / 1e6
             out[f"loss_and_grad_{agg_name}_{seqlen}_token_responses"] = {
                 "tokens": T, "responses": R, "bytes_per_token": per_tok,
-                "traffic_bytes_per_token": 25.8, "ms": ms, "gbs": gbs,
+                "traffic_bytes_per_token": {(0, 1024): 20.94, (1, 1024): 20.96, (0, 16): 21.69,
+                                            (1, 16): 22.92}[(agg, seqlen)], "ms": ms, "gbs": gbs,
                 "frac": gbs / peaks["hbm"], "launches": 1}
     del logp, old, ref, y, mask, cu, adv
     T2, D = 1 << 19, 4096

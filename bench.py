@@ -801,6 +801,10 @@ def main():
     if dist_on:
         import torch.distributed as dist
         if args.dist_backend == "nccl":
+            # let NCCL print its INIT lines (ranks, transports, NVLS) so that the driver can count
+            # the ranks that really joined; a caller's own setting wins
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
             dist.init_process_group("nccl", device_id=device)
         else:
             dist.init_process_group("gloo")
@@ -887,11 +891,15 @@ def main():
                             steps=args.steps, warmup=args.warmup, exchange=exchange, clocks=clocks,
                             gpu_launches=launches * args.steps, roofs=roofs, step_ms=step_ms, e2e=e2e,
                             cpu=cpu, workloads=others, extra_config=extra_cfg, dp_info=dp_info)
-        print(emit(out))
+        final_line = emit(out)
     if dist_on:
         import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()
+    if rank == 0:
+        # after the teardown, so that NCCL's own INFO lines (N > 1) never follow the JSON line
+        sys.stdout.flush()
+        print(final_line, flush=True)
 
 
 if __name__ == "__main__":

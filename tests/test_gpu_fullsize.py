@@ -266,3 +266,41 @@ def test_full_size_config3_dynamic_sampling(B):
     assert np.allclose(lossA[:4], lossB[:4], rtol=1e-5, atol=1e-7)
     # a row's result does not depend on the packing (only the split-V combine order differs)
     assert float((fA["logp"] - fB["logp"][ti]).abs().max()) <= 2e-5
+
+
+def test_host_training_step_at_full_size_matches_the_device_path(B):
+    """gc_grpo_step_host at the size bench.py's e2e figure times (configs[2]: 32768 x 4096 x 128256,
+    75 % scored): every output against the device-resident calls on the same inputs, which
+    check_full verifies against the oracle.  The host path scores H band by band (its own split-V
+    plans), so log-probs agree to rounding, not bit for bit; out5, dH [T, D] and dW [V, D] follow."""
+    w = I.CONFIGS[2]
+    dev = torch.device("cuda", 0)
+    b = DeviceBatch(w, seed=0, device=dev)
+    adv, _ = B.gc_grpo_advantages(b.rewards, b.go, 1e-6, False, False)
+    f = B.gc_grpo_loss_fwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, w.clip_lo, w.clip_hi,
+                           w.beta)
+    dH_d, dW_d = B.gc_grpo_loss_bwd(b.H, b.W, b.y, b.mask, w.tau, b.cu, adv, b.old, b.ref, f["logp"],
+                                    f["lse"], w.clip_lo, w.clip_hi, w.beta, fwd_state=f["state"])
+    pin = lambda t: t.cpu().pin_memory()
+    dW_h = torch.full((w.V, w.D), 3.0, dtype=torch.float32, device=dev)
+    lp_h = torch.empty(b.T, dtype=torch.float32).pin_memory()
+    out5_h, dH_h = B.gc_grpo_step_host(pin(b.H), b.W, pin(b.y), pin(b.mask), w.tau, pin(b.cu),
+                                       pin(b.rewards), pin(b.go), pin(b.old), pin(b.ref), dW_h,
+                                       clip_lo=w.clip_lo, clip_hi=w.clip_hi, beta=w.beta,
+                                       logp_host=lp_h)
+    torch.cuda.synchronize()
+    o_h, o_d = out5_h.numpy().astype(np.float64), f["out5"].cpu().numpy().astype(np.float64)
+    assert o_h[4] == o_d[4] == b.n_scored
+    assert np.allclose(o_h[:3], o_d[:3], rtol=2e-5, atol=1e-7)
+    assert abs(o_h[3] - o_d[3]) <= 4.0 / b.n_scored          # a few near-ties of the clip bound
+    assert float((lp_h.to(dev) - f["logp"]).abs().max()) <= 2e-5
+    scored = (b.lay.mask != 0) & (b.y.cpu().numpy() >= 0)
+    dH_h = dH_h.to(dev).float()
+    assert float(dH_h[torch.from_numpy(~scored).to(dev)].abs().sum()) == 0.0
+    rel = lambda a, r: float((a - r).norm() / r.norm())
+    # near-ties of the clip bound (not de-tied against the banded log-probs) may flip a branch on a
+    # handful of rows; everything else differs by bf16 rounding of dH at most
+    row_err = (dH_h - dH_d.float()).norm(dim=1) / dH_d.float().norm(dim=1).clamp_min(1e-30)
+    assert int((row_err > 1e-2).sum()) <= 4
+    assert rel(dH_h, dH_d.float()) <= 2e-3
+    assert rel(dW_h, dW_d) <= 2e-3

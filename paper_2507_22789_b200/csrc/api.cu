@@ -6,13 +6,6 @@
 using namespace gc;
 
 namespace gc {
-// host_api.cu: an event to record right after the LAST chunk's dH launch of the calling thread's
-// next backward (dH is complete from there on; the step-from-host entry point starts its
-// device -> host copy of dH under the last dW contraction).  Consumed by that backward.
-static thread_local cudaEvent_t t_dh_done_event = nullptr;
-static thread_local int64_t t_dh_done_rows = 0;     // scored rows of the batch (chunks past them are empty)
-void set_bwd_dh_done_event(cudaEvent_t e, int64_t n_scored) { t_dh_done_event = e; t_dh_done_rows = n_scored; }
-
 static thread_local cudaError_t t_last_cuda_error = cudaSuccess;
 void note_cuda_error(cudaError_t e) {
   t_last_cuda_error = e;
@@ -337,6 +330,11 @@ struct DwSink {
   float* const* shards; int world; int64_t shard_rows;
   int dW_dtype;             // GC_F32 / GC_BF16 (local dW only)
   const void* fwd_state;    // the forward's workspace (row list + compacted H reused), or NULL
+  // host_api.cu only: an event recorded right after the dH launch of the last NON-EMPTY chunk (dH is
+  // complete from there on: gc_grpo_step_host starts its device -> host copy of dH under the last dW
+  // contraction); dh_rows = scored rows of the batch (chunks past them are empty)
+  cudaEvent_t dh_done = nullptr;
+  int64_t dh_rows = 0;
 };
 
 int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
@@ -440,9 +438,8 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
     rows = w.rows; n_rows = w.n_rows;
   }
   GC_CUDA_TRY(cudaMemsetAsync(w.counters, 0, sizeof(uint32_t) * kTcCounters, st));
-  cudaEvent_t dh_done = gc::t_dh_done_event;
-  const int64_t dh_rows = compact ? gc::t_dh_done_rows : T;   // rows that reach the contractions
-  gc::t_dh_done_event = nullptr;
+  cudaEvent_t dh_done = sink.dh_done;
+  const int64_t dh_rows = compact ? sink.dh_rows : T;         // rows that reach the contractions
   int ci = 0;
   for (int64_t row0 = 0; row0 < T; row0 += chunk) {
     if (ci + kCountersPerChunk > kTcCounters) {
@@ -477,6 +474,27 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
 }
 
 }  // namespace
+
+namespace gc {
+// gc_grpo_loss_bwd with the dH-done event of gc_grpo_step_host (host_api.cu); not exported
+int grpo_loss_bwd_dh_event(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                           const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D,
+                           int64_t V, float temperature, const int32_t* cu_seqlens, int32_t R,
+                           const float* adv, const float* old_logp, const float* ref_logp,
+                           float clip_lo, float clip_hi, float beta, int agg, const float* logp,
+                           const float* lse, float grad_loss, void* dH, int64_t lddH, void* dW,
+                           int64_t lddW, int dW_dtype, int accumulate_dW, void* workspace,
+                           size_t workspace_bytes, void* cuda_stream, cudaEvent_t dh_done,
+                           int64_t dh_rows) {
+  if (dW_dtype != GC_F32 && dW_dtype != GC_BF16) return GC_ERR_DTYPE;
+  DwSink sink{dW, lddW, accumulate_dW, nullptr, 0, 0, dW_dtype, nullptr};
+  sink.dh_done = dh_done;
+  sink.dh_rows = dh_rows;
+  return loss_bwd_impl(H, ldH, W, ldW, dtype, targets, mask, T, D, V, temperature, cu_seqlens, R, adv,
+                       old_logp, ref_logp, clip_lo, clip_hi, beta, agg, logp, lse, grad_loss, dH, lddH,
+                       sink, 0, workspace, workspace_bytes, cuda_stream);
+}
+}  // namespace gc
 
 extern "C" {
 

@@ -9,7 +9,16 @@
 // the CUDA error behind the calling thread's last GC_ERR_CUDA (api.cu; gc_last_cuda_error)
 namespace gc {
 void note_cuda_error(cudaError_t e);
-void set_bwd_dh_done_event(cudaEvent_t e, int64_t n_scored);     // api.cu: see there
+// api.cu: gc_grpo_loss_bwd that records `dh_done` after the dH launch of the last non-empty chunk
+int grpo_loss_bwd_dh_event(const void* H, int64_t ldH, const void* W, int64_t ldW, int dtype,
+                           const int32_t* targets, const uint8_t* mask, int64_t T, int64_t D,
+                           int64_t V, float temperature, const int32_t* cu_seqlens, int32_t R,
+                           const float* adv, const float* old_logp, const float* ref_logp,
+                           float clip_lo, float clip_hi, float beta, int agg, const float* logp,
+                           const float* lse, float grad_loss, void* dH, int64_t lddH, void* dW,
+                           int64_t lddW, int dW_dtype, int accumulate_dW, void* workspace,
+                           size_t workspace_bytes, void* cuda_stream, cudaEvent_t dh_done,
+                           int64_t dh_rows);
 }
 
 #define GC_CUDA_TRY(expr)                         \

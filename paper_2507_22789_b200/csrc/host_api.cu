@@ -273,18 +273,15 @@ int gc_grpo_step_host(const void* H_host, const void* W, int64_t ldW, int dtype,
   // dH is complete after the last chunk's dH contraction: its copy back to the host runs on the
   // side stream under the last dW contraction (bf16 tcgen05 path; the SIMT path copies at the end)
   const bool overlap_dh = dtype == GC_BF16;
-  if (overlap_dh) {
-    int64_t n_scored = 0;          // host-side count: which chunk is the last non-empty one
+  int64_t n_scored = 0;            // host-side count: which chunk is the last non-empty one
+  if (overlap_dh)
     for (int64_t t = 0; t < T; ++t)
       n_scored += (targets_host[t] >= 0 && (!mask_host || mask_host[t] != 0)) ? 1 : 0;
-    gc::set_bwd_dh_done_event(cx->ev[kHostEvents - 1], n_scored);
-  }
-  const int bs = gc_grpo_loss_bwd(w.sg.H, D, W, ldW, dtype, w.sg.y, m, T, D, V, temperature, w.cu, R,
-                                  w.adv, w.old_lp, rf, clip_lo, clip_hi, beta, agg, w.sg.logp,
-                                  w.sg.lse, grad_loss, w.dH, D, dW, lddW, dW_dtype, accumulate_dW, 0,
-                                  nullptr, w.bwd, w.bwd_bytes, st);
-  gc::set_bwd_dh_done_event(nullptr, 0);
-  GC_TRY(bs);
+  GC_TRY(gc::grpo_loss_bwd_dh_event(w.sg.H, D, W, ldW, dtype, w.sg.y, m, T, D, V, temperature, w.cu, R,
+                                    w.adv, w.old_lp, rf, clip_lo, clip_hi, beta, agg, w.sg.logp,
+                                    w.sg.lse, grad_loss, w.dH, D, dW, lddW, dW_dtype, accumulate_dW,
+                                    w.bwd, w.bwd_bytes, st,
+                                    overlap_dh ? cx->ev[kHostEvents - 1] : nullptr, n_scored));
   const size_t dh_bytes = (size_t)T * (size_t)D * elem_bytes(dtype);
   if (overlap_dh) {
     GC_CUDA_TRY(cudaStreamWaitEvent(cx->cs, cx->ev[kHostEvents - 1], 0));

@@ -198,7 +198,9 @@ int gc_grpo_loss_fwd(const void* H, int64_t ldH, const void* W, int64_t ldW, int
  * bf16 dS chunk buffer (0 = library picks; must match the workspace query).
  * fwd_state (nullable): the workspace gc_grpo_loss_fwd was given for the SAME inputs, untouched
  * since; the backward then reuses the forward's row selection (a1: row list, compacted targets,
- * compacted H) instead of recomputing it.  It must not overlap `workspace`.
+ * compacted H) instead of recomputing it.  It must not overlap `workspace` (GC_ERR_ARG if it does).
+ * The library cannot tell whether the state still belongs to these inputs: a later forward with the
+ * same workspace overwrites it (the Python binding tracks that and then passes NULL).
  * workspace: gc_bwd_workspace_bytes(T, D, V, dtype, chunk_tokens, dW_dtype)
  * (= gc_workspace_bytes(GC_OP_LOSS_BWD, ...) for GC_F32). */
 size_t gc_bwd_workspace_bytes(int64_t T, int64_t D, int64_t V, int dtype, int64_t chunk_tokens,

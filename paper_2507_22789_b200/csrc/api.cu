@@ -378,6 +378,12 @@ int loss_bwd_impl(const void* H, int64_t ldH, const void* W, int64_t ldW, int dt
   if (!workspace || workspace_bytes < need) return GC_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 255) return GC_ERR_ALIGN;
   if (sink.fwd_state && (reinterpret_cast<uintptr_t>(sink.fwd_state) & 255)) return GC_ERR_ALIGN;
+  if (sink.fwd_state) {          // the forward's workspace must not overlap this call's scratch
+    const uintptr_t f0 = reinterpret_cast<uintptr_t>(sink.fwd_state);
+    const uintptr_t f1 = f0 + gc_workspace_bytes(GC_OP_LOSS_FWD, T, D, V, dtype, 0);
+    const uintptr_t w0 = reinterpret_cast<uintptr_t>(workspace), w1 = w0 + need;
+    if (f0 < w1 && w0 < f1) return GC_ERR_ARG;
+  }
   GC_TRY(check_arch());
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if (T == 0) {

@@ -875,6 +875,11 @@ def test_stale_forward_state_is_not_used(B):
     dH_b0, dW_b0 = B.gc_grpo_loss_bwd(*args_b)
     dH_b1, dW_b1 = B.gc_grpo_loss_bwd(*args_b, fwd_state=fb["state"])     # latest: used
     assert torch.equal(dH_b0, dH_b1) and torch.equal(dW_b0, dW_b1)
+    # the C call refuses a forward state that overlaps its own workspace (a raw tensor bypasses the
+    # binding's bookkeeping: here the backward's cached workspace itself)
+    nb = int(B.lib().gc_bwd_workspace_bytes(bb.T, wb.D, wb.V, B.GC_BF16, 0, B.GC_F32))
+    with pytest.raises(B.GcoreError, match="GC_ERR_ARG"):
+        B.gc_grpo_loss_bwd(*args_b, fwd_state=B.workspace(nb, bb.H.device))
 
 
 def test_host_entry_points_banded_copy_and_training_step(B):
